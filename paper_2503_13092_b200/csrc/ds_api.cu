@@ -1,0 +1,424 @@
+// C ABI of libds (include/ds.h): handle, argument checks, workspace carving, launch order, host-buffer path.
+// No arithmetic of the method lives here.
+#include <new>
+
+#include "ds_common.cuh"
+
+using namespace ds;
+
+struct ds_handle {
+    int device;
+    bool has_geom;
+    ds_geometry geom;
+    DevMlp *d_mlp;
+    // arena of the *_host path, grown on demand
+    unsigned char *arena;
+    size_t arena_bytes;
+};
+
+namespace {
+
+struct DeviceGuard {
+    int prev = -1;
+    bool ok = true;
+    explicit DeviceGuard(int dev)
+    {
+        if (cudaGetDevice(&prev) != cudaSuccess) { ok = false; return; }
+        if (prev != dev && cudaSetDevice(dev) != cudaSuccess) ok = false;
+        if (prev == dev) prev = -1;
+    }
+    ~DeviceGuard()
+    {
+        if (prev >= 0) cudaSetDevice(prev);
+    }
+};
+
+inline size_t up256(size_t v) { return (v + 255) & ~(size_t)255; }
+
+int n_bins_of(const ds_geometry &g) { return 4 * g.n_sectors_y * kXBins; }
+
+bool make_const(const ds_geometry &g, const ds_params *p, DevConst &c)
+{
+    if (!p || p->struct_size != sizeof(ds_params)) return false;
+    if (p->max_first_hits < 1 || p->max_first_hits > DS_MAX_FIRST_HITS) return false;
+    double dmax = 0.0;
+    for (int l = 0; l < 4; ++l) {
+        c.z_layer[l] = g.z_layer[l];
+        c.dxdy[l] = g.dxdy[l];
+        c.zmag_c[l] = g.zmag_c[l];
+        const double a = g.dxdy[l] < 0 ? -g.dxdy[l] : g.dxdy[l];
+        if (a > dmax) dmax = a;
+    }
+    c.y0 = -g.y_half;
+    c.inv_h = 1.0 / g.sector_height;
+    c.z_seed = g.z_seed;
+    c.z_ref = g.z_ref;
+    c.kick = g.kick;
+    c.inv_kick = 1.0 / g.kick;
+    c.n_sectors = g.n_sectors_y;
+    c.n_bins = n_bins_of(g);
+    const float X = (float)(g.x_half + g.y_half * dmax);
+    c.xb_off = X;
+    c.xb_scale = (float)kXBins / (2.0f * X);
+    c.w0_a = p->w0_a; c.w0_b = p->w0_b; c.w0_max = p->w0_max; c.w1_a = p->w1_a; c.w1_b = p->w1_b;
+    c.y_tol = p->y_tol; c.w_mag = p->w_mag; c.chi2ndf_max = p->chi2ndf_max; c.miss_penalty = p->miss_penalty;
+    c.min_hits = p->min_hits; c.max_first = p->max_first_hits;
+    c.mlp_thr = p->mlp_thr; c.mlp_keep_above = p->mlp_keep_above; c.pad_ = 0;
+    c.doca_max = p->doca_max; c.zv_min = p->zv_min; c.zv_max = p->zv_max;
+    c.m_pi = p->m_pi; c.m_p = p->m_p; c.m_ks = p->m_ks; c.m_lambda = p->m_lambda;
+    c.dm_ks = p->dm_ks; c.dm_lambda = p->dm_lambda; c.n2_min = p->n2_min;
+    return true;
+}
+
+bool hits_ok(const ds_hits *h)
+{
+    if (!h || h->n < 0 || h->n >= ((int64_t)1 << 31)) return false;
+    return h->n == 0 || (h->x0 && h->z && h->ymin && h->ymax && h->w && h->id);
+}
+
+bool seeds_ok(const ds_seeds *s)
+{
+    if (!s || s->n < 0 || s->n >= ((int64_t)1 << 31)) return false;
+    return s->n == 0 || (s->x && s->y && s->tx && s->ty && s->qop);
+}
+
+bool tracks_ok(const ds_tracks *t, int64_t n)
+{
+    if (!t || t->n != n) return false;
+    return n == 0 || (t->x && t->y && t->tx && t->ty && t->qop && t->chi2 && t->score && t->nhits && t->hit &&
+                      t->found && t->keep && (reinterpret_cast<uintptr_t>(t->hit) & 15) == 0);
+}
+
+bool vertices_ok(const ds_vertices *v)
+{
+    if (!v || v->capacity < 0 || !v->n_per_event || !v->offsets || !v->overflow) return false;
+    return v->capacity == 0 ||
+           (v->evt && v->ia && v->ib && v->x && v->y && v->z && v->doca && v->m_pipi && v->m_ppi && v->flags);
+}
+
+// carve the S1 arrays out of a workspace
+size_t layout_bytes(int n_bins, int n_events, int64_t n_hits)
+{
+    const size_t nh = (size_t)(n_hits > 0 ? n_hits : 1) + 4;
+    return 7 * up256(4 * nh) + up256(4 * (size_t)(n_events > 0 ? n_events : 1) * (n_bins + 1));
+}
+
+void carve_layout(void *ws, int n_bins, int n_events, int64_t n_hits, LayoutPtrs &L)
+{
+    const size_t nh = (size_t)(n_hits > 0 ? n_hits : 1) + 4;
+    unsigned char *w = static_cast<unsigned char *>(ws);
+    auto take = [&](size_t bytes) { unsigned char *r = w; w += up256(bytes); return r; };
+    L.sx0 = reinterpret_cast<float *>(take(4 * nh));
+    L.sz = reinterpret_cast<float *>(take(4 * nh));
+    L.symin = reinterpret_cast<float *>(take(4 * nh));
+    L.symax = reinterpret_cast<float *>(take(4 * nh));
+    L.sw = reinterpret_cast<float *>(take(4 * nh));
+    L.sid = reinterpret_cast<int32_t *>(take(4 * nh));
+    L.perm = reinterpret_cast<int32_t *>(take(4 * nh));
+    L.bin_offsets = reinterpret_cast<int32_t *>(take(4 * (size_t)(n_events > 0 ? n_events : 1) * (n_bins + 1)));
+}
+
+void set_inputs(LayoutPtrs &L, const ds_hits *hits)
+{
+    L.x0 = hits->x0; L.z = hits->z; L.ymin = hits->ymin; L.ymax = hits->ymax; L.w = hits->w; L.id = hits->id;
+}
+
+}  // namespace
+
+extern "C" {
+
+int ds_version(void) { return DS_VERSION; }
+
+const char *ds_error_string(int code)
+{
+    switch (code) {
+        case DS_OK: return "ok";
+        case DS_E_ARG: return "invalid argument";
+        case DS_E_NOGEOM: return "geometry not uploaded";
+        case DS_E_WORKSPACE: return "workspace missing or too small";
+        case DS_E_CUDA: return "CUDA error";
+        default: return "unknown error";
+    }
+}
+
+int ds_create(ds_handle **h, int cuda_device)
+{
+    if (!h) return DS_E_ARG;
+    *h = nullptr;
+    int n = 0;
+    if (cudaGetDeviceCount(&n) != cudaSuccess || cuda_device < 0 || cuda_device >= n) {
+        cudaGetLastError();
+        return DS_E_CUDA;
+    }
+    DeviceGuard guard(cuda_device);
+    if (!guard.ok) return DS_E_CUDA;
+    ds_handle *p = new (std::nothrow) ds_handle();
+    if (!p) return DS_E_CUDA;
+    p->device = cuda_device;
+    p->has_geom = false;
+    p->arena = nullptr;
+    p->arena_bytes = 0;
+    if (cudaMalloc(&p->d_mlp, sizeof(DevMlp)) != cudaSuccess) {
+        cudaGetLastError();
+        delete p;
+        return DS_E_CUDA;
+    }
+    *h = p;
+    return DS_OK;
+}
+
+void ds_destroy(ds_handle *h)
+{
+    if (!h) return;
+    DeviceGuard guard(h->device);
+    if (h->d_mlp) cudaFree(h->d_mlp);
+    if (h->arena) cudaFree(h->arena);
+    delete h;
+}
+
+int ds_upload_geometry(ds_handle *h, const ds_geometry *g, const ds_mlp *m)
+{
+    if (!h || !g || !m) return DS_E_ARG;
+    if (g->struct_size != sizeof(ds_geometry) || m->struct_size != sizeof(ds_mlp)) return DS_E_ARG;
+    if (g->n_sectors_y < 1 || g->n_sectors_y > DS_MAX_SECTORS || !(g->sector_height > 0.0) || !(g->x_half > 0.0) ||
+        !(g->y_half > 0.0) || g->kick == 0.0)
+        return DS_E_ARG;
+    DeviceGuard guard(h->device);
+    if (!guard.ok) return DS_E_CUDA;
+    DevMlp host;
+    for (int j = 0; j < DS_MLP_H1; ++j) {
+        for (int i = 0; i < DS_MLP_IN; ++i) host.W1[j * DS_MLP_IN + i] = m->W1[j][i];
+        host.b1[j] = m->b1[j];
+    }
+    for (int j = 0; j < DS_MLP_H2; ++j) {
+        for (int i = 0; i < DS_MLP_H1; ++i) host.W2[j * DS_MLP_H1 + i] = m->W2[j][i];
+        host.b2[j] = m->b2[j];
+        host.W3[j] = m->W3[j];
+    }
+    host.b3 = m->b3;
+    for (int i = 0; i < DS_MLP_IN; ++i) { host.mu[i] = m->mu[i]; host.inv_sigma[i] = m->inv_sigma[i]; }
+    host.pad_[0] = host.pad_[1] = host.pad_[2] = 0.f;
+    if (cudaMemcpy(h->d_mlp, &host, sizeof host, cudaMemcpyHostToDevice) != cudaSuccess) {
+        cudaGetLastError();
+        return DS_E_CUDA;
+    }
+    h->geom = *g;
+    h->has_geom = true;
+    return DS_OK;
+}
+
+int ds_layout(ds_handle *h, const ds_hits *hits, const int32_t *hit_offsets, int n_events, const ds_params *p,
+              ds_layout_out *out, void *cuda_stream)
+{
+    if (!h || !hits_ok(hits) || !hit_offsets || n_events < 0 || !out) return DS_E_ARG;
+    if (!h->has_geom) return DS_E_NOGEOM;
+    DevConst c;
+    if (!make_const(h->geom, p, c)) return DS_E_ARG;
+    if (out->n != hits->n || !out->bin_offsets) return DS_E_ARG;
+    if (hits->n > 0 && !(out->x0 && out->z && out->ymin && out->ymax && out->w && out->id && out->perm)) return DS_E_ARG;
+    DeviceGuard guard(h->device);
+    if (!guard.ok) return DS_E_CUDA;
+    LayoutPtrs L;
+    set_inputs(L, hits);
+    L.sx0 = out->x0; L.sz = out->z; L.symin = out->ymin; L.symax = out->ymax; L.sw = out->w; L.sid = out->id;
+    L.perm = out->perm; L.bin_offsets = out->bin_offsets;
+    if (launch_layout(c, L, hit_offsets, n_events, p->max_event_hits_hint, (cudaStream_t)cuda_stream) != cudaSuccess) {
+        cudaGetLastError();
+        return DS_E_CUDA;
+    }
+    return DS_OK;
+}
+
+int ds_extrapolate(ds_handle *h, const ds_seeds *seeds, const ds_params *p, double *out, void *cuda_stream)
+{
+    if (!h || !seeds_ok(seeds) || (!out && seeds->n > 0)) return DS_E_ARG;
+    if (!h->has_geom) return DS_E_NOGEOM;
+    DevConst c;
+    if (!make_const(h->geom, p, c)) return DS_E_ARG;
+    DeviceGuard guard(h->device);
+    if (!guard.ok) return DS_E_CUDA;
+    if (launch_extrapolate(c, *seeds, out, (cudaStream_t)cuda_stream) != cudaSuccess) {
+        cudaGetLastError();
+        return DS_E_CUDA;
+    }
+    return DS_OK;
+}
+
+size_t ds_workspace_bytes(const ds_handle *h, int n_events, int64_t n_hits, int64_t n_seeds)
+{
+    (void)n_seeds;
+    const int nb = (h && h->has_geom) ? n_bins_of(h->geom) : 4 * DS_MAX_SECTORS * kXBins;
+    return layout_bytes(nb, n_events, n_hits);
+}
+
+int ds_ghost_killer(ds_handle *h, const ds_seeds *seeds, const ds_params *p, ds_tracks *trk, void *cuda_stream)
+{
+    if (!h || !seeds_ok(seeds) || !tracks_ok(trk, seeds ? seeds->n : 0)) return DS_E_ARG;
+    if (!h->has_geom) return DS_E_NOGEOM;
+    DevConst c;
+    if (!make_const(h->geom, p, c)) return DS_E_ARG;
+    DeviceGuard guard(h->device);
+    if (!guard.ok) return DS_E_CUDA;
+    if (launch_mlp(c, h->d_mlp, *seeds, *trk, (cudaStream_t)cuda_stream) != cudaSuccess) {
+        cudaGetLastError();
+        return DS_E_CUDA;
+    }
+    return DS_OK;
+}
+
+int ds_reconstruct(ds_handle *h, const ds_hits *hits, const ds_seeds *seeds, const int32_t *hit_offsets,
+                   const int32_t *seed_offsets, int n_events, const ds_params *p, ds_tracks *out, void *workspace,
+                   size_t workspace_bytes, void *cuda_stream)
+{
+    if (!h || !hits_ok(hits) || !seeds_ok(seeds) || !hit_offsets || !seed_offsets || n_events < 0) return DS_E_ARG;
+    if (!tracks_ok(out, seeds->n)) return DS_E_ARG;
+    if (!h->has_geom) return DS_E_NOGEOM;
+    DevConst c;
+    if (!make_const(h->geom, p, c)) return DS_E_ARG;
+    if (!workspace || (reinterpret_cast<uintptr_t>(workspace) & 255) != 0 ||
+        workspace_bytes < layout_bytes(c.n_bins, n_events, hits->n))
+        return DS_E_WORKSPACE;
+    DeviceGuard guard(h->device);
+    if (!guard.ok) return DS_E_CUDA;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    LayoutPtrs L;
+    set_inputs(L, hits);
+    carve_layout(workspace, c.n_bins, n_events, hits->n, L);
+    cudaError_t err = launch_layout(c, L, hit_offsets, n_events, p->max_event_hits_hint, st);
+    if (err == cudaSuccess) err = launch_track(c, L, *seeds, hit_offsets, seed_offsets, n_events, *out, st);
+    if (err == cudaSuccess) err = launch_mlp(c, h->d_mlp, *seeds, *out, st);
+    if (err != cudaSuccess) {
+        cudaGetLastError();
+        return DS_E_CUDA;
+    }
+    return DS_OK;
+}
+
+size_t ds_vertex_workspace_bytes(const ds_handle *h, int n_events, int64_t n_seeds)
+{
+    (void)h;
+    return vertex_workspace_bytes(n_events, n_seeds);
+}
+
+int ds_vertex(ds_handle *h, const ds_tracks *trk, const int32_t *seed_offsets, int n_events, const ds_params *p,
+              ds_vertices *out, void *workspace, size_t workspace_bytes, void *cuda_stream)
+{
+    if (!h || !trk || trk->n < 0 || !seed_offsets || n_events < 0 || !vertices_ok(out)) return DS_E_ARG;
+    if (trk->n > 0 && !(trk->x && trk->y && trk->tx && trk->ty && trk->qop && trk->keep)) return DS_E_ARG;
+    if (!h->has_geom) return DS_E_NOGEOM;
+    DevConst c;
+    if (!make_const(h->geom, p, c)) return DS_E_ARG;
+    if (!workspace || (reinterpret_cast<uintptr_t>(workspace) & 255) != 0 ||
+        workspace_bytes < vertex_workspace_bytes(n_events, trk->n))
+        return DS_E_WORKSPACE;
+    DeviceGuard guard(h->device);
+    if (!guard.ok) return DS_E_CUDA;
+    if (launch_vertex(c, *trk, seed_offsets, n_events, *out, workspace, (cudaStream_t)cuda_stream) != cudaSuccess) {
+        cudaGetLastError();
+        return DS_E_CUDA;
+    }
+    return DS_OK;
+}
+
+int ds_process_host(ds_handle *h, const ds_hits *hits, const ds_seeds *seeds, const int32_t *hit_offsets,
+                    const int32_t *seed_offsets, int n_events, const ds_params *p, ds_tracks *out_tracks,
+                    ds_vertices *out_vertices, int64_t *n_vertices_total, void *cuda_stream)
+{
+    if (!h || !hits_ok(hits) || !seeds_ok(seeds) || !hit_offsets || !seed_offsets || n_events < 0) return DS_E_ARG;
+    if (!tracks_ok(out_tracks, seeds->n) || !vertices_ok(out_vertices)) return DS_E_ARG;
+    if (!h->has_geom) return DS_E_NOGEOM;
+    DevConst c;
+    if (!make_const(h->geom, p, c)) return DS_E_ARG;
+    DeviceGuard guard(h->device);
+    if (!guard.ok) return DS_E_CUDA;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const size_t nh = (size_t)hits->n, ns = (size_t)seeds->n, ne = (size_t)n_events, cap = (size_t)out_vertices->capacity;
+    const size_t ws_rec = layout_bytes(c.n_bins, n_events, hits->n), ws_vtx = vertex_workspace_bytes(n_events, seeds->n);
+    const size_t need = 6 * up256(4 * nh + 4) + 6 * up256(4 * ns + 4) + 2 * up256(4 * (ne + 1)) + 10 * up256(4 * ns + 4) +
+                        up256(16 * ns + 16) + 10 * up256(4 * cap + 4) + up256(4 * ne + 4) + up256(8 * (ne + 1)) + 256 +
+                        ws_rec + ws_vtx;
+    if (need > h->arena_bytes) {
+        if (h->arena) cudaFree(h->arena);
+        h->arena = nullptr;
+        h->arena_bytes = 0;
+        const size_t want = need + need / 8;
+        if (cudaMalloc(&h->arena, want) != cudaSuccess) {
+            cudaGetLastError();
+            return DS_E_CUDA;
+        }
+        h->arena_bytes = want;
+    }
+    unsigned char *w = h->arena;
+    auto take = [&](size_t bytes) { unsigned char *r = w; w += up256(bytes); return r; };
+    cudaError_t err = cudaSuccess;
+    auto h2d = [&](const void *src, size_t bytes) -> void * {
+        void *d = take(bytes + 4);
+        if (bytes && err == cudaSuccess) err = cudaMemcpyAsync(d, src, bytes, cudaMemcpyHostToDevice, st);
+        return d;
+    };
+    ds_hits dh;
+    dh.n = hits->n;
+    dh.x0 = (const float *)h2d(hits->x0, 4 * nh); dh.z = (const float *)h2d(hits->z, 4 * nh);
+    dh.ymin = (const float *)h2d(hits->ymin, 4 * nh); dh.ymax = (const float *)h2d(hits->ymax, 4 * nh);
+    dh.w = (const float *)h2d(hits->w, 4 * nh); dh.id = (const int32_t *)h2d(hits->id, 4 * nh);
+    ds_seeds dsd;
+    dsd.n = seeds->n;
+    dsd.x = (const float *)h2d(seeds->x, 4 * ns); dsd.y = (const float *)h2d(seeds->y, 4 * ns);
+    dsd.tx = (const float *)h2d(seeds->tx, 4 * ns); dsd.ty = (const float *)h2d(seeds->ty, 4 * ns);
+    dsd.qop = (const float *)h2d(seeds->qop, 4 * ns);
+    {
+        void *d = h2d(seeds->chi2, seeds->chi2 ? 4 * ns : 0);
+        dsd.chi2 = seeds->chi2 ? (const float *)d : nullptr;
+    }
+    const int32_t *d_hoff = (const int32_t *)h2d(hit_offsets, 4 * (ne + 1));
+    const int32_t *d_soff = (const int32_t *)h2d(seed_offsets, 4 * (ne + 1));
+    ds_tracks dt;
+    dt.n = seeds->n;
+    dt.x = (float *)take(4 * ns + 4); dt.y = (float *)take(4 * ns + 4); dt.tx = (float *)take(4 * ns + 4);
+    dt.ty = (float *)take(4 * ns + 4); dt.qop = (float *)take(4 * ns + 4); dt.chi2 = (float *)take(4 * ns + 4);
+    dt.score = (float *)take(4 * ns + 4); dt.nhits = (int32_t *)take(4 * ns + 4); dt.found = (int32_t *)take(4 * ns + 4);
+    dt.keep = (int32_t *)take(4 * ns + 4); dt.hit = (int32_t *)take(16 * ns + 16);
+    ds_vertices dv;
+    dv.capacity = out_vertices->capacity;
+    dv.evt = (int32_t *)take(4 * cap + 4); dv.ia = (int32_t *)take(4 * cap + 4); dv.ib = (int32_t *)take(4 * cap + 4);
+    dv.x = (float *)take(4 * cap + 4); dv.y = (float *)take(4 * cap + 4); dv.z = (float *)take(4 * cap + 4);
+    dv.doca = (float *)take(4 * cap + 4); dv.m_pipi = (float *)take(4 * cap + 4); dv.m_ppi = (float *)take(4 * cap + 4);
+    dv.flags = (int32_t *)take(4 * cap + 4);
+    dv.n_per_event = (int32_t *)take(4 * ne + 4);
+    dv.offsets = (int64_t *)take(8 * (ne + 1));
+    dv.overflow = (int32_t *)take(256);
+    void *wrec = take(ws_rec), *wvtx = take(ws_vtx);
+    if (err != cudaSuccess) { cudaGetLastError(); return DS_E_CUDA; }
+
+    LayoutPtrs L;
+    set_inputs(L, &dh);
+    carve_layout(wrec, c.n_bins, n_events, hits->n, L);
+    err = launch_layout(c, L, d_hoff, n_events, p->max_event_hits_hint, st);
+    if (err == cudaSuccess) err = launch_track(c, L, dsd, d_hoff, d_soff, n_events, dt, st);
+    if (err == cudaSuccess) err = launch_mlp(c, h->d_mlp, dsd, dt, st);
+    if (err == cudaSuccess) err = launch_vertex(c, dt, d_soff, n_events, dv, wvtx, st);
+    auto d2h = [&](void *dst, const void *src, size_t bytes) {
+        if (bytes && err == cudaSuccess) err = cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToHost, st);
+    };
+    d2h(out_vertices->offsets, dv.offsets, 8 * (ne + 1));
+    d2h(out_vertices->n_per_event, dv.n_per_event, 4 * ne);
+    d2h(out_vertices->overflow, dv.overflow, 4);
+    d2h(out_tracks->x, dt.x, 4 * ns); d2h(out_tracks->y, dt.y, 4 * ns); d2h(out_tracks->tx, dt.tx, 4 * ns);
+    d2h(out_tracks->ty, dt.ty, 4 * ns); d2h(out_tracks->qop, dt.qop, 4 * ns); d2h(out_tracks->chi2, dt.chi2, 4 * ns);
+    d2h(out_tracks->score, dt.score, 4 * ns); d2h(out_tracks->nhits, dt.nhits, 4 * ns);
+    d2h(out_tracks->found, dt.found, 4 * ns); d2h(out_tracks->keep, dt.keep, 4 * ns); d2h(out_tracks->hit, dt.hit, 16 * ns);
+    if (err == cudaSuccess) err = cudaStreamSynchronize(st);
+    if (err != cudaSuccess) { cudaGetLastError(); return DS_E_CUDA; }
+    const int64_t total = out_vertices->offsets[n_events];
+    if (n_vertices_total) *n_vertices_total = total;
+    const size_t nv = (size_t)(total < out_vertices->capacity ? total : out_vertices->capacity);
+    d2h(out_vertices->evt, dv.evt, 4 * nv); d2h(out_vertices->ia, dv.ia, 4 * nv); d2h(out_vertices->ib, dv.ib, 4 * nv);
+    d2h(out_vertices->x, dv.x, 4 * nv); d2h(out_vertices->y, dv.y, 4 * nv); d2h(out_vertices->z, dv.z, 4 * nv);
+    d2h(out_vertices->doca, dv.doca, 4 * nv); d2h(out_vertices->m_pipi, dv.m_pipi, 4 * nv);
+    d2h(out_vertices->m_ppi, dv.m_ppi, 4 * nv); d2h(out_vertices->flags, dv.flags, 4 * nv);
+    if (err == cudaSuccess) err = cudaStreamSynchronize(st);
+    if (err != cudaSuccess) { cudaGetLastError(); return DS_E_CUDA; }
+    return DS_OK;
+}
+
+}  // extern "C"

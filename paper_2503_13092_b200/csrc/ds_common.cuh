@@ -1,0 +1,94 @@
+// Shared device-side definitions of libds (CUDA, sm_100a).  Not part of the C ABI.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/ds.h"
+
+namespace ds {
+
+constexpr int kLayers = 4;
+constexpr int kXBins = DS_XBINS;
+constexpr int kMaxFirst = DS_MAX_FIRST_HITS;
+constexpr int kIdLayerShift = 24;
+constexpr int kIdSectorShift = 20;
+constexpr int kIdSeqMask = (1 << 20) - 1;
+
+// Geometry + parameters as the kernels see them (passed by value as a __grid_constant__ kernel argument).
+struct DevConst {
+    // geometry
+    double z_layer[4], dxdy[4];
+    double y0;            // -y_half: lower edge of sector 0
+    double inv_h;         // 1 / sector_height
+    double z_seed, z_ref, zmag_c[4], kick, inv_kick;
+    int n_sectors, n_bins; // n_bins = 4 * n_sectors * kXBins
+    float xb_off, xb_scale; // xbin(x0) = clamp(floor((x0 + xb_off) * xb_scale))
+    // parameters
+    double w0_a, w0_b, w0_max, w1_a, w1_b, y_tol, w_mag, chi2ndf_max, miss_penalty;
+    int min_hits, max_first;
+    double mlp_thr;
+    int mlp_keep_above, pad_;
+    double doca_max, zv_min, zv_max, m_pi, m_p, m_ks, m_lambda, dm_ks, dm_lambda, n2_min;
+};
+
+// Device copy of the ghost-killer weights (global memory, staged to shared memory by the kernel).
+struct DevMlp {
+    float W1[DS_MLP_H1 * DS_MLP_IN], b1[DS_MLP_H1];
+    float W2[DS_MLP_H2 * DS_MLP_H1], b2[DS_MLP_H2];
+    float W3[DS_MLP_H2], b3;
+    float mu[DS_MLP_IN], inv_sigma[DS_MLP_IN];
+    float pad_[3];
+};
+static_assert(sizeof(DevMlp) % 16 == 0, "DevMlp is copied as float4");
+
+__device__ __forceinline__ int id_layer(int id) { return (id >> kIdLayerShift) & 3; }
+__device__ __forceinline__ int id_sector(int id) { return (id >> kIdSectorShift) & 15; }
+
+// x0 slice of a hit inside its (layer, sector) bin.  fp32 and monotone non-decreasing in x0, so the slices respect
+// the x0 order and a window [lo, hi] in x0 maps to the slice range [xbin(lo'), xbin(hi')] for any lo' <= lo, hi' >= hi.
+__device__ __forceinline__ int xbin(float x0, float off, float scale)
+{
+    float t = floorf((x0 + off) * scale);
+    t = fminf(fmaxf(t, 0.0f), (float)(kXBins - 1));
+    return (int)t;
+}
+
+// Order-preserving map float -> uint32 (-0.0 is first folded onto +0.0 so that it compares equal, like IEEE ==).
+__device__ __forceinline__ uint32_t float_key(float x)
+{
+    uint32_t u = __float_as_uint(x + 0.0f);
+    return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
+}
+
+__device__ __forceinline__ unsigned lanemask_lt()
+{
+    unsigned m;
+    asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m));
+    return m;
+}
+
+// ---- launchers (host side, defined in the .cu files; all enqueue on `st` and return the launch error) ------------
+struct LayoutPtrs {
+    const float *x0, *z, *ymin, *ymax, *w;
+    const int32_t *id;
+    float *sx0, *sz, *symin, *symax, *sw;
+    int32_t *sid, *perm, *bin_offsets;
+};
+
+cudaError_t launch_layout(const DevConst &c, const LayoutPtrs &p, const int32_t *hit_offsets, int n_events,
+                          int max_event_hits_hint, cudaStream_t st);
+
+cudaError_t launch_extrapolate(const DevConst &c, const ds_seeds &seeds, double *out, cudaStream_t st);
+
+cudaError_t launch_track(const DevConst &c, const LayoutPtrs &lay, const ds_seeds &seeds, const int32_t *hit_offsets,
+                         const int32_t *seed_offsets, int n_events, const ds_tracks &out, cudaStream_t st);
+
+cudaError_t launch_mlp(const DevConst &c, const DevMlp *mlp, const ds_seeds &seeds, const ds_tracks &trk,
+                       cudaStream_t st);
+
+cudaError_t launch_vertex(const DevConst &c, const ds_tracks &trk, const int32_t *seed_offsets, int n_events,
+                          const ds_vertices &out, void *workspace, cudaStream_t st);
+size_t vertex_workspace_bytes(int n_events, int64_t n_seeds);
+
+}  // namespace ds

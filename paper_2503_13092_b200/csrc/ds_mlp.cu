@@ -1,0 +1,115 @@
+// S7 / K4: ghost-killer feed-forward network (inputs = downstream state (x, y, tx, ty, q/p, chi2) + SciFi
+// (q/p, chi2); ReLU hidden layers, sigmoid output).  Architecture 8 -> 32 -> 16 -> 1 from BASELINE cfg0, fixed at
+// compile time so that the activations live in registers ("static structs").
+//
+// Thread per seed slot, weights staged once per block in shared memory and read as broadcast float4.  fp32 FMA on
+// CUDA cores: the contraction per track is [1x8][8x32] + [1x32][32x16] + [1x16][16x1] = 784 MAC -- far too thin for
+// tensor cores.  IEEE expf and division (no fast-math intrinsics, unlike P:157: parity bound is 1e-4).  A score within
+// 1e-3 relative of the threshold is re-evaluated in fp64 so that the keep decision equals an fp64 evaluation.
+#include "ds_common.cuh"
+
+namespace ds {
+
+constexpr int kMlpThreads = 128;
+
+// fp64 evaluation for the rare score that sits on the threshold: rolled loops, out of line (keeps the fp32 path lean)
+__device__ __noinline__ double mlp_forward_f64(const DevMlp &m, const float *v)
+{
+    double f[DS_MLP_IN], h1[DS_MLP_H1], h2[DS_MLP_H2];
+    for (int i = 0; i < DS_MLP_IN; ++i) f[i] = ((double)v[i] - (double)m.mu[i]) * (double)m.inv_sigma[i];
+#pragma unroll 1
+    for (int j = 0; j < DS_MLP_H1; ++j) {
+        double t = (double)m.b1[j];
+#pragma unroll 1
+        for (int i = 0; i < DS_MLP_IN; ++i) t += (double)m.W1[j * DS_MLP_IN + i] * f[i];
+        h1[j] = t > 0.0 ? t : 0.0;
+    }
+#pragma unroll 1
+    for (int j = 0; j < DS_MLP_H2; ++j) {
+        double t = (double)m.b2[j];
+#pragma unroll 1
+        for (int i = 0; i < DS_MLP_H1; ++i) t += (double)m.W2[j * DS_MLP_H1 + i] * h1[i];
+        h2[j] = t > 0.0 ? t : 0.0;
+    }
+    double t = (double)m.b3;
+#pragma unroll 1
+    for (int i = 0; i < DS_MLP_H2; ++i) t += (double)m.W3[i] * h2[i];
+    return t;
+}
+
+template <typename T>
+__device__ __forceinline__ T mlp_forward(const DevMlp &m, const float (&v)[DS_MLP_IN])
+{
+    T f[DS_MLP_IN], h1[DS_MLP_H1], h2[DS_MLP_H2];
+#pragma unroll
+    for (int i = 0; i < DS_MLP_IN; ++i) f[i] = ((T)v[i] - (T)m.mu[i]) * (T)m.inv_sigma[i];
+#pragma unroll
+    for (int j = 0; j < DS_MLP_H1; ++j) {
+        T t = (T)m.b1[j];
+        const float4 *w = reinterpret_cast<const float4 *>(m.W1 + j * DS_MLP_IN);
+#pragma unroll
+        for (int i = 0; i < DS_MLP_IN / 4; ++i) {
+            const float4 q = w[i];
+            t += (T)q.x * f[4 * i] + (T)q.y * f[4 * i + 1] + (T)q.z * f[4 * i + 2] + (T)q.w * f[4 * i + 3];
+        }
+        h1[j] = t > (T)0 ? t : (T)0;
+    }
+#pragma unroll
+    for (int j = 0; j < DS_MLP_H2; ++j) {
+        T t = (T)m.b2[j];
+        const float4 *w = reinterpret_cast<const float4 *>(m.W2 + j * DS_MLP_H1);
+#pragma unroll
+        for (int i = 0; i < DS_MLP_H1 / 4; ++i) {
+            const float4 q = w[i];
+            t += (T)q.x * h1[4 * i] + (T)q.y * h1[4 * i + 1] + (T)q.z * h1[4 * i + 2] + (T)q.w * h1[4 * i + 3];
+        }
+        h2[j] = t > (T)0 ? t : (T)0;
+    }
+    T t = (T)m.b3;
+#pragma unroll
+    for (int i = 0; i < DS_MLP_H2; ++i) t += (T)m.W3[i] * h2[i];
+    return t;
+}
+
+__global__ void __launch_bounds__(kMlpThreads)
+k_mlp(const __grid_constant__ DevConst c, const DevMlp *__restrict__ gm, const ds_seeds seeds, const ds_tracks trk)
+{
+    __shared__ __align__(16) DevMlp m;
+    {
+        const float4 *src = reinterpret_cast<const float4 *>(gm);
+        float4 *dst = reinterpret_cast<float4 *>(&m);
+        for (int i = threadIdx.x; i < (int)(sizeof(DevMlp) / 16); i += kMlpThreads) dst[i] = src[i];
+    }
+    __syncthreads();
+    const int64_t s = (int64_t)blockIdx.x * kMlpThreads + threadIdx.x;
+    if (s >= trk.n) return;
+    float score = 0.f;
+    int keep = 0;
+    if (trk.found[s]) {
+        float v[DS_MLP_IN];
+        v[0] = trk.x[s]; v[1] = trk.y[s]; v[2] = trk.tx[s]; v[3] = trk.ty[s]; v[4] = trk.qop[s]; v[5] = trk.chi2[s];
+        v[6] = seeds.qop[s];
+        v[7] = seeds.chi2 ? seeds.chi2[s] : 0.f;
+        const float t = mlp_forward<float>(m, v);
+        score = 1.0f / (1.0f + expf(-t));
+        double sd = (double)score;
+        if (fabs(sd - c.mlp_thr) <= 1e-3 * fabs(c.mlp_thr)) {
+            const double td = mlp_forward_f64(m, v);
+            sd = 1.0 / (1.0 + exp(-td));
+            score = (float)sd;
+        }
+        keep = c.mlp_keep_above ? (sd > c.mlp_thr) : (sd < c.mlp_thr);
+    }
+    trk.score[s] = score;
+    trk.keep[s] = keep;
+}
+
+cudaError_t launch_mlp(const DevConst &c, const DevMlp *mlp, const ds_seeds &seeds, const ds_tracks &trk,
+                       cudaStream_t st)
+{
+    if (trk.n <= 0) return cudaSuccess;
+    k_mlp<<<(unsigned)((trk.n + kMlpThreads - 1) / kMlpThreads), kMlpThreads, 0, st>>>(c, mlp, seeds, trk);
+    return cudaGetLastError();
+}
+
+}  // namespace ds

@@ -1,0 +1,455 @@
+"""Thin ctypes binding of libds (include/ds.h): argument marshalling only, every step runs in the CUDA kernels.
+
+Functions carry the C names (ds_create, ds_upload_geometry, ds_layout, ds_extrapolate, ds_reconstruct,
+ds_ghost_killer, ds_vertex, ds_process_host); `Downstream` bundles a handle with its geometry / parameters and
+allocates outputs and workspaces as torch tensors.  torch is used for device memory and streams only.
+
+There is no CPU fallback: if libds.so is missing it is built with nvcc, and if that fails, or there is no CUDA
+device, the calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as ct
+import os
+
+import numpy as np
+
+from . import build as _build
+
+DS_OK, DS_E_ARG, DS_E_NOGEOM, DS_E_WORKSPACE, DS_E_CUDA = 0, -1, -2, -3, -4
+DS_MLP_IN, DS_MLP_H1, DS_MLP_H2 = 8, 32, 16
+DS_XBINS, DS_MAX_SECTORS, DS_MAX_FIRST_HITS = 16, 16, 10
+
+c_fp = ct.POINTER(ct.c_float)
+c_ip = ct.POINTER(ct.c_int32)
+c_lp = ct.POINTER(ct.c_int64)
+
+
+class DsGeometry(ct.Structure):
+    _fields_ = [("struct_size", ct.c_size_t), ("z_layer", ct.c_double * 4), ("dxdy", ct.c_double * 4),
+                ("x_half", ct.c_double), ("y_half", ct.c_double), ("hole_half", ct.c_double),
+                ("n_sectors_y", ct.c_int32), ("pad_", ct.c_int32), ("sector_height", ct.c_double),
+                ("z_seed", ct.c_double), ("z_ref", ct.c_double), ("zmag_c", ct.c_double * 4), ("kick", ct.c_double)]
+
+
+class DsMlp(ct.Structure):
+    _fields_ = [("struct_size", ct.c_size_t),
+                ("W1", ct.c_float * (DS_MLP_H1 * DS_MLP_IN)), ("b1", ct.c_float * DS_MLP_H1),
+                ("W2", ct.c_float * (DS_MLP_H2 * DS_MLP_H1)), ("b2", ct.c_float * DS_MLP_H2),
+                ("W3", ct.c_float * DS_MLP_H2), ("b3", ct.c_float),
+                ("mu", ct.c_float * DS_MLP_IN), ("inv_sigma", ct.c_float * DS_MLP_IN)]
+
+
+class DsParams(ct.Structure):
+    _fields_ = [("struct_size", ct.c_size_t), ("w0_a", ct.c_double), ("w0_b", ct.c_double), ("w0_max", ct.c_double),
+                ("w1_a", ct.c_double), ("w1_b", ct.c_double), ("y_tol", ct.c_double), ("w_mag", ct.c_double),
+                ("chi2ndf_max", ct.c_double), ("miss_penalty", ct.c_double), ("min_hits", ct.c_int32),
+                ("max_first_hits", ct.c_int32), ("mlp_thr", ct.c_double), ("mlp_keep_above", ct.c_int32),
+                ("max_event_hits_hint", ct.c_int32), ("doca_max", ct.c_double), ("zv_min", ct.c_double),
+                ("zv_max", ct.c_double), ("m_pi", ct.c_double), ("m_p", ct.c_double), ("m_ks", ct.c_double),
+                ("m_lambda", ct.c_double), ("dm_ks", ct.c_double), ("dm_lambda", ct.c_double), ("n2_min", ct.c_double)]
+
+
+class DsHits(ct.Structure):
+    _fields_ = [("x0", ct.c_void_p), ("z", ct.c_void_p), ("ymin", ct.c_void_p), ("ymax", ct.c_void_p),
+                ("w", ct.c_void_p), ("id", ct.c_void_p), ("n", ct.c_int64)]
+
+
+class DsSeeds(ct.Structure):
+    _fields_ = [("x", ct.c_void_p), ("y", ct.c_void_p), ("tx", ct.c_void_p), ("ty", ct.c_void_p),
+                ("qop", ct.c_void_p), ("chi2", ct.c_void_p), ("n", ct.c_int64)]
+
+
+class DsTracks(ct.Structure):
+    _fields_ = [("x", ct.c_void_p), ("y", ct.c_void_p), ("tx", ct.c_void_p), ("ty", ct.c_void_p),
+                ("qop", ct.c_void_p), ("chi2", ct.c_void_p), ("score", ct.c_void_p), ("nhits", ct.c_void_p),
+                ("hit", ct.c_void_p), ("found", ct.c_void_p), ("keep", ct.c_void_p), ("n", ct.c_int64)]
+
+
+class DsVertices(ct.Structure):
+    _fields_ = [("evt", ct.c_void_p), ("ia", ct.c_void_p), ("ib", ct.c_void_p), ("x", ct.c_void_p),
+                ("y", ct.c_void_p), ("z", ct.c_void_p), ("doca", ct.c_void_p), ("m_pipi", ct.c_void_p),
+                ("m_ppi", ct.c_void_p), ("flags", ct.c_void_p), ("n_per_event", ct.c_void_p),
+                ("offsets", ct.c_void_p), ("overflow", ct.c_void_p), ("capacity", ct.c_int64)]
+
+
+class DsLayoutOut(ct.Structure):
+    _fields_ = [("x0", ct.c_void_p), ("z", ct.c_void_p), ("ymin", ct.c_void_p), ("ymax", ct.c_void_p),
+                ("w", ct.c_void_p), ("id", ct.c_void_p), ("perm", ct.c_void_p), ("bin_offsets", ct.c_void_p),
+                ("n", ct.c_int64)]
+
+
+HIT_F = ("x0", "z", "ymin", "ymax", "w")
+SEED_F = ("x", "y", "tx", "ty", "qop")
+TRACK_F = ("x", "y", "tx", "ty", "qop", "chi2", "score")
+TRACK_I = ("nhits", "found", "keep")
+VTX_I = ("evt", "ia", "ib", "flags")
+VTX_F = ("x", "y", "z", "doca", "m_pipi", "m_ppi")
+
+_lib = None
+
+
+class DsError(RuntimeError):
+    def __init__(self, code, where):
+        self.code = code
+        super().__init__(f"{where}: {ds_error_string(code)} ({code})")
+
+
+def lib() -> ct.CDLL:
+    """Load libds.so, building it with nvcc if it is missing or stale.  Raises if that is impossible."""
+    global _lib
+    if _lib is None:
+        path = _build.build()
+        L = ct.CDLL(path)
+        vp = ct.c_void_p
+        L.ds_create.argtypes = [ct.POINTER(vp), ct.c_int]
+        L.ds_destroy.argtypes = [vp]
+        L.ds_destroy.restype = None
+        L.ds_error_string.argtypes = [ct.c_int]
+        L.ds_error_string.restype = ct.c_char_p
+        L.ds_upload_geometry.argtypes = [vp, ct.POINTER(DsGeometry), ct.POINTER(DsMlp)]
+        L.ds_layout.argtypes = [vp, ct.POINTER(DsHits), vp, ct.c_int, ct.POINTER(DsParams), ct.POINTER(DsLayoutOut), vp]
+        L.ds_extrapolate.argtypes = [vp, ct.POINTER(DsSeeds), ct.POINTER(DsParams), vp, vp]
+        L.ds_workspace_bytes.argtypes = [vp, ct.c_int, ct.c_int64, ct.c_int64]
+        L.ds_workspace_bytes.restype = ct.c_size_t
+        L.ds_reconstruct.argtypes = [vp, ct.POINTER(DsHits), ct.POINTER(DsSeeds), vp, vp, ct.c_int,
+                                     ct.POINTER(DsParams), ct.POINTER(DsTracks), vp, ct.c_size_t, vp]
+        L.ds_ghost_killer.argtypes = [vp, ct.POINTER(DsSeeds), ct.POINTER(DsParams), ct.POINTER(DsTracks), vp]
+        L.ds_vertex_workspace_bytes.argtypes = [vp, ct.c_int, ct.c_int64]
+        L.ds_vertex_workspace_bytes.restype = ct.c_size_t
+        L.ds_vertex.argtypes = [vp, ct.POINTER(DsTracks), vp, ct.c_int, ct.POINTER(DsParams), ct.POINTER(DsVertices),
+                                vp, ct.c_size_t, vp]
+        L.ds_process_host.argtypes = [vp, ct.POINTER(DsHits), ct.POINTER(DsSeeds), vp, vp, ct.c_int,
+                                      ct.POINTER(DsParams), ct.POINTER(DsTracks), ct.POINTER(DsVertices),
+                                      ct.POINTER(ct.c_int64), vp]
+        _lib = L
+    return _lib
+
+
+def _check(code, where):
+    if code != DS_OK:
+        raise DsError(code, where)
+
+
+# ---- struct builders ------------------------------------------------------------------------------------------------
+def make_geometry(g: dict) -> DsGeometry:
+    o = DsGeometry()
+    o.struct_size = ct.sizeof(DsGeometry)
+    o.z_layer[:] = g["z_layer"]
+    o.dxdy[:] = g["dxdy"]
+    o.zmag_c[:] = g["zmag_c"]
+    for k in ("x_half", "y_half", "hole_half", "n_sectors_y", "sector_height", "z_seed", "z_ref", "kick"):
+        setattr(o, k, g[k])
+    return o
+
+
+def make_mlp(w: dict) -> DsMlp:
+    o = DsMlp()
+    o.struct_size = ct.sizeof(DsMlp)
+    for k, shape in (("W1", (DS_MLP_H1, DS_MLP_IN)), ("b1", (DS_MLP_H1,)), ("W2", (DS_MLP_H2, DS_MLP_H1)),
+                     ("b2", (DS_MLP_H2,)), ("W3", (DS_MLP_H2,)), ("mu", (DS_MLP_IN,)), ("inv_sigma", (DS_MLP_IN,))):
+        a = np.ascontiguousarray(w[k], dtype=np.float32).reshape(-1)
+        if a.size != int(np.prod(shape)):
+            raise ValueError(f"mlp weight {k}: expected shape {shape}")
+        getattr(o, k)[:] = a.tolist()
+    o.b3 = float(np.asarray(w["b3"]).reshape(-1)[0])
+    return o
+
+
+def make_params(p: dict) -> DsParams:
+    o = DsParams()
+    o.struct_size = ct.sizeof(DsParams)
+    for name, _ in DsParams._fields_:
+        if name in p:
+            setattr(o, name, p[name])
+    return o
+
+
+def _ptr(t):
+    return None if t is None else t.data_ptr()
+
+
+def _np_ptr(a):
+    return None if a is None else a.ctypes.data
+
+
+def _stream_ptr(stream):
+    if stream is None:
+        import torch
+        return torch.cuda.current_stream().cuda_stream
+    return stream if isinstance(stream, int) else stream.cuda_stream
+
+
+# ---- C-named functions (handles are c_void_p; tensors are torch CUDA tensors) -------------------------------------------
+def ds_error_string(code: int) -> str:
+    return lib().ds_error_string(code).decode()
+
+
+def ds_version() -> int:
+    return lib().ds_version()
+
+
+def ds_create(device: int = 0) -> ct.c_void_p:
+    h = ct.c_void_p()
+    _check(lib().ds_create(ct.byref(h), device), "ds_create")
+    return h
+
+
+def ds_destroy(h) -> None:
+    lib().ds_destroy(h)
+
+
+def ds_upload_geometry(h, geometry: dict, mlp: dict) -> None:
+    g, m = make_geometry(geometry), make_mlp(mlp)
+    _check(lib().ds_upload_geometry(h, ct.byref(g), ct.byref(m)), "ds_upload_geometry")
+
+
+def _hits(hits) -> DsHits:
+    s = DsHits()
+    for k in HIT_F + ("id",):
+        setattr(s, k, _ptr(hits[k]))
+    s.n = hits["id"].numel()
+    return s
+
+
+def _seeds(seeds) -> DsSeeds:
+    s = DsSeeds()
+    for k in SEED_F:
+        setattr(s, k, _ptr(seeds[k]))
+    s.chi2 = _ptr(seeds.get("chi2"))
+    s.n = seeds["x"].numel()
+    return s
+
+
+def _tracks(trk) -> DsTracks:
+    s = DsTracks()
+    for k in TRACK_F + TRACK_I + ("hit",):
+        setattr(s, k, _ptr(trk.get(k)))
+    s.n = trk["x"].numel()
+    return s
+
+
+def _vertices(v, capacity) -> DsVertices:
+    s = DsVertices()
+    for k in VTX_I + VTX_F + ("n_per_event", "offsets", "overflow"):
+        setattr(s, k, _ptr(v[k]))
+    s.capacity = capacity
+    return s
+
+
+def ds_layout(h, hits, hit_offsets, n_events, params: DsParams, out, stream=None) -> None:
+    hs = _hits(hits)
+    o = DsLayoutOut()
+    for k in HIT_F + ("id", "perm", "bin_offsets"):
+        setattr(o, k, _ptr(out[k]))
+    o.n = hs.n
+    _check(lib().ds_layout(h, ct.byref(hs), _ptr(hit_offsets), n_events, ct.byref(params), ct.byref(o),
+                           _stream_ptr(stream)), "ds_layout")
+
+
+def ds_extrapolate(h, seeds, params: DsParams, out, stream=None) -> None:
+    ss = _seeds(seeds)
+    _check(lib().ds_extrapolate(h, ct.byref(ss), ct.byref(params), _ptr(out), _stream_ptr(stream)), "ds_extrapolate")
+
+
+def ds_workspace_bytes(h, n_events, n_hits, n_seeds) -> int:
+    return lib().ds_workspace_bytes(h, n_events, n_hits, n_seeds)
+
+
+def ds_reconstruct(h, hits, seeds, hit_offsets, seed_offsets, n_events, params: DsParams, out, workspace,
+                   stream=None) -> None:
+    hs, ss, ts = _hits(hits), _seeds(seeds), _tracks(out)
+    _check(lib().ds_reconstruct(h, ct.byref(hs), ct.byref(ss), _ptr(hit_offsets), _ptr(seed_offsets), n_events,
+                                ct.byref(params), ct.byref(ts), _ptr(workspace),
+                                0 if workspace is None else workspace.numel() * workspace.element_size(),
+                                _stream_ptr(stream)), "ds_reconstruct")
+
+
+def ds_ghost_killer(h, seeds, params: DsParams, tracks, stream=None) -> None:
+    ss, ts = _seeds(seeds), _tracks(tracks)
+    _check(lib().ds_ghost_killer(h, ct.byref(ss), ct.byref(params), ct.byref(ts), _stream_ptr(stream)),
+           "ds_ghost_killer")
+
+
+def ds_vertex_workspace_bytes(h, n_events, n_seeds) -> int:
+    return lib().ds_vertex_workspace_bytes(h, n_events, n_seeds)
+
+
+def ds_vertex(h, tracks, seed_offsets, n_events, params: DsParams, out, capacity, workspace, stream=None) -> None:
+    ts, vs = _tracks(tracks), _vertices(out, capacity)
+    _check(lib().ds_vertex(h, ct.byref(ts), _ptr(seed_offsets), n_events, ct.byref(params), ct.byref(vs),
+                           _ptr(workspace), 0 if workspace is None else workspace.numel() * workspace.element_size(),
+                           _stream_ptr(stream)), "ds_vertex")
+
+
+def _hp(a):
+    """Host pointer of a numpy array or a (pinned) torch CPU tensor."""
+    if a is None:
+        return None
+    return a.data_ptr() if hasattr(a, "data_ptr") else a.ctypes.data
+
+
+def _hn(a):
+    return a.numel() if hasattr(a, "numel") else a.size
+
+
+def ds_process_host(h, hits, seeds, hit_offsets, seed_offsets, n_events, params: DsParams, out_tracks, out_vertices,
+                    capacity, stream=None) -> int:
+    """All arrays in HOST memory (numpy or pinned torch CPU tensors).  Returns the true number of vertices."""
+    hs, ss, ts, vs = DsHits(), DsSeeds(), DsTracks(), DsVertices()
+    for k in HIT_F + ("id",):
+        setattr(hs, k, _hp(hits[k]))
+    hs.n = _hn(hits["id"])
+    for k in SEED_F:
+        setattr(ss, k, _hp(seeds[k]))
+    ss.chi2 = _hp(seeds.get("chi2"))
+    ss.n = _hn(seeds["x"])
+    for k in TRACK_F + TRACK_I + ("hit",):
+        setattr(ts, k, _hp(out_tracks[k]))
+    ts.n = ss.n
+    for k in VTX_I + VTX_F + ("n_per_event", "offsets", "overflow"):
+        setattr(vs, k, _hp(out_vertices[k]))
+    vs.capacity = capacity
+    total = ct.c_int64(0)
+    _check(lib().ds_process_host(h, ct.byref(hs), ct.byref(ss), _hp(hit_offsets), _hp(seed_offsets), n_events,
+                                 ct.byref(params), ct.byref(ts), ct.byref(vs), ct.byref(total),
+                                 _stream_ptr(stream)), "ds_process_host")
+    return total.value
+
+
+# ---- convenience wrapper: allocation of outputs / workspaces as torch tensors ----------------------------------------
+class Downstream:
+    """A libds handle with its geometry, MLP weights and parameters.  All compute happens in libds."""
+
+    def __init__(self, geometry: dict, mlp: dict, params: dict, device: int = 0):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2503_13092_b200 needs a CUDA device (there is no CPU fallback)")
+        self.torch = torch
+        self.device = torch.device("cuda", device)
+        self.geometry = dict(geometry)
+        self.n_bins = 4 * int(geometry["n_sectors_y"]) * DS_XBINS
+        self.h = ds_create(device)
+        ds_upload_geometry(self.h, geometry, mlp)
+        self.set_params(params)
+
+    def set_params(self, params: dict) -> None:
+        self.params_dict = dict(params)
+        self.params = make_params(params)
+
+    def close(self) -> None:
+        if getattr(self, "h", None):
+            ds_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # -- helpers -------------------------------------------------------------------------------------------------
+    def to_device(self, arrays: dict) -> dict:
+        t = self.torch
+        return {k: t.as_tensor(np.ascontiguousarray(v)).to(self.device) for k, v in arrays.items() if v is not None}
+
+    def empty_tracks(self, n: int) -> dict:
+        t = self.torch
+        out = {k: t.empty(n, dtype=t.float32, device=self.device) for k in TRACK_F}
+        out.update({k: t.empty(n, dtype=t.int32, device=self.device) for k in TRACK_I})
+        out["hit"] = t.empty((n, 4), dtype=t.int32, device=self.device)
+        return out
+
+    def empty_vertices(self, capacity: int, n_events: int) -> dict:
+        t = self.torch
+        out = {k: t.empty(capacity, dtype=t.int32, device=self.device) for k in VTX_I}
+        out.update({k: t.empty(capacity, dtype=t.float32, device=self.device) for k in VTX_F})
+        out["n_per_event"] = t.empty(max(n_events, 1), dtype=t.int32, device=self.device)
+        out["offsets"] = t.empty(n_events + 1, dtype=t.int64, device=self.device)
+        out["overflow"] = t.zeros(1, dtype=t.int32, device=self.device)
+        out["capacity"] = capacity
+        return out
+
+    def workspace(self, n_events: int, n_hits: int, n_seeds: int):
+        nbytes = ds_workspace_bytes(self.h, n_events, n_hits, n_seeds)
+        return self.torch.empty(nbytes, dtype=self.torch.uint8, device=self.device)
+
+    def vertex_workspace(self, n_events: int, n_seeds: int):
+        nbytes = ds_vertex_workspace_bytes(self.h, n_events, n_seeds)
+        return self.torch.empty(nbytes, dtype=self.torch.uint8, device=self.device)
+
+    # -- the calls ---------------------------------------------------------------------------------------------------
+    def layout(self, hits: dict, hit_offsets, stream=None) -> dict:
+        t = self.torch
+        n, ne = hits["id"].numel(), hit_offsets.numel() - 1
+        out = {k: t.empty(n, dtype=t.float32, device=self.device) for k in HIT_F}
+        out["id"] = t.empty(n, dtype=t.int32, device=self.device)
+        out["perm"] = t.empty(n, dtype=t.int32, device=self.device)
+        out["bin_offsets"] = t.empty((max(ne, 1), self.n_bins + 1), dtype=t.int32, device=self.device)
+        ds_layout(self.h, hits, hit_offsets, ne, self.params, out, stream)
+        return out
+
+    def extrapolate(self, seeds: dict, stream=None):
+        t = self.torch
+        out = t.empty((seeds["x"].numel(), 12), dtype=t.float64, device=self.device)
+        ds_extrapolate(self.h, seeds, self.params, out, stream)
+        return out
+
+    def reconstruct(self, hits: dict, seeds: dict, hit_offsets, seed_offsets, out=None, workspace=None, stream=None):
+        ne = hit_offsets.numel() - 1
+        if out is None:
+            out = self.empty_tracks(seeds["x"].numel())
+        if workspace is None:
+            workspace = self.workspace(ne, hits["id"].numel(), seeds["x"].numel())
+        ds_reconstruct(self.h, hits, seeds, hit_offsets, seed_offsets, ne, self.params, out, workspace, stream)
+        return out
+
+    def ghost_killer(self, seeds: dict, tracks: dict, stream=None):
+        ds_ghost_killer(self.h, seeds, self.params, tracks, stream)
+        return tracks
+
+    def vertex(self, tracks: dict, seed_offsets, capacity: int = None, out=None, workspace=None, stream=None):
+        ne = seed_offsets.numel() - 1
+        if out is None:
+            out = self.empty_vertices(capacity if capacity is not None else 1 << 20, ne)
+        if workspace is None:
+            workspace = self.vertex_workspace(ne, tracks["x"].numel())
+        ds_vertex(self.h, tracks, seed_offsets, ne, self.params, out, out["capacity"], workspace, stream)
+        return out
+
+    def process_host(self, hits: dict, seeds: dict, hit_offsets, seed_offsets, out_tracks: dict, out_vertices: dict,
+                     capacity: int, stream=None) -> int:
+        ne = _hn(hit_offsets) - 1
+        return ds_process_host(self.h, hits, seeds, hit_offsets, seed_offsets, ne, self.params, out_tracks,
+                               out_vertices, capacity, stream)
+
+
+def host_tracks(n: int, pinned: bool = False) -> dict:
+    """HOST output buffers for ds_process_host (numpy, or pinned torch tensors)."""
+    if pinned:
+        import torch
+        out = {k: torch.empty(n, dtype=torch.float32).pin_memory() for k in TRACK_F}
+        out.update({k: torch.empty(n, dtype=torch.int32).pin_memory() for k in TRACK_I})
+        out["hit"] = torch.empty((n, 4), dtype=torch.int32).pin_memory()
+        return out
+    out = {k: np.empty(n, dtype=np.float32) for k in TRACK_F}
+    out.update({k: np.empty(n, dtype=np.int32) for k in TRACK_I})
+    out["hit"] = np.empty((n, 4), dtype=np.int32)
+    return out
+
+
+def host_vertices(capacity: int, n_events: int, pinned: bool = False) -> dict:
+    if pinned:
+        import torch
+        out = {k: torch.empty(capacity, dtype=torch.int32).pin_memory() for k in VTX_I}
+        out.update({k: torch.empty(capacity, dtype=torch.float32).pin_memory() for k in VTX_F})
+        out["n_per_event"] = torch.empty(max(n_events, 1), dtype=torch.int32).pin_memory()
+        out["offsets"] = torch.empty(n_events + 1, dtype=torch.int64).pin_memory()
+        out["overflow"] = torch.zeros(1, dtype=torch.int32).pin_memory()
+        return out
+    out = {k: np.empty(capacity, dtype=np.int32) for k in VTX_I}
+    out.update({k: np.empty(capacity, dtype=np.float32) for k in VTX_F})
+    out["n_per_event"] = np.empty(max(n_events, 1), dtype=np.int32)
+    out["offsets"] = np.empty(n_events + 1, dtype=np.int64)
+    out["overflow"] = np.zeros(1, dtype=np.int32)
+    return out
