@@ -215,6 +215,26 @@ int ds_process_host(ds_handle *h, const ds_hits *hits, const ds_seeds *seeds, co
                     const int32_t *seed_offsets, int n_events, const ds_params *p, ds_tracks *out_tracks,
                     ds_vertices *out_vertices, int64_t *n_vertices_total, void *cuda_stream);
 
+/* ---- per-kernel device timing (measurement aid; no effect on results) ------------------------------------------ */
+
+/* Kernels of the path, in launch order. */
+enum { DS_K_LAYOUT = 0, DS_K_TRACK, DS_K_MLP, DS_K_VTX_COUNT, DS_K_VTX_SCAN, DS_K_VTX_WRITE, DS_K_COUNT };
+
+typedef struct {
+    size_t struct_size;
+    double ms[DS_K_COUNT];        /* summed device time of the kernel's launches, CUDA events on the launching stream */
+    int64_t launches[DS_K_COUNT]; /* number of launches                                                             */
+} ds_profile;
+
+/* on != 0: every kernel launched through this handle from now on is bracketed by a pair of CUDA events recorded on
+ * the stream it is launched on.  Off by default. */
+int ds_profile_enable(ds_handle *h, int on);
+/* Waits for all recorded events (blocks the calling thread until the bracketed kernels have finished), adds their
+ * elapsed times into *out (HOST) and forgets them.  Counters start from zero at every call. */
+int ds_profile_read(ds_handle *h, ds_profile *out);
+/* Name of kernel k ("k_layout", ...), NULL if k is out of range. */
+const char *ds_kernel_name(int k);
+
 #ifdef __cplusplus
 }
 #endif

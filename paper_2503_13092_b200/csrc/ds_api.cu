@@ -14,6 +14,7 @@ struct ds_handle {
     // arena of the *_host path, grown on demand
     unsigned char *arena;
     size_t arena_bytes;
+    Prof prof;
 };
 
 namespace {
@@ -173,6 +174,7 @@ void ds_destroy(ds_handle *h)
     DeviceGuard guard(h->device);
     if (h->d_mlp) cudaFree(h->d_mlp);
     if (h->arena) cudaFree(h->arena);
+    h->prof.destroy();
     delete h;
 }
 
@@ -222,7 +224,7 @@ int ds_layout(ds_handle *h, const ds_hits *hits, const int32_t *hit_offsets, int
     set_inputs(L, hits);
     L.sx0 = out->x0; L.sz = out->z; L.symin = out->ymin; L.symax = out->ymax; L.sw = out->w; L.sid = out->id;
     L.perm = out->perm; L.bin_offsets = out->bin_offsets;
-    if (launch_layout(c, L, hit_offsets, n_events, p->max_event_hits_hint, (cudaStream_t)cuda_stream) != cudaSuccess) {
+    if (launch_layout(c, L, hit_offsets, n_events, p->max_event_hits_hint, (cudaStream_t)cuda_stream, h->prof) != cudaSuccess) {
         cudaGetLastError();
         return DS_E_CUDA;
     }
@@ -259,7 +261,7 @@ int ds_ghost_killer(ds_handle *h, const ds_seeds *seeds, const ds_params *p, ds_
     if (!make_const(h->geom, p, c)) return DS_E_ARG;
     DeviceGuard guard(h->device);
     if (!guard.ok) return DS_E_CUDA;
-    if (launch_mlp(c, h->d_mlp, *seeds, *trk, (cudaStream_t)cuda_stream) != cudaSuccess) {
+    if (launch_mlp(c, h->d_mlp, *seeds, *trk, (cudaStream_t)cuda_stream, h->prof) != cudaSuccess) {
         cudaGetLastError();
         return DS_E_CUDA;
     }
@@ -284,9 +286,9 @@ int ds_reconstruct(ds_handle *h, const ds_hits *hits, const ds_seeds *seeds, con
     LayoutPtrs L;
     set_inputs(L, hits);
     carve_layout(workspace, c.n_bins, n_events, hits->n, L);
-    cudaError_t err = launch_layout(c, L, hit_offsets, n_events, p->max_event_hits_hint, st);
-    if (err == cudaSuccess) err = launch_track(c, L, *seeds, hit_offsets, seed_offsets, n_events, *out, st);
-    if (err == cudaSuccess) err = launch_mlp(c, h->d_mlp, *seeds, *out, st);
+    cudaError_t err = launch_layout(c, L, hit_offsets, n_events, p->max_event_hits_hint, st, h->prof);
+    if (err == cudaSuccess) err = launch_track(c, L, *seeds, hit_offsets, seed_offsets, n_events, *out, st, h->prof);
+    if (err == cudaSuccess) err = launch_mlp(c, h->d_mlp, *seeds, *out, st, h->prof);
     if (err != cudaSuccess) {
         cudaGetLastError();
         return DS_E_CUDA;
@@ -313,7 +315,7 @@ int ds_vertex(ds_handle *h, const ds_tracks *trk, const int32_t *seed_offsets, i
         return DS_E_WORKSPACE;
     DeviceGuard guard(h->device);
     if (!guard.ok) return DS_E_CUDA;
-    if (launch_vertex(c, *trk, seed_offsets, n_events, *out, workspace, (cudaStream_t)cuda_stream) != cudaSuccess) {
+    if (launch_vertex(c, *trk, seed_offsets, n_events, *out, workspace, (cudaStream_t)cuda_stream, h->prof) != cudaSuccess) {
         cudaGetLastError();
         return DS_E_CUDA;
     }
@@ -393,10 +395,10 @@ int ds_process_host(ds_handle *h, const ds_hits *hits, const ds_seeds *seeds, co
     LayoutPtrs L;
     set_inputs(L, &dh);
     carve_layout(wrec, c.n_bins, n_events, hits->n, L);
-    err = launch_layout(c, L, d_hoff, n_events, p->max_event_hits_hint, st);
-    if (err == cudaSuccess) err = launch_track(c, L, dsd, d_hoff, d_soff, n_events, dt, st);
-    if (err == cudaSuccess) err = launch_mlp(c, h->d_mlp, dsd, dt, st);
-    if (err == cudaSuccess) err = launch_vertex(c, dt, d_soff, n_events, dv, wvtx, st);
+    err = launch_layout(c, L, d_hoff, n_events, p->max_event_hits_hint, st, h->prof);
+    if (err == cudaSuccess) err = launch_track(c, L, dsd, d_hoff, d_soff, n_events, dt, st, h->prof);
+    if (err == cudaSuccess) err = launch_mlp(c, h->d_mlp, dsd, dt, st, h->prof);
+    if (err == cudaSuccess) err = launch_vertex(c, dt, d_soff, n_events, dv, wvtx, st, h->prof);
     auto d2h = [&](void *dst, const void *src, size_t bytes) {
         if (bytes && err == cudaSuccess) err = cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToHost, st);
     };
@@ -419,6 +421,40 @@ int ds_process_host(ds_handle *h, const ds_hits *hits, const ds_seeds *seeds, co
     if (err == cudaSuccess) err = cudaStreamSynchronize(st);
     if (err != cudaSuccess) { cudaGetLastError(); return DS_E_CUDA; }
     return DS_OK;
+}
+
+int ds_profile_enable(ds_handle *h, int on)
+{
+    if (!h) return DS_E_ARG;
+    h->prof.on = on != 0;
+    return DS_OK;
+}
+
+int ds_profile_read(ds_handle *h, ds_profile *out)
+{
+    if (!h || !out || out->struct_size != sizeof(ds_profile)) return DS_E_ARG;
+    DeviceGuard guard(h->device);
+    if (!guard.ok) return DS_E_CUDA;
+    for (int k = 0; k < DS_K_COUNT; ++k) { out->ms[k] = 0.0; out->launches[k] = 0; }
+    int rc = DS_OK;
+    for (auto &r : h->prof.recs) {
+        float ms = 0.f;
+        if (cudaEventSynchronize(r.b) != cudaSuccess || cudaEventElapsedTime(&ms, r.a, r.b) != cudaSuccess) {
+            cudaGetLastError();
+            rc = DS_E_CUDA;
+            continue;
+        }
+        out->ms[r.k] += (double)ms;
+        out->launches[r.k] += 1;
+    }
+    h->prof.release();
+    return rc;
+}
+
+const char *ds_kernel_name(int k)
+{
+    static const char *names[DS_K_COUNT] = {"k_layout", "k_track", "k_mlp", "k_vertex_count", "k_vertex_scan", "k_vertex_write"};
+    return (k >= 0 && k < DS_K_COUNT) ? names[k] : nullptr;
 }
 
 }  // extern "C"

@@ -4,6 +4,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <vector>
+
 #include "../../include/ds.h"
 
 namespace ds {
@@ -68,6 +70,43 @@ __device__ __forceinline__ unsigned lanemask_lt()
     return m;
 }
 
+// Optional per-kernel device timing (ds_profile_enable / ds_profile_read): a pair of events around each launch, on the
+// launching stream.  Host side only.
+struct Prof {
+    struct Rec { int k; cudaEvent_t a, b; };
+    bool on = false;
+    std::vector<Rec> recs;
+    std::vector<cudaEvent_t> pool;
+    cudaEvent_t get()
+    {
+        cudaEvent_t e = nullptr;
+        if (!pool.empty()) { e = pool.back(); pool.pop_back(); }
+        else if (cudaEventCreate(&e) != cudaSuccess) { cudaGetLastError(); e = nullptr; }
+        return e;
+    }
+    void begin(int k, cudaStream_t st)
+    {
+        if (!on) return;
+        Rec r{k, get(), get()};
+        if (r.a && r.b) { cudaEventRecord(r.a, st); recs.push_back(r); }
+    }
+    void end(cudaStream_t st)
+    {
+        if (on && !recs.empty()) cudaEventRecord(recs.back().b, st);
+    }
+    void release()
+    {
+        for (auto &r : recs) { pool.push_back(r.a); pool.push_back(r.b); }
+        recs.clear();
+    }
+    void destroy()
+    {
+        release();
+        for (auto e : pool) cudaEventDestroy(e);
+        pool.clear();
+    }
+};
+
 // ---- launchers (host side, defined in the .cu files; all enqueue on `st` and return the launch error) ------------
 struct LayoutPtrs {
     const float *x0, *z, *ymin, *ymax, *w;
@@ -77,18 +116,18 @@ struct LayoutPtrs {
 };
 
 cudaError_t launch_layout(const DevConst &c, const LayoutPtrs &p, const int32_t *hit_offsets, int n_events,
-                          int max_event_hits_hint, cudaStream_t st);
+                          int max_event_hits_hint, cudaStream_t st, Prof &prof);
 
 cudaError_t launch_extrapolate(const DevConst &c, const ds_seeds &seeds, double *out, cudaStream_t st);
 
 cudaError_t launch_track(const DevConst &c, const LayoutPtrs &lay, const ds_seeds &seeds, const int32_t *hit_offsets,
-                         const int32_t *seed_offsets, int n_events, const ds_tracks &out, cudaStream_t st);
+                         const int32_t *seed_offsets, int n_events, const ds_tracks &out, cudaStream_t st, Prof &prof);
 
 cudaError_t launch_mlp(const DevConst &c, const DevMlp *mlp, const ds_seeds &seeds, const ds_tracks &trk,
-                       cudaStream_t st);
+                       cudaStream_t st, Prof &prof);
 
 cudaError_t launch_vertex(const DevConst &c, const ds_tracks &trk, const int32_t *seed_offsets, int n_events,
-                          const ds_vertices &out, void *workspace, cudaStream_t st);
+                          const ds_vertices &out, void *workspace, cudaStream_t st, Prof &prof);
 size_t vertex_workspace_bytes(int n_events, int64_t n_seeds);
 
 }  // namespace ds

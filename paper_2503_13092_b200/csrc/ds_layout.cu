@@ -191,7 +191,7 @@ k_layout(const __grid_constant__ DevConst c, const LayoutPtrs p, const int32_t *
 static size_t layout_smem_bytes(int cap) { return sizeof(int) * (kMaxBins + 1) + (size_t)cap * (4 * 4 + 2) + 16; }
 
 cudaError_t launch_layout(const DevConst &c, const LayoutPtrs &p, const int32_t *hit_offsets, int n_events,
-                          int max_event_hits_hint, cudaStream_t st)
+                          int max_event_hits_hint, cudaStream_t st, Prof &prof)
 {
     if (n_events <= 0) return cudaSuccess;
     int hint = max_event_hits_hint > 0 ? max_event_hits_hint : 4096;
@@ -202,7 +202,9 @@ cudaError_t launch_layout(const DevConst &c, const LayoutPtrs &p, const int32_t 
     const size_t smem = layout_smem_bytes(cap);
     cudaError_t err = cudaFuncSetAttribute(k_layout, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (err != cudaSuccess) return err;
+    prof.begin(DS_K_LAYOUT, st);
     k_layout<<<n_events, kLayoutThreads, smem, st>>>(c, p, hit_offsets, cap);
+    prof.end(st);
     return cudaGetLastError();
 }
 

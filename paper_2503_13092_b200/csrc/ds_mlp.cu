@@ -105,10 +105,12 @@ k_mlp(const __grid_constant__ DevConst c, const DevMlp *__restrict__ gm, const d
 }
 
 cudaError_t launch_mlp(const DevConst &c, const DevMlp *mlp, const ds_seeds &seeds, const ds_tracks &trk,
-                       cudaStream_t st)
+                       cudaStream_t st, Prof &prof)
 {
     if (trk.n <= 0) return cudaSuccess;
+    prof.begin(DS_K_MLP, st);
     k_mlp<<<(unsigned)((trk.n + kMlpThreads - 1) / kMlpThreads), kMlpThreads, 0, st>>>(c, mlp, seeds, trk);
+    prof.end(st);
     return cudaGetLastError();
 }
 

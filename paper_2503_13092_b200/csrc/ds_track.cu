@@ -404,10 +404,12 @@ k_track(const __grid_constant__ DevConst c, const LayoutPtrs L, const ds_seeds s
 }
 
 cudaError_t launch_track(const DevConst &c, const LayoutPtrs &lay, const ds_seeds &seeds, const int32_t *hit_offsets,
-                         const int32_t *seed_offsets, int n_events, const ds_tracks &out, cudaStream_t st)
+                         const int32_t *seed_offsets, int n_events, const ds_tracks &out, cudaStream_t st, Prof &prof)
 {
     if (n_events <= 0) return cudaSuccess;
+    prof.begin(DS_K_TRACK, st);
     k_track<<<n_events, kTrackThreads, 0, st>>>(c, lay, seeds, hit_offsets, seed_offsets, out);
+    prof.end(st);
     return cudaGetLastError();
 }
 

@@ -231,7 +231,7 @@ size_t vertex_workspace_bytes(int n_events, int64_t n_seeds)
 }
 
 cudaError_t launch_vertex(const DevConst &c, const ds_tracks &trk, const int32_t *seed_offsets, int n_events,
-                          const ds_vertices &out, void *workspace, cudaStream_t st)
+                          const ds_vertices &out, void *workspace, cudaStream_t st, Prof &prof)
 {
     auto up = [](size_t v) { return (v + 255) & ~(size_t)255; };
     PairLists pl;
@@ -242,15 +242,21 @@ cudaError_t launch_vertex(const DevConst &c, const ds_tracks &trk, const int32_t
     w += up(sizeof(int32_t) * (size_t)(n_events > 0 ? n_events : 1));
     pl.nneg = reinterpret_cast<int32_t *>(w);
     if (n_events > 0) {
+        prof.begin(DS_K_VTX_COUNT, st);
         k_vertex_count<<<n_events, kVtxThreads, 0, st>>>(c, trk, seed_offsets, pl, out.n_per_event);
+        prof.end(st);
         cudaError_t err = cudaGetLastError();
         if (err != cudaSuccess) return err;
     }
+    prof.begin(DS_K_VTX_SCAN, st);
     k_vertex_scan<<<1, kScanThreads, 0, st>>>(out.n_per_event, n_events, out.offsets, out.capacity, out.overflow);
+    prof.end(st);
     cudaError_t err = cudaGetLastError();
     if (err != cudaSuccess) return err;
     if (n_events > 0) {
+        prof.begin(DS_K_VTX_WRITE, st);
         k_vertex_write<<<n_events, kVtxThreads, 0, st>>>(c, trk, seed_offsets, pl, out);
+        prof.end(st);
         err = cudaGetLastError();
     }
     return err;

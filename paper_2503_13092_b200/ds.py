@@ -73,6 +73,13 @@ class DsVertices(ct.Structure):
                 ("offsets", ct.c_void_p), ("overflow", ct.c_void_p), ("capacity", ct.c_int64)]
 
 
+DS_K_COUNT = 6
+
+
+class DsProfile(ct.Structure):
+    _fields_ = [("struct_size", ct.c_size_t), ("ms", ct.c_double * DS_K_COUNT), ("launches", ct.c_int64 * DS_K_COUNT)]
+
+
 class DsLayoutOut(ct.Structure):
     _fields_ = [("x0", ct.c_void_p), ("z", ct.c_void_p), ("ymin", ct.c_void_p), ("ymax", ct.c_void_p),
                 ("w", ct.c_void_p), ("id", ct.c_void_p), ("perm", ct.c_void_p), ("bin_offsets", ct.c_void_p),
@@ -122,6 +129,10 @@ def lib() -> ct.CDLL:
         L.ds_process_host.argtypes = [vp, ct.POINTER(DsHits), ct.POINTER(DsSeeds), vp, vp, ct.c_int,
                                       ct.POINTER(DsParams), ct.POINTER(DsTracks), ct.POINTER(DsVertices),
                                       ct.POINTER(ct.c_int64), vp]
+        L.ds_profile_enable.argtypes = [vp, ct.c_int]
+        L.ds_profile_read.argtypes = [vp, ct.POINTER(DsProfile)]
+        L.ds_kernel_name.argtypes = [ct.c_int]
+        L.ds_kernel_name.restype = ct.c_char_p
         _lib = L
     return _lib
 
@@ -315,6 +326,18 @@ def ds_process_host(h, hits, seeds, hit_offsets, seed_offsets, n_events, params:
                                  ct.byref(params), ct.byref(ts), ct.byref(vs), ct.byref(total),
                                  _stream_ptr(stream)), "ds_process_host")
     return total.value
+
+
+def ds_profile_enable(h, on: bool) -> None:
+    _check(lib().ds_profile_enable(h, 1 if on else 0), "ds_profile_enable")
+
+
+def ds_profile_read(h) -> dict:
+    """{kernel name: (summed device ms, launches)} since the last read (waits for the recorded events)."""
+    p = DsProfile()
+    p.struct_size = ct.sizeof(DsProfile)
+    _check(lib().ds_profile_read(h, ct.byref(p)), "ds_profile_read")
+    return {lib().ds_kernel_name(k).decode(): (p.ms[k], p.launches[k]) for k in range(DS_K_COUNT)}
 
 
 # ---- convenience wrapper: allocation of outputs / workspaces as torch tensors ----------------------------------------

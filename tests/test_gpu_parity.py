@@ -1,0 +1,438 @@
+"""Parity of libds (CUDA, through the C ABI) against the CPU oracle on the same seeded inputs.  Needs a GPU.
+
+Stage-wise: tracks are compared with the oracle's tracks; vertices are compared with the oracle run on
+the GPU's own fp32 track arrays.  Rules in tests/parity.py.
+"""
+import numpy as np
+import pytest
+
+import gen
+from gen import constants as C
+from oracle import ds_oracle as O
+
+import parity
+
+pytestmark = pytest.mark.gpu
+G, P = C.GEOMETRY, C.PARAMS
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device (there is no CPU fallback)")
+    return torch
+
+
+@pytest.fixture(scope="module")
+def ds(torch, mlp_w):
+    import paper_2503_13092_b200 as pk
+    d = pk.Downstream(G, mlp_w, P)
+    yield d
+    d.close()
+
+
+def to_host(t):
+    return {k: (v.cpu().numpy() if hasattr(v, "cpu") else v) for k, v in t.items()}
+
+
+def gpu_run(ds, d, capacity=None, params=None):
+    """ds_reconstruct + ds_vertex on device-resident copies of the generated arrays -> host dicts."""
+    if params is not None:
+        ds.set_params(params)
+    try:
+        hits, seeds = ds.to_device(d["hits"]), ds.to_device(d["seeds"])
+        ho, so = ds.to_device(dict(h=d["hit_offsets"], s=d["seed_offsets"])).values()
+        trk = ds.reconstruct(hits, seeds, ho, so)
+        cap = capacity if capacity is not None else max(1024, 64 * len(d["seeds"]["x"]))
+        vtx = ds.vertex(trk, so, capacity=cap)
+        ds.torch.cuda.synchronize()
+    finally:
+        if params is not None:
+            ds.set_params(P)
+    t, v = to_host(trk), to_host(vtx)
+    n = int(v["offsets"][-1])
+    v["n"] = n
+    for k in ("evt", "ia", "ib", "flags", "x", "y", "z", "doca", "m_pipi", "m_ppi"):
+        v[k] = v[k][: min(n, cap)]
+    return t, v
+
+
+def oracle_run(d, orc_mlp, params=P):
+    return O.reconstruct(d["hits"], d["hit_offsets"], d["seeds"], d["seed_offsets"], G, params, orc_mlp)
+
+
+def check_both(ds, d, orc_mlp, params=None):
+    pp = params if params is not None else P
+    t, v = gpu_run(ds, d, params=params)
+    r = oracle_run(d, orc_mlp, pp)
+    st = parity.compare_tracks(t, r)
+    ov = O.vertex(t, d["seed_offsets"], G, pp)          # oracle vertexing of the GPU's own tracks (stage-wise)
+    assert v["n"] == ov["n"] or ov["edge_pairs"]
+    sv = parity.compare_vertices(v, ov)
+    assert (v["n_per_event"][: d["n_events"]] == ov["n_per_event"]).all() or ov["edge_pairs"]
+    assert (np.diff(v["offsets"]) == v["n_per_event"][: d["n_events"]]).all() and v["overflow"][0] == 0
+    return st, sv, t, v
+
+
+# ---- S1 layout ---------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("cfg,n_events,hint", [(0, 10, 0), (1, 64, 0), (2, 24, 0), (2, 24, 12288), (1, 8, 256)])
+def test_layout_equals_lexsort(ds, cfg, n_events, hint):
+    d = gen.generate(cfg, n_events=n_events)
+    ds.set_params(dict(P, max_event_hits_hint=hint))
+    try:
+        hits = ds.to_device(d["hits"])
+        ho = ds.to_device(dict(h=d["hit_offsets"]))["h"]
+        out = to_host(ds.layout(hits, ho))
+    finally:
+        ds.set_params(P)
+    h = d["hits"]
+    ev = np.repeat(np.arange(n_events), np.diff(d["hit_offsets"]))
+    layer, sector = (h["id"] >> 24) & 3, (h["id"] >> 20) & 15
+    order = np.lexsort((h["id"], h["x0"], sector, layer, ev))          # last key is the primary one
+    assert np.array_equal(out["perm"], order.astype(np.int32))
+    for k in ("x0", "z", "ymin", "ymax", "w", "id"):
+        assert np.array_equal(out[k], h[k][order]), k
+    # bin table: entries of the (layer, sector) boundaries equal the counts; x0 slices are monotone and hold their x0 range
+    nb = 4 * G["n_sectors_y"] * 16
+    tab = out["bin_offsets"].reshape(-1, nb + 1)[:n_events]
+    assert (np.diff(tab, axis=1) >= 0).all() and (tab[:, 0] == 0).all()
+    assert (tab[:, nb] == np.diff(d["hit_offsets"])).all()
+    coarse = (ev * 4 + layer) * G["n_sectors_y"] + sector
+    cnt = np.bincount(coarse, minlength=n_events * 4 * G["n_sectors_y"]).reshape(n_events, -1)
+    assert np.array_equal(np.diff(tab[:, ::16], axis=1), cnt)
+    X = G["x_half"] + G["y_half"] * max(abs(v) for v in G["dxdy"])
+    width = 2 * X / 16
+    for e in range(min(n_events, 4)):
+        xs = out["x0"][d["hit_offsets"][e]: d["hit_offsets"][e + 1]]
+        b = np.searchsorted(tab[e], np.arange(len(xs)), side="right") - 1
+        xb = b % 16
+        lo, hi = -X + xb * width, -X + (xb + 1) * width
+        assert ((xs >= lo - 1e-3) | (xb == 0)).all() and ((xs <= hi + 1e-3) | (xb == 15)).all()
+
+
+# ---- S2 extrapolation ----------------------------------------------------------------------------------------------
+def test_extrapolate_equals_oracle(ds):
+    d = gen.generate(1, n_events=4)
+    s = d["seeds"]
+    out = ds.extrapolate(ds.to_device(s)).cpu().numpy()
+    for i in range(0, len(s["x"]), 7):
+        ex = O.extrapolate(G, P, *(float(s[k][i]) for k in ("x", "y", "tx", "ty", "qop")))
+        ref = np.array([ex["z_m"], ex["x_m"], ex["y_m"], *ex["y_l"], ex["tx_pred"], ex["xc3"], ex["w0"], ex["w1"], 0.0])
+        assert np.allclose(out[i], ref, rtol=1e-13, atol=1e-10)
+
+
+# ---- S1..S10 on the five configs ------------------------------------------------------------------------------------
+def test_cfg0_noise_free(ds, orc_mlp):
+    d = gen.generate(0)
+    st, sv, t, v = check_both(ds, d, orc_mlp)
+    assert st["found"] == 200 and (t["nhits"] == 4).all()
+    sp = d["truth"]["seed_particle"]
+    assert (d["truth"]["hit_particle"][t["hit"]] == sp[:, None]).all()     # P-1 on the GPU output itself
+
+
+@pytest.mark.parametrize("cfg,n_events", [(1, 1000), (2, 1000), (3, 2000)])
+def test_full_configs(ds, orc_mlp, cfg, n_events):
+    d = gen.generate(cfg, n_events=n_events, workers=4)
+    hint = 16384 if cfg == 2 else 0
+    st, sv, t, v = check_both(ds, d, orc_mlp, params=dict(P, max_event_hits_hint=hint))
+    assert st["found"] > 10 * n_events and sv["n"] > n_events
+    print(f"cfg{cfg}: tracks {st}, vertices {sv}")
+
+
+def test_cfg2_oversize_path(ds, orc_mlp):
+    """cfg2 events (~8000 hits) with the default 4096-hit hint: the layout takes its global-memory path."""
+    d = gen.generate(2, n_events=12)
+    check_both(ds, d, orc_mlp)
+
+
+def test_cfg4_subbatch_sampled(ds, orc_mlp):
+    """One 10 000-event sub-batch of cfg4 in the launch configuration bench.py times; the oracle recomputes a
+    sample of events one by one (events are independent)."""
+    d = gen.generate(4, n_events=C.SUBBATCH_EVENTS, workers=8)
+    t, v = gpu_run(ds, d, capacity=1 << 20)
+    rng = np.random.default_rng(0)
+    sample = np.sort(rng.choice(C.SUBBATCH_EVENTS, 300, replace=False))
+    ho, so = d["hit_offsets"], d["seed_offsets"]
+    n_seeds = n_edge = n_vtx = 0
+    for e in sample:
+        h0, h1, s0, s1 = ho[e], ho[e + 1], so[e], so[e + 1]
+        hits = {k: a[h0:h1] for k, a in d["hits"].items()}
+        seeds = {k: a[s0:s1] for k, a in d["seeds"].items()}
+        r = O.reconstruct(hits, [0, h1 - h0], seeds, [0, s1 - s0], G, P, orc_mlp, n_threads=1)
+        r["hit"] = np.where(r["hit"] >= 0, r["hit"] + h0, -1)
+        te = {k: a[s0:s1] for k, a in t.items()}
+        # the 0.01 % bound is checked over the whole sample below
+        bad = ((te["found"] != r["found"]) | (te["nhits"] != r["nhits"]) | (te["keep"] != r["keep"])
+               | (te["hit"] != r["hit"]).any(axis=1))
+        assert not (bad & (r["edge"] == 0)).any(), f"event {e}"
+        n_edge += int(bad.sum())
+        ok = ~bad & (r["found"] == 1)
+        for k, floor in parity.TRACK_FLOORS.items():
+            assert parity.close(te[k][ok], r[k][ok], floor).all(), (e, k)
+        ov = O.vertex(te, [0, s1 - s0], G, P, n_threads=1)
+        v0, v1 = v["offsets"][e], v["offsets"][e + 1]
+        ge = {k: v[k][v0:v1] for k in ("evt", "flags", "x", "y", "z", "doca", "m_pipi", "m_ppi")}
+        ge["ia"], ge["ib"] = v["ia"][v0:v1] - s0, v["ib"][v0:v1] - s0
+        ge["evt"] = np.zeros_like(ge["evt"])
+        assert (v["evt"][v0:v1] == e).all()
+        parity.compare_vertices(ge, ov)
+        n_seeds += s1 - s0
+        n_vtx += ov["n"]
+    assert n_edge <= 1e-4 * n_seeds + 1 and n_vtx > 300
+    # properties that hold at any size, on the whole sub-batch
+    assert ((t["found"] == 0) | (t["hit"][:, 3] >= 0)).all()                  # UTbX hit is mandatory
+    ev_of_seed = np.repeat(np.arange(d["n_events"]), np.diff(so))
+    hh = t["hit"]
+    inside = (hh < 0) | ((hh >= ho[ev_of_seed][:, None]) & (hh < ho[ev_of_seed + 1][:, None]))
+    assert inside.all()                                                        # hits belong to the seed's event
+    lay = (d["hits"]["id"][np.maximum(hh, 0)] >> 24) & 3
+    assert ((hh < 0) | (lay == np.arange(4)[None, :])).all()
+    assert (t["nhits"] == (hh >= 0).sum(axis=1)).all() and ((t["found"] == 0) | (t["nhits"] >= P["min_hits"])).all()
+    assert (t["chi2"][t["found"] == 1] <= P["chi2ndf_max"] * (t["nhits"][t["found"] == 1] - 1) * (1 + 1e-6)).all()
+    assert (v["doca"] < P["doca_max"]).all() and (v["z"] >= P["zv_min"]).all() and (v["z"] <= P["zv_max"]).all()
+    assert (t["qop"][v["ia"]] > 0).all() and (t["qop"][v["ib"]] < 0).all() and (v["flags"] > 0).all()
+    assert (ev_of_seed[v["ia"]] == v["evt"]).all() and (ev_of_seed[v["ib"]] == v["evt"]).all()
+
+
+# ---- variants of the parameters ---------------------------------------------------------------------------------------
+@pytest.mark.parametrize("override", [
+    dict(max_first_hits=3), dict(min_hits=4), dict(mlp_keep_above=0, mlp_thr=0.5), dict(w0_b=400.0, w0_max=600.0),
+    dict(chi2ndf_max=1.0, miss_penalty=0.5), dict(y_tol=60.0), dict(doca_max=0.5, dm_ks=10.0, zv_min=1000.0),
+])
+def test_parameter_variants(ds, orc_mlp, override):
+    d = gen.generate(1, n_events=100)
+    check_both(ds, d, orc_mlp, params=dict(P, **override))
+
+
+def test_mirror_geometry_and_zmag_hook(ds, orc_mlp, mlp_w):
+    """Another geometry on a second handle: mirrored (U/V swapped) and the z_mag polynomial (A-3) switched on."""
+    import paper_2503_13092_b200 as pk
+    g2 = dict(C.GEOMETRY, dxdy=tuple(-v for v in C.GEOMETRY["dxdy"]), zmag_c=(5282.0, 30.0, -20.0, 4.0))
+    d = gen.generate(1, n_events=60)
+    hits = dict(d["hits"], x0=-d["hits"]["x0"])
+    seeds = dict(d["seeds"], x=-d["seeds"]["x"], tx=-d["seeds"]["tx"], qop=-d["seeds"]["qop"])
+    d2 = dict(d, hits=hits, seeds=seeds)
+    ds2 = pk.Downstream(g2, mlp_w, P)
+    try:
+        t, v = gpu_run(ds2, d2)
+    finally:
+        ds2.close()
+    r = O.reconstruct(hits, d["hit_offsets"], seeds, d["seed_offsets"], g2, P, orc_mlp)
+    parity.compare_tracks(t, r)
+    parity.compare_vertices(v, O.vertex(t, d["seed_offsets"], g2, P))
+
+
+# ---- S7 on its own ------------------------------------------------------------------------------------------------------
+def test_ghost_killer_alone(ds, orc_mlp, torch):
+    rng = np.random.default_rng(7)
+    n = 5000
+    trk = {k: (rng.normal(0, 1, n) * s + m).astype(np.float32)
+           for k, m, s in zip(("x", "y", "tx", "ty", "qop", "chi2"), C.MLP_MU[:6], C.MLP_SIGMA[:6])}
+    seeds = dict(x=trk["x"], y=trk["y"], tx=trk["tx"], ty=trk["ty"],
+                 qop=(rng.normal(0, 0.25, n)).astype(np.float32), chi2=rng.chisquare(7, n).astype(np.float32) / 7)
+    found = (rng.uniform(size=n) < 0.8).astype(np.int32)
+    dev = ds.empty_tracks(n)
+    for k, a in trk.items():
+        dev[k].copy_(torch.as_tensor(a))
+    dev["found"].copy_(torch.as_tensor(found))
+    for thr, above in ((0.1, 1), (0.5, 0), (0.5, 1)):
+        ds.set_params(dict(P, mlp_thr=thr, mlp_keep_above=above))
+        try:
+            ds.ghost_killer(ds.to_device(seeds), dev)
+            torch.cuda.synchronize()
+        finally:
+            ds.set_params(P)
+        score, keep = dev["score"].cpu().numpy(), dev["keep"].cpu().numpy()
+        ref = np.array([orc_mlp.eval([trk["x"][i], trk["y"][i], trk["tx"][i], trk["ty"][i], trk["qop"][i], trk["chi2"][i],
+                                      seeds["qop"][i], seeds["chi2"][i]]) for i in range(n)])
+        f = found == 1
+        assert parity.close(score[f], ref[f], 1e-3).all() and not score[~f].any() and not keep[~f].any()
+        want = (ref > thr) if above else (ref < thr)
+        margin = np.abs(ref - thr) / thr
+        assert (keep[f] == want[f])[margin[f] >= 1e-5].all()
+        assert 0.02 < keep[f].mean() < 0.999
+
+
+# ---- S8..S10 on hand-made tracks -----------------------------------------------------------------------------------------
+def _tracks_from(ds, torch, arr):
+    n = len(arr["x"])
+    dev = ds.empty_tracks(n)
+    for k in ("x", "y", "tx", "ty", "qop"):
+        dev[k].copy_(torch.as_tensor(np.asarray(arr[k], dtype=np.float32)))
+    dev["keep"].copy_(torch.as_tensor(np.asarray(arr["keep"], dtype=np.int32)))
+    return dev
+
+
+def test_vertex_closed_forms_and_overflow(ds, torch):
+    """P-7 on the GPU: two lines through a common point; capacity overflow bookkeeping; cuts disabled -> n+ * n-."""
+    zref = G["z_ref"]
+    rng = np.random.default_rng(3)
+    n_ev, per = 40, 30
+    pts = np.stack([rng.normal(0, 80, n_ev), rng.normal(0, 80, n_ev), rng.uniform(700, 2300, n_ev)], 1)
+    tx, ty = rng.uniform(-0.2, 0.2, (n_ev, per)), rng.uniform(-0.2, 0.2, (n_ev, per))
+    arr = dict(x=(pts[:, None, 0] + tx * (zref - pts[:, None, 2])).ravel(), y=(pts[:, None, 1] + ty * (zref - pts[:, None, 2])).ravel(),
+               tx=tx.ravel(), ty=ty.ravel(), qop=(rng.choice([-1.0, 1.0], n_ev * per) / rng.uniform(2, 50, n_ev * per)),
+               keep=(rng.uniform(size=n_ev * per) < 0.9).astype(np.int32))
+    so = np.arange(0, n_ev * per + 1, per, dtype=np.int32)
+    loose = dict(P, doca_max=1e30, zv_min=-1e30, zv_max=1e30, dm_ks=1e30, dm_lambda=1e30, n2_min=0.0)
+    ds.set_params(loose)
+    try:
+        dev = _tracks_from(ds, torch, arr)
+        dso = ds.to_device(dict(s=so))["s"]
+        v = to_host(ds.vertex(dev, dso, capacity=1 << 16))
+        n = int(v["offsets"][-1])
+        a32 = {k: np.asarray(arr[k], dtype=np.float32) for k in ("x", "y", "tx", "ty", "qop")}
+        kq = (arr["keep"] == 1)
+        npos = np.add.reduceat((kq & (a32["qop"] > 0)).astype(np.int64), so[:-1])
+        nneg = np.add.reduceat((kq & (a32["qop"] < 0)).astype(np.int64), so[:-1])
+        assert (v["n_per_event"][:n_ev] == npos * nneg).all() and n == int((npos * nneg).sum())
+        assert (v["doca"][:n] < 2e-3).all()                           # fp32 storage of x, y at ~100 mm
+        assert np.allclose(np.stack([v["x"][:n], v["y"][:n]], 1), pts[v["evt"][:n], :2], atol=0.05)
+        assert np.allclose(v["z"][:n], pts[v["evt"][:n], 2], atol=2.0)
+        ov = O.vertex(dict(a32, keep=arr["keep"]), so, G, loose)
+        vv = {k: v[k][:n] for k in ("evt", "ia", "ib", "flags", "x", "y", "z", "doca", "m_pipi", "m_ppi")}
+        # DOCA ~ 0 here: compare what is well-conditioned (the list, the masses)
+        assert list(zip(vv["evt"], vv["ia"], vv["ib"])) == list(zip(ov["evt"], ov["ia"], ov["ib"]))
+        assert parity.close(vv["m_pipi"], ov["m_pipi"], 0).all() and parity.close(vv["m_ppi"], ov["m_ppi"], 0).all()
+        # overflow: capacity smaller than the list
+        cap = n // 3
+        v2 = to_host(ds.vertex(dev, dso, capacity=cap))
+        assert int(v2["offsets"][-1]) == n and v2["overflow"][0] == n - cap
+        assert np.array_equal(v2["ia"][:cap], v["ia"][:cap]) and np.array_equal(v2["doca"][:cap], v["doca"][:cap])
+    finally:
+        ds.set_params(P)
+    # (0,0)+(t,0,1)s and (0,d)+(-t,0,1)s: DOCA = d, vertex (0, d/2, z_ref); parallel pair: no vertex (A-14)
+    arr = dict(x=[0, 0, 5, 9], y=[0, 1.5, 0, 3], tx=[0.1, -0.1, 0.05, 0.05], ty=[0, 0, 0.02, 0.02], qop=[0.2, -0.25, 0.1, -0.1],
+               keep=[1, 1, 1, 1])
+    ds.set_params(dict(P, zv_min=-1e9, zv_max=1e9, dm_ks=1e9, dm_lambda=1e9, doca_max=1e9))
+    try:
+        v = to_host(ds.vertex(_tracks_from(ds, torch, arr), ds.to_device(dict(s=np.array([0, 2, 4], dtype=np.int32)))["s"], capacity=16))
+    finally:
+        ds.set_params(P)
+    assert int(v["offsets"][-1]) == 1 and v["n_per_event"][1] == 0
+    assert v["doca"][0] == pytest.approx(1.5, rel=1e-6) and v["z"][0] == pytest.approx(zref, abs=1e-3) and v["y"][0] == pytest.approx(0.75, rel=1e-6)
+
+
+# ---- degenerate inputs -----------------------------------------------------------------------------------------------------
+def test_empty_and_ragged_inputs(ds, orc_mlp):
+    d = gen.generate(1, n_events=9)
+    ho, so = d["hit_offsets"].copy(), d["seed_offsets"].copy()
+    # event 2: no seeds; event 4: no hits; event 6: neither; last event: one seed
+    def cut(arrs, off, e, keep_n=0):
+        a, b = off[e] + keep_n, off[e + 1]
+        out = {k: np.concatenate([v[:a], v[b:]]) for k, v in arrs.items()}
+        off = off.copy()
+        off[e + 1:] -= b - a
+        return out, off
+    hits, seeds = d["hits"], d["seeds"]
+    seeds, so = cut(seeds, so, 2)
+    hits, ho = cut(hits, ho, 4)
+    seeds, so = cut(seeds, so, 6)
+    hits, ho = cut(hits, ho, 6)
+    seeds, so = cut(seeds, so, 8, keep_n=1)
+    d2 = dict(n_events=9, hits=hits, seeds=seeds, hit_offsets=ho, seed_offsets=so)
+    st, sv, t, v = check_both(ds, d2, orc_mlp)
+    assert not t["found"][so[4]:so[5]].any()
+    # no events at all / no seeds at all / no hits at all
+    z = dict(n_events=0, hits={k: v[:0] for k, v in hits.items()}, seeds={k: v[:0] for k, v in seeds.items()},
+             hit_offsets=np.zeros(1, np.int32), seed_offsets=np.zeros(1, np.int32))
+    t0, v0 = gpu_run(ds, z)
+    assert v0["n"] == 0 and len(t0["found"]) == 0
+    z = dict(d2, seeds={k: v[:0] for k, v in seeds.items()}, seed_offsets=np.zeros(10, np.int32))
+    t0, v0 = gpu_run(ds, z)
+    assert v0["n"] == 0
+    z = dict(d2, hits={k: v[:0] for k, v in hits.items()}, hit_offsets=np.zeros(10, np.int32))
+    t0, v0 = gpu_run(ds, z)
+    assert not t0["found"].any() and v0["n"] == 0
+
+
+def test_duplicate_hits_and_ties(ds, orc_mlp):
+    """Every hit duplicated with a different id: equal distances and equal scores everywhere -> id tie-breaks decide."""
+    d = gen.generate(1, n_events=20)
+    h = d["hits"]
+    n = len(h["id"])
+    ev = np.repeat(np.arange(20), np.diff(d["hit_offsets"]))
+    dup = {k: np.concatenate([v, v]) for k, v in h.items()}
+    dup["id"] = np.concatenate([h["id"], h["id"] + 50000])                # seq + 50000 stays below 2^20
+    order = np.argsort(np.concatenate([ev, ev]), kind="stable")
+    rng = np.random.default_rng(1)
+    hits = {k: v[order] for k, v in dup.items()}
+    ho = (2 * d["hit_offsets"]).astype(np.int32)
+    for e in range(20):                                                      # shuffle inside the event
+        p = rng.permutation(ho[e + 1] - ho[e]) + ho[e]
+        for k in hits:
+            hits[k][ho[e]:ho[e + 1]] = hits[k][p]
+    assert n * 2 == ho[-1]
+    check_both(ds, dict(d, hits=hits, hit_offsets=ho), orc_mlp)
+
+
+def test_dense_window_more_than_ten_first_hits(ds, orc_mlp):
+    """A crowded UTbX: > 10 (and > 32) hits inside the first window -> the 10 closest by (distance, id)."""
+    d = gen.generate(1, n_events=6)
+    rng = np.random.default_rng(2)
+    extra_n = 6000
+    lay = np.full(extra_n, 3)
+    x = rng.uniform(-860, 860, extra_n)
+    x[: extra_n // 2] = np.round(x[: extra_n // 2])                      # many exact ties in distance
+    y = rng.uniform(-700, 700, extra_n)
+    sec = np.clip(np.floor((y + 700) / 100).astype(np.int64), 0, 13)
+    add = dict(x0=x.astype(np.float32), z=np.full(extra_n, G["z_layer"][3], np.float32), ymin=(-700 + 100 * sec).astype(np.float32),
+               ymax=(-600 + 100 * sec).astype(np.float32), w=np.full(extra_n, C.W_HIT, np.float32),
+               id=((100000 + np.arange(extra_n)) | (sec << 20) | (lay << 24)).astype(np.int32))
+    e = 3
+    at = d["hit_offsets"][e + 1]
+    hits = {k: np.concatenate([v[:at], add[k], v[at:]]) for k, v in d["hits"].items()}
+    ho = d["hit_offsets"].copy()
+    ho[e + 1:] += extra_n
+    st, sv, t, v = check_both(ds, dict(d, hits=hits, hit_offsets=ho), orc_mlp, params=dict(P, max_event_hits_hint=12288))
+    assert st["found"] > 0
+
+
+# ---- host-buffer path ---------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("pinned", [False, True])
+def test_process_host_equals_device_path(ds, torch, pinned):
+    import paper_2503_13092_b200 as pk
+    d = gen.generate(1, n_events=50)
+    t, v = gpu_run(ds, d)
+    ns, ne = len(d["seeds"]["x"]), d["n_events"]
+    cap = 4096
+    ot, ovx = pk.host_tracks(ns, pinned), pk.host_vertices(cap, ne, pinned)
+    n = ds.process_host(d["hits"], d["seeds"], d["hit_offsets"], d["seed_offsets"], ot, ovx, cap)
+    ot, ovx = to_host({k: (a.numpy() if hasattr(a, "numpy") else a) for k, a in ot.items()}), \
+        {k: (a.numpy() if hasattr(a, "numpy") else a) for k, a in ovx.items()}
+    assert n == v["n"]
+    for k in t:
+        assert np.array_equal(np.asarray(ot[k]).reshape(t[k].shape), t[k]), k
+    for k in ("evt", "ia", "ib", "flags", "x", "y", "z", "doca", "m_pipi", "m_ppi"):
+        assert np.array_equal(ovx[k][:n], v[k]), k
+    assert np.array_equal(ovx["offsets"], v["offsets"])
+
+
+# ---- error codes -----------------------------------------------------------------------------------------------------------------
+def test_error_codes(ds, torch, mlp_w):
+    import paper_2503_13092_b200 as pk
+    d = gen.generate(0)
+    hits, seeds = ds.to_device(d["hits"]), ds.to_device(d["seeds"])
+    ho, so = ds.to_device(dict(h=d["hit_offsets"], s=d["seed_offsets"])).values()
+    trk = ds.empty_tracks(len(d["seeds"]["x"]))
+    small = torch.empty(256, dtype=torch.uint8, device="cuda")
+    with pytest.raises(pk.DsError) as e:
+        pk.ds_reconstruct(ds.h, hits, seeds, ho, so, 10, ds.params, trk, small)
+    assert e.value.code == pk.ds.DS_E_WORKSPACE
+    with pytest.raises(pk.DsError) as e:
+        pk.ds_reconstruct(ds.h, hits, seeds, ho, so, 10, pk.make_params(dict(P, max_first_hits=11)), trk, ds.workspace(10, 2000, 200))
+    assert e.value.code == pk.ds.DS_E_ARG
+    h2 = pk.ds_create(0)
+    try:
+        with pytest.raises(pk.DsError) as e:
+            pk.ds_reconstruct(h2, hits, seeds, ho, so, 10, ds.params, trk, ds.workspace(10, 2000, 200))
+        assert e.value.code == pk.ds.DS_E_NOGEOM
+        with pytest.raises(pk.DsError) as e:
+            pk.ds_upload_geometry(h2, dict(G, n_sectors_y=17), mlp_w)
+        assert e.value.code == pk.ds.DS_E_ARG
+    finally:
+        pk.ds_destroy(h2)
+    with pytest.raises(pk.DsError) as e:
+        pk.ds_create(99)
+    assert e.value.code == pk.ds.DS_E_CUDA
