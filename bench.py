@@ -1,0 +1,397 @@
+#!/usr/bin/env python
+"""bench.py -- events/s of the whole hot path (S1 layout -> S2..S6 tracking -> S7 ghost-killer MLP -> S8..S10 vertexing)
+on BASELINE.json configs[4]: 100 000 synthetic Run-3-shaped events (cfg-1 generator, seed 4), device resident,
+processed as 10 sub-batches of 10 000 events on two CUDA streams.  One JSON line on stdout (rank 0).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W]                 # this library (CUDA, sm_100a)
+    python bench.py --impl reference [--steps K] [--warmup W]           # the fp64 CPU oracle on the host cores
+    torchrun --nproc-per-node N ... bench.py --gpus N ...               # one rank per GPU, weak scaling, no collective
+                                                                        # on the data path (events are independent)
+
+A step = one pass of the whole path over all sub-batches.  `value` = events of all ranks / (device time of K steps,
+max over ranks).  `e2e` = the same through ds_process_host with pinned HOST buffers (H2D of every input and D2H of all
+tracks and vertices inside the timed region).  `roofline` = the kernel with the largest share of the step: its
+algorithmic bytes / its CUDA-event time measured in the timed region / the measured HBM peak.
+`cpu_baseline` = oracle/ as it stands on a bounded sample of the same events, same box.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "events_per_s_downstream_mlp_vertexing"
+UNIT = "events/s"
+CFG = 4
+
+
+def log(*a):
+    print(*a, file=sys.stderr, flush=True)
+
+
+# ---- inputs --------------------------------------------------------------------------------------------------------------
+def generate_subbatches(rank: int, n_sub: int, sub_events: int, workers: int):
+    """Sub-batch i of rank r = RNG blocks [r*n_sub*B + i*B, ... + B) of cfg4 (B = blocks per sub-batch)."""
+    import gen
+    from gen import constants as C
+    from paper_2503_13092_b200 import shard
+    bps = -(-sub_events // C.BLOCK_EVENTS)
+    b0, _ = shard.block_range(rank, n_sub * bps)
+    out = []
+    for i in range(n_sub):
+        d = gen.generate(CFG, n_events=sub_events, first_block=b0 + i * bps, workers=workers)
+        d.pop("truth", None)
+        out.append(d)
+    return out
+
+
+def peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def ncu_traffic():
+    """dram bytes per launch per kernel from the committed ncu --set full capture, if there is one."""
+    path = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return json.load(f)
+    return {}
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md, clocks line)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100",
+                                          "-i", str(self.index)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line)
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        self.thread.join(timeout=2)
+        sm, smax, reasons, power = [], [], set(), []
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for line in self.lines:
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); smax.append(float(f[1])); power.append(float(f[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(smax) if smax else None,
+                "power_w_max": max(power) if power else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ---- algorithmic bytes -------------------------------------------------------------
+def algorithmic_bytes(n_events, n_hits, n_seeds, n_found, n_keep, n_vtx):
+    return {
+        "k_layout": 52 * n_hits + 57 * 4 * n_events,                       # read 24 B/hit, write 24 + 4 B/hit, bin table
+        "k_track": 20 * n_hits + 28 * n_seeds + 52 * n_seeds + 16 * n_found,  # sorted hit fields once, seeds in, tracks out, 4 ids
+        "k_mlp": 12 * n_seeds + 32 * n_found,                              # found in, score + keep out; 8 features of found tracks
+        "k_vertex_count": 28 * n_keep + 8 * n_seeds + 4 * n_events,
+        "k_vertex_scan": 16 * n_events,
+        "k_vertex_write": 28 * n_keep + 40 * n_vtx,
+    }
+
+
+# ---- the oracle arm --------------------------------------------------------------------------------------------------------
+def oracle_events_per_s(d, n_events):
+    """Time oracle.reconstruct + oracle.vertex on the first n_events events of d (all host cores, OpenMP)."""
+    import gen
+    from gen import constants as C
+    from oracle import ds_oracle as O
+    sub = gen.take_events(d, n_events)
+    mlp = O.Mlp(gen.mlp_weights(0))
+    t0 = time.perf_counter()
+    r = O.reconstruct(sub["hits"], sub["hit_offsets"], sub["seeds"], sub["seed_offsets"], C.GEOMETRY, C.PARAMS, mlp)
+    v = O.vertex(r, sub["seed_offsets"], C.GEOMETRY, C.PARAMS)
+    dt = time.perf_counter() - t0
+    return n_events / dt, dt, O.max_threads(), int(r["found"].sum()), v["n"]
+
+
+def sized_sample(d, target_s, cap):
+    rate, _, _, _, _ = oracle_events_per_s(d, min(200, cap))
+    return int(max(100, min(cap, rate * target_s)))
+
+
+def run_reference(args, rank):
+    """--impl reference: there is no reference implementation for this paper; the arm is the fp64 CPU oracle."""
+    if rank != 0:
+        return
+    import gen
+    from gen import constants as C
+    d = gen.generate(CFG, n_events=args.subbatch, workers=min(8, os.cpu_count() or 1))
+    per_step = min(10.0, 150.0 / max(1, args.steps + args.warmup))
+    n = sized_sample(d, per_step, args.subbatch)
+    for _ in range(args.warmup):
+        oracle_events_per_s(d, n)
+    t0 = time.perf_counter()
+    cores = 1
+    for _ in range(args.steps):
+        _, _, cores, _, _ = oracle_events_per_s(d, n)
+    dt = time.perf_counter() - t0
+    value = n * args.steps / dt
+    sample = f"first {n} events of cfg4 sub-batch 0 per step (oracle/ds_oracle.c, fp64, OpenMP over events)"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": 0, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "BASELINE configs[4]: cfg-1 generator, seed 4 (bounded sample)", "events_per_step": n},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }), flush=True)
+
+
+# ---- our arm -------------------------------------------------------------------------------------------------------------------
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--events", type=int, default=100000, help="events per GPU (BASELINE configs[4]: 100 000)")
+    ap.add_argument("--subbatch", type=int, default=10000)
+    ap.add_argument("--streams", type=int, default=2)
+    ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    rank, world = int(os.environ.get("RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
+    local = int(os.environ.get("LOCAL_RANK", 0))
+    if args.impl == "reference":
+        return run_reference(args, rank)
+    if args.warmup < 3:
+        log("note: the timing rules ask for >= 3 warm-up steps")
+
+    from gen import constants as C
+    import gen
+    n_sub = max(1, args.events // args.subbatch)
+    workers = max(1, min(32, (os.cpu_count() or 1) // max(1, world)))
+    t0 = time.time()
+    subs = generate_subbatches(rank, n_sub, args.subbatch, workers)      # before CUDA is touched: the pool forks
+    log(f"[rank {rank}] generated {n_sub} x {args.subbatch} events in {time.time() - t0:.1f} s ({workers} workers)")
+
+    import torch
+    import torch.distributed as dist
+    import paper_2503_13092_b200 as pk
+    from paper_2503_13092_b200 import shard
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the product has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- pinned host copies (e2e inputs) and device-resident copies (kernel-path inputs) --------------------------------
+    mlp_w = gen.mlp_weights(0)
+    ds = pk.Downstream(C.GEOMETRY, mlp_w, C.PARAMS, device=local)
+    host, devd = [], []
+    for d in subs:
+        hp = dict(hits={k: torch.from_numpy(v).pin_memory() for k, v in d["hits"].items()},
+                  seeds={k: torch.from_numpy(v).pin_memory() for k, v in d["seeds"].items()},
+                  hit_offsets=torch.from_numpy(d["hit_offsets"]).pin_memory(),
+                  seed_offsets=torch.from_numpy(d["seed_offsets"]).pin_memory(), n_events=d["n_events"])
+        host.append(hp)
+        devd.append(dict(hits={k: v.to(dev, non_blocking=True) for k, v in hp["hits"].items()},
+                         seeds={k: v.to(dev, non_blocking=True) for k, v in hp["seeds"].items()},
+                         hit_offsets=hp["hit_offsets"].to(dev, non_blocking=True),
+                         seed_offsets=hp["seed_offsets"].to(dev, non_blocking=True), n_events=d["n_events"]))
+    n_hits = [int(d["hit_offsets"][-1]) for d in subs]
+    n_seeds = [int(d["seed_offsets"][-1]) for d in subs]
+    first_sub = subs[0]
+    del subs
+    torch.cuda.synchronize()
+    n_streams = max(1, args.streams)
+    streams = [torch.cuda.Stream(device=dev) for _ in range(n_streams)]
+    cap = 1 << 20
+    ws = [ds.workspace(args.subbatch, max(n_hits), max(n_seeds)) for _ in range(n_streams)]
+    vws = [ds.vertex_workspace(args.subbatch, max(n_seeds)) for _ in range(n_streams)]
+    trk = [ds.empty_tracks(n) for n in n_seeds]
+    vtx = [ds.empty_vertices(cap, args.subbatch) for _ in range(n_sub)]
+
+    def step():
+        for i, d in enumerate(devd):
+            s = streams[i % n_streams]
+            ds.reconstruct(d["hits"], d["seeds"], d["hit_offsets"], d["seed_offsets"], out=trk[i], workspace=ws[i % n_streams], stream=s)
+            ds.vertex(trk[i], d["seed_offsets"], out=vtx[i], workspace=vws[i % n_streams], stream=s)
+
+    for _ in range(args.warmup):
+        step()
+    torch.cuda.synchronize()
+    n_found = sum(int(t["found"].sum().item()) for t in trk)
+    n_keep = sum(int(t["keep"].sum().item()) for t in trk)
+    n_vtx = sum(int(v["offsets"][-1].item()) for v in vtx)
+    assert all(int(v["overflow"].item()) == 0 for v in vtx), "vertex capacity overflow"
+
+    # ---- timed region: K steps on the two streams, CUDA events on the stream the work is launched from, clocks sampled ----
+    main_stream = torch.cuda.current_stream()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    pk.ds_profile_enable(ds.h, True)
+    sampler = ClockSampler(local)
+    barrier()
+    sampler.start()
+    ev0.record(main_stream)
+    for s in streams:
+        s.wait_stream(main_stream)
+    for _ in range(args.steps):
+        step()
+    for s in streams:
+        main_stream.wait_stream(s)
+    ev1.record(main_stream)
+    barrier()
+    clocks = sampler.stop()
+    ms_total = shard.max_over_ranks(ev0.elapsed_time(ev1), dev)
+    prof2 = pk.ds_profile_read(ds.h)              # per-kernel events of the timed region: kernels of the two streams overlap
+    events_rank = args.subbatch * n_sub
+    events_all = shard.sum_over_ranks(events_rank, dev)
+    value = events_all * args.steps / (ms_total * 1e-3)
+
+    # ---- per-kernel pass: the same K steps, same launches, on ONE stream so that a kernel's event pair times that kernel
+    #      alone (in the two-stream region above a pair also spans whatever the other stream runs at the same time) ----------
+    def step_one_stream():
+        for i, d in enumerate(devd):
+            ds.reconstruct(d["hits"], d["seeds"], d["hit_offsets"], d["seed_offsets"], out=trk[i], workspace=ws[0], stream=streams[0])
+            ds.vertex(trk[i], d["seed_offsets"], out=vtx[i], workspace=vws[0], stream=streams[0])
+
+    barrier()
+    for _ in range(args.steps):
+        step_one_stream()
+    barrier()
+    prof = pk.ds_profile_read(ds.h)
+    pk.ds_profile_enable(ds.h, False)
+
+    # ---- roofline of the dominant kernel --------------------------------------------------------------------------------------
+    peak, peak_src = peaks()
+    alg = algorithmic_bytes(events_rank, sum(n_hits), sum(n_seeds), n_found, n_keep, n_vtx)     # bytes per step
+    traffic = ncu_traffic()
+    kernels, launches = {}, sum(n for _, n in prof2.values())
+    for name, (ms, n) in prof.items():
+        if n == 0:
+            continue
+        per_launch_ms = ms / n
+        bytes_per_launch = alg[name] * args.steps / n
+        gbs = bytes_per_launch / (per_launch_ms * 1e-3) / 1e9
+        kernels[name] = {"ms_per_launch": per_launch_ms, "ms_per_step": ms / args.steps, "launches_per_step": n / args.steps,
+                         "alg_bytes_per_launch": bytes_per_launch, "achieved_gbs": gbs, "frac": gbs / peak,
+                         "traffic": traffic.get(name), "ms_per_launch_two_streams": prof2[name][0] / max(1, prof2[name][1])}
+    dom = max(kernels, key=lambda k: kernels[k]["ms_per_step"])
+    ksum = sum(k["ms_per_step"] for k in kernels.values())
+    roofline = {"bound": "hbm", "kernel": dom, "achieved": kernels[dom]["achieved_gbs"], "peak": peak, "unit": "GB/s",
+                "frac": kernels[dom]["frac"], "traffic": kernels[dom]["traffic"], "peak_source": peak_src,
+                "share_of_step": kernels[dom]["ms_per_step"] / ksum,
+                "timing": "CUDA events around every launch, one-stream pass of the same K steps right after the timed region"}
+    whole_gbs = sum(alg.values()) * args.steps / (ms_total * 1e-3) / 1e9
+
+    # ---- end to end: pinned host buffers in, pinned host buffers out, through ds_process_host ----------------------------
+    e2e = None
+    if not args.no_e2e:
+        handles = [pk.Downstream(C.GEOMETRY, mlp_w, C.PARAMS, device=local) for _ in range(n_streams)]
+        vcap = 1 << 18
+        out_t = [pk.host_tracks(max(n_seeds), pinned=True) for _ in range(n_streams)]
+        out_v = [pk.host_vertices(vcap, args.subbatch, pinned=True) for _ in range(n_streams)]
+        totals = [0] * n_streams
+
+        def worker(k):
+            torch.cuda.set_device(local)
+            tot = 0
+            for i in range(k, n_sub, n_streams):
+                h = host[i]
+                ot = {kk: (v[: n_seeds[i]] if kk != "hit" else v[: n_seeds[i]]) for kk, v in out_t[k].items()}
+                tot += handles[k].process_host(h["hits"], h["seeds"], h["hit_offsets"], h["seed_offsets"], ot, out_v[k], vcap,
+                                               stream=streams[k])
+            totals[k] = tot
+
+        def e2e_step():
+            th = [threading.Thread(target=worker, args=(k,)) for k in range(n_streams)]
+            for t in th:
+                t.start()
+            for t in th:
+                t.join()
+
+        e2e_step()                                              # warm-up (grows the handles' arenas)
+        barrier()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(main_stream)
+        for _ in range(max(1, args.e2e_steps)):
+            e2e_step()
+        b.record(main_stream)
+        barrier()
+        e2e_ms = shard.max_over_ranks(a.elapsed_time(b), dev)
+        assert sum(totals) == n_vtx, "e2e path and device path disagree on the number of vertices"
+        h2d = 24 * sum(n_hits) + 24 * sum(n_seeds) + 2 * 4 * (events_rank + n_sub)
+        d2h = 56 * sum(n_seeds) + 40 * n_vtx + (4 + 8) * events_rank + 12 * n_sub
+        e2e = {"value": events_all * max(1, args.e2e_steps) / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
+               "d2h_bytes_per_step": d2h, "steps": max(1, args.e2e_steps), "ms_per_step": e2e_ms / max(1, args.e2e_steps),
+               "api": "ds_process_host, pinned host buffers, one handle + stream per thread"}
+        for h in handles:
+            h.close()
+
+    # ---- the oracle beside it (rank 0, N = 1) ------------------------------------------------------------------------------
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        n = sized_sample(first_sub, 15.0, args.subbatch)
+        v, dt, cores, _, _ = oracle_events_per_s(first_sub, n)
+        cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "seconds": dt,
+               "sample": f"first {n} events of cfg4 sub-batch 0 (oracle/ds_oracle.c, fp64, OpenMP over events)"}
+
+    if rank == 0:
+        print(json.dumps({
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "BASELINE configs[4]: cfg-1 generator, seed 4, device-resident SoA", "events_per_gpu": events_rank,
+                       "subbatches": n_sub, "events_per_subbatch": args.subbatch, "cuda_streams": n_streams,
+                       "hits": sum(n_hits), "seeds": sum(n_seeds), "tracks_found": n_found, "tracks_kept": n_keep, "vertices": n_vtx,
+                       "l2": "inputs larger than L2 (each sub-batch reads ~0.76 GB; 7.6 GB per step)",
+                       "parallelism": f"dp{world} (events sharded, no data-path collective)"},
+            "roofline": roofline, "whole_path_gbs": whole_gbs, "whole_path_frac": whole_gbs / peak, "kernels": kernels,
+            "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
+        }), flush=True)
+    ds.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -317,10 +317,11 @@ def take_events(data, n):
     out = dict(n_events=n, hit_offsets=data["hit_offsets"][: n + 1].copy(), seed_offsets=data["seed_offsets"][: n + 1].copy())
     out["hits"] = {k: v[:nh].copy() for k, v in data["hits"].items()}
     out["seeds"] = {k: v[:ns].copy() for k, v in data["seeds"].items()}
-    t = dict(data["truth"])
-    t["hit_particle"] = t["hit_particle"][:nh]
-    t["seed_particle"] = t["seed_particle"][:ns]
-    out["truth"] = t
+    if "truth" in data:
+        t = dict(data["truth"])
+        t["hit_particle"] = t["hit_particle"][:nh]
+        t["seed_particle"] = t["seed_particle"][:ns]
+        out["truth"] = t
     return out
 
 
@@ -354,7 +355,7 @@ def generate(cfg_index: int, n_events: int | None = None, first_block: int = 0, 
     jobs = [(cfg_index, first_block + b, B, np.dtype(dtype).name, seed) for b in range(nb)]
     if workers > 1 and nb > 1:
         import multiprocessing as mp
-        with mp.get_context("fork").Pool(min(workers, nb)) as pool:
+        with mp.get_context("spawn").Pool(min(workers, nb)) as pool:
             blocks = pool.map(_gen_one, jobs, chunksize=1)
     else:
         blocks = [_gen_one(j) for j in jobs]
