@@ -287,7 +287,7 @@ int ds_reconstruct(ds_handle *h, const ds_hits *hits, const ds_seeds *seeds, con
     set_inputs(L, hits);
     carve_layout(workspace, c.n_bins, n_events, hits->n, L);
     cudaError_t err = launch_layout(c, L, hit_offsets, n_events, p->max_event_hits_hint, st, h->prof);
-    if (err == cudaSuccess) err = launch_track(c, L, *seeds, hit_offsets, seed_offsets, n_events, *out, st, h->prof);
+    if (err == cudaSuccess) err = launch_track(c, L, *seeds, hit_offsets, seed_offsets, n_events, p->max_event_hits_hint, *out, st, h->prof);
     if (err == cudaSuccess) err = launch_mlp(c, h->d_mlp, *seeds, *out, st, h->prof);
     if (err != cudaSuccess) {
         cudaGetLastError();
@@ -396,7 +396,7 @@ int ds_process_host(ds_handle *h, const ds_hits *hits, const ds_seeds *seeds, co
     set_inputs(L, &dh);
     carve_layout(wrec, c.n_bins, n_events, hits->n, L);
     err = launch_layout(c, L, d_hoff, n_events, p->max_event_hits_hint, st, h->prof);
-    if (err == cudaSuccess) err = launch_track(c, L, dsd, d_hoff, d_soff, n_events, dt, st, h->prof);
+    if (err == cudaSuccess) err = launch_track(c, L, dsd, d_hoff, d_soff, n_events, p->max_event_hits_hint, dt, st, h->prof);
     if (err == cudaSuccess) err = launch_mlp(c, h->d_mlp, dsd, dt, st, h->prof);
     if (err == cudaSuccess) err = launch_vertex(c, dt, d_soff, n_events, dv, wvtx, st, h->prof);
     auto d2h = [&](void *dst, const void *src, size_t bytes) {

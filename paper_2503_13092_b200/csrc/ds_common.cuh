@@ -121,7 +121,8 @@ cudaError_t launch_layout(const DevConst &c, const LayoutPtrs &p, const int32_t 
 cudaError_t launch_extrapolate(const DevConst &c, const ds_seeds &seeds, double *out, cudaStream_t st);
 
 cudaError_t launch_track(const DevConst &c, const LayoutPtrs &lay, const ds_seeds &seeds, const int32_t *hit_offsets,
-                         const int32_t *seed_offsets, int n_events, const ds_tracks &out, cudaStream_t st, Prof &prof);
+                         const int32_t *seed_offsets, int n_events, int max_event_hits_hint, const ds_tracks &out,
+                         cudaStream_t st, Prof &prof);
 
 cudaError_t launch_mlp(const DevConst &c, const DevMlp *mlp, const ds_seeds &seeds, const ds_tracks &trk,
                        cudaStream_t st, Prof &prof);

@@ -3,21 +3,24 @@
 // per first hit a new trajectory through (hit, magnet point) and refined windows in UTaX/UTaU/UTbV keeping the
 // closest 1/2/2 hits; one final candidate per SciFi seed by score.  Readings A-1..A-9 in DESIGN.md.
 //
-// Mapping: one thread block per event.  Seeds are taken in chunks of blockDim.x: a thread-per-seed prefilter (S2 and
-// "is there any hit in the x0 slices the first window touches") rejects most fake seeds at once and queues the rest
-// in shared memory; then each warp takes queued seeds one at a time and works on them cooperatively:
-//   S3  lanes over the candidate hits of the window (coalesced x0 reads of the sorted SoA), ballot compaction;
-//       only if more than max_first hits pass, max_first selection passes by (distance, id)
-//   S4  lanes over (first hit, layer): 3 * n_first independent searches of a few hits each
-//   S5  lanes over combinations (first hit, i1, i2): every lane fits its own candidate
-//   S6  warp argmin of the score, ties resolved by (more hits, ids)
+// Mapping: one thread block per event.  The event's slice of the sorted x0 / ymin / ymax arrays (everything a window
+// search reads) is staged in shared memory by three 1-D bulk async copies (cp.async.bulk + mbarrier), issued by one
+// thread while the block loads the bin table.  The work is then flattened over the block in rounds of three phases:
+//   A  thread per seed:      S2, first window in UTbX (S3) -> the seed's <= max_first first hits appended to a block-wide
+//                            list (block scan of the counts; only if more hits pass than are tried, a selection by
+//                            (distance, id))
+//   B  thread per first hit: the three refined windows (S4), the <= 4 fits (S5) -> best score of this first hit
+//   C  thread per seed:      best first hit (S6; exact score ties resolved by (more hits, ids)), the winner's fit is
+//                            evaluated once more and the track record written, coalesced over the seeds
+// z, w, id and perm are read from global memory only for hits that passed a window.  Events larger than the staging
+// buffer run the same code on the global arrays.
 // All of this arithmetic is fp64 in registers on fp32 inputs (the deciding comparisons must agree with an fp64
 // reference to ~1e-5 relative; fp32 would not: one ulp of x at 800 mm is 6e-5 mm).
 #include "ds_common.cuh"
 
 namespace ds {
 
-constexpr int kTrackThreads = 128;
+constexpr int kTrackThreads = 256;
 constexpr int kTrackWarps = kTrackThreads / 32;
 constexpr int kMaxBins = 4 * DS_MAX_SECTORS * kXBins;
 
@@ -84,32 +87,209 @@ __device__ __forceinline__ void slice_range(const DevConst &c, const int *tab, i
     b = tab[base + xh + 1];
 }
 
-struct Cand {
-    double xh;   // measured x at the track's y
-    int idx;     // position in the event's sorted slice
-    int id;
-};
 
-struct WarpScratch {
-    Cand first[kMaxFirst];
-    Cand task[3 * kMaxFirst][2];
-    int tn[3 * kMaxFirst];
-};
+// ---- 1-D bulk async copy global -> shared, completion on an mbarrier (PTX ISA: cp.async.bulk, mbarrier) -------------
+__device__ __forceinline__ uint32_t smem_addr(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
-__device__ __forceinline__ bool key_less(double d1, int id1, double d2, int id2)
+__device__ __forceinline__ void mbar_init(unsigned long long *bar, int count)
 {
-    return d1 < d2 || (d1 == d2 && id1 < id2);
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_addr(bar)), "r"(count) : "memory");
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
 }
 
-struct SortedHits {   // the event's slice of the sorted SoA
-    const float *x0, *z, *ymin, *ymax, *w;
-    const int32_t *id, *perm;
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long *bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_addr(bar)), "r"(bytes) : "memory");
+}
+
+// dst, src 16-byte aligned, bytes a multiple of 16
+__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t bytes, unsigned long long *bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                     smem_addr(dst)),
+                 "l"(src), "r"(bytes), "r"(smem_addr(bar))
+                 : "memory");
+}
+
+__device__ __forceinline__ void mbar_wait(unsigned long long *bar, uint32_t parity)
+{
+    uint32_t ok = 0;
+    while (!ok) {
+        asm volatile(
+            "{\n"
+            ".reg .pred p;\n"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+            "selp.u32 %0, 1, 0, p;\n"
+            "}\n"
+            : "=r"(ok)
+            : "r"(smem_addr(bar)), "r"(parity)
+            : "memory");
+    }
+}
+
+constexpr int kFirstCap = 768;   // first hits handled per round (>= DS_MAX_FIRST_HITS)
+constexpr double kNoScore = 1e300;
+
+// Block-shared state of k_track (carved from dynamic shared memory, followed by the staged hit arrays).
+struct TrackShared {
+    unsigned long long bar;
+    double fscore[kFirstCap];             // phase B: best score of the first hit (kNoScore = no candidate)
+    int tab[kMaxBins + 1];                // the event's bin table
+    int fj[kFirstCap];                    // first-hit list: position of the UTbX hit in the event's sorted slice
+    float sx[kTrackThreads], sy[kTrackThreads], stx[kTrackThreads], sty[kTrackThreads], sqop[kTrackThreads];
+    int foff[kTrackThreads];              // where the seed's first hits start in the list
+    int warp_sums[kTrackWarps + 1];
+    int n_first;                          // entries of the first-hit list this round
+    unsigned short fs[kFirstCap];         // first-hit list: owning seed (thread index of this round)
+    unsigned char fn[kTrackThreads];      // number of first hits of the seed
+};
+
+// The event's hits as the searches see them: x0 / ymin / ymax from the staging buffer (or global for an oversize
+// event), the rest always from global memory.  Indices are relative to the event's sorted slice.
+struct EventHits {
+    const float *x0, *ymin, *ymax;   // shared or global
+    const float *z, *w;              // global
+    const int32_t *id, *perm;        // global
 };
 
 // y-compatibility of hit j (O-S3: ymin - y_tol <= y <= ymax + y_tol)
-__device__ __forceinline__ bool y_compatible(const DevConst &c, const SortedHits &H, int j, double y)
+__device__ __forceinline__ bool y_compatible(const DevConst &c, const EventHits &H, int j, double y)
 {
     return ((double)H.ymin[j] - c.y_tol <= y) && (y <= (double)H.ymax[j] + c.y_tol);
+}
+
+// (distance, id) order of the "closest hits" rules; ids are only read on an exact distance tie
+__device__ __forceinline__ bool closer(const EventHits &H, double d1, int j1, double d2, int j2)
+{
+    if (d1 != d2) return d1 < d2;
+    if (j2 < 0) return true;
+    return H.id[j1] < H.id[j2];
+}
+
+// Result of one refined-window search: the closest and second closest hit
+struct Near {
+    int n;          // hits kept (0..keepn)
+    int j0, j1;     // positions, -1 = none
+    double x0, x1;  // measured x at the track's y
+};
+
+// S4: closest `keepn` y-compatible hits of layer l within w1 of the prediction xp
+__device__ __forceinline__ Near search_layer(const DevConst &c, const EventHits &H, const int *tab, int l, double xp,
+                                             double y, double w1, int keepn)
+{
+    Near r;
+    r.n = 0; r.j0 = -1; r.j1 = -1; r.x0 = 0.0; r.x1 = 0.0;
+    double d0 = 1e300, d1 = 1e300;
+    const double off = c.dxdy[l] * y;
+    const double lo = xp - off - w1, hi = xp - off + w1;
+    int tl, th, n = 0;
+    sector_range(c, y, tl, th);
+    for (int sec = tl; sec <= th; ++sec) {
+        int a, b;
+        slice_range(c, tab, l, sec, lo, hi, a, b);
+        for (int j = a; j < b; ++j) {
+            const double xh = (double)H.x0[j] + off;
+            const double d = fabs(xh - xp);
+            if (d <= w1 && y_compatible(c, H, j, y)) {
+                if (closer(H, d, j, d0, r.j0)) {
+                    d1 = d0; r.j1 = r.j0; r.x1 = r.x0;
+                    d0 = d; r.j0 = j; r.x0 = xh;
+                } else if (closer(H, d, j, d1, r.j1)) {
+                    d1 = d; r.j1 = j; r.x1 = xh;
+                }
+                ++n;
+            }
+        }
+    }
+    r.n = min(n, keepn);
+    if (r.n < 2) r.j1 = -1;
+    if (r.n < 1) r.j0 = -1;
+    return r;
+}
+
+// Best candidate of one first hit (S4 + S5 and the part of S6 that stays inside the first hit).
+struct FirstBest {
+    double score, a, b, chi2;   // score = kNoScore: no candidate
+    int nh, j0, j1, j2, j3;     // chosen hits (positions in the event's sorted slice), -1 = layer missing
+};
+
+// A-9 order of two candidates with the same score: more hits, then smaller (id3, id0, id1, id2); missing = INT32_MAX
+__device__ __forceinline__ bool tie_better(const EventHits &H, const FirstBest &p, const FirstBest &q)
+{
+    if (p.nh != q.nh) return p.nh > q.nh;
+    const int pj[4] = {p.j3, p.j0, p.j1, p.j2}, qj[4] = {q.j3, q.j0, q.j1, q.j2};
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const int pi = pj[k] >= 0 ? H.id[pj[k]] : INT32_MAX, qi = qj[k] >= 0 ? H.id[qj[k]] : INT32_MAX;
+        if (pi != qi) return pi < qi;
+    }
+    return false;
+}
+
+__device__ FirstBest eval_first_hit(const DevConst &c, const EventHits &H, const int *tab, const S2 &s2, int j3)
+{
+    FirstBest best;
+    best.score = kNoScore; best.a = 0.0; best.b = 0.0; best.chi2 = 0.0;
+    best.nh = 0; best.j0 = -1; best.j1 = -1; best.j2 = -1; best.j3 = j3;
+
+    // S4: trajectory through (first hit, magnet point), refined windows
+    const double x3 = (double)H.x0[j3] + c.dxdy[3] * s2.y3;
+    const double z3 = (double)H.z[j3];
+    const double txc = (x3 - s2.xm) / (z3 - s2.zm);
+    const Near n0 = search_layer(c, H, tab, 0, s2.xm + txc * (c.z_layer[0] - s2.zm), s2.y0, s2.w1, 1);
+    const Near n1 = search_layer(c, H, tab, 1, s2.xm + txc * (c.z_layer[1] - s2.zm), s2.y1, s2.w1, 2);
+    const Near n2 = search_layer(c, H, tab, 2, s2.xm + txc * (c.z_layer[2] - s2.zm), s2.y2, s2.w1, 2);
+    const int nh = 1 + (n0.n > 0) + (n1.n > 0) + (n2.n > 0);
+    if (nh < c.min_hits) return best;
+
+    // S5: weighted line through the hits and the magnet point (A-8); terms shared by all combinations first
+    const double w3 = (double)H.w[j3];
+    const double pz3 = z3 - c.z_ref, pzm = s2.zm - c.z_ref;
+    double pz0 = 0.0, pw0 = 0.0, px0 = 0.0;
+    if (n0.n > 0) { pz0 = (double)H.z[n0.j0] - c.z_ref; pw0 = (double)H.w[n0.j0]; px0 = n0.x0; }
+    const double ndf = (double)(nh - 1);
+    const int m1 = max(n1.n, 1), m2 = max(n2.n, 1);
+    for (int i1 = 0; i1 < m1; ++i1) {
+        const int j1 = n1.n > 0 ? (i1 ? n1.j1 : n1.j0) : -1;
+        double pz1 = 0.0, pw1 = 0.0, px1 = 0.0;
+        if (j1 >= 0) { pz1 = (double)H.z[j1] - c.z_ref; pw1 = (double)H.w[j1]; px1 = i1 ? n1.x1 : n1.x0; }
+        for (int i2 = 0; i2 < m2; ++i2) {
+            const int j2 = n2.n > 0 ? (i2 ? n2.j1 : n2.j0) : -1;
+            double pz2 = 0.0, pw2 = 0.0, px2 = 0.0;
+            if (j2 >= 0) { pz2 = (double)H.z[j2] - c.z_ref; pw2 = (double)H.w[j2]; px2 = i2 ? n2.x1 : n2.x0; }
+            const double pz[5] = {pz0, pz1, pz2, pz3, pzm};
+            const double px[5] = {px0, px1, px2, x3, s2.xm};
+            const double pw[5] = {pw0, pw1, pw2, w3, c.w_mag};
+            double S = 0, Sz = 0, Szz = 0, Sx = 0, Sxz = 0;
+#pragma unroll
+            for (int k = 0; k < 5; ++k) {
+                S += pw[k];
+                Sz += pw[k] * pz[k];
+                Szz += pw[k] * pz[k] * pz[k];
+                Sx += pw[k] * px[k];
+                Sxz += pw[k] * px[k] * pz[k];
+            }
+            const double D = S * Szz - Sz * Sz;
+            const double fb = (S * Sxz - Sz * Sx) / D;
+            const double fa = (Szz * Sx - Sz * Sxz) / D;
+            double chi2 = 0.0;
+#pragma unroll
+            for (int k = 0; k < 5; ++k) {
+                const double r = px[k] - fa - fb * pz[k];
+                chi2 += pw[k] * r * r;
+            }
+            if (!(chi2 / ndf <= c.chi2ndf_max)) continue;
+            FirstBest cand;
+            cand.score = chi2 + c.miss_penalty * (double)(4 - nh);
+            cand.a = fa; cand.b = fb; cand.chi2 = chi2;
+            cand.nh = nh; cand.j0 = n0.j0; cand.j1 = j1; cand.j2 = j2; cand.j3 = j3;
+            if (best.score == kNoScore || cand.score < best.score ||
+                (cand.score == best.score && tie_better(H, cand, best)))
+                best = cand;
+        }
+    }
+    return best;
 }
 
 __device__ __forceinline__ void write_not_found(const ds_tracks &out, int64_t s)
@@ -119,296 +299,235 @@ __device__ __forceinline__ void write_not_found(const ds_tracks &out, int64_t s)
     reinterpret_cast<int4 *>(out.hit)[s] = make_int4(-1, -1, -1, -1);
 }
 
-// One seed, whole warp.  Returns through `out` slot s.
-__device__ void reconstruct_seed(const DevConst &c, const SortedHits &H, const int *tab, WarpScratch &ws, const S2 &s2,
-                                 double ys, double txs, double tys, int64_t s, const ds_tracks &out)
+// inclusive scan of one int per thread over the block; every thread of the block calls it
+__device__ __forceinline__ int block_inclusive_scan(int v, int *warp_sums)
 {
-    const int lane = threadIdx.x & 31;
-    const unsigned FULL = 0xffffffffu;
-    const int max_first = c.max_first;
-
-    // ---- S3: first window in UTbX (layer 3) -------------------------------------------------------------------
-    int s_lo, s_hi;
-    sector_range(c, s2.y3, s_lo, s_hi);
-    const double off3 = c.dxdy[3] * s2.y3;
-    const double lo3 = s2.xc3 - off3 - s2.w0, hi3 = s2.xc3 - off3 + s2.w0;
-    int nF = 0;
-    for (int sec = s_lo; sec <= s_hi; ++sec) {
-        int a, b;
-        slice_range(c, tab, 3, sec, lo3, hi3, a, b);
-        for (int base = a; base < b; base += 32) {
-            const int j = base + lane;
-            bool pass = false;
-            double xh = 0.0;
-            if (j < b) {
-                xh = (double)H.x0[j] + off3;
-                pass = fabs(xh - s2.xc3) <= s2.w0 && y_compatible(c, H, j, s2.y3);
-            }
-            const unsigned m = __ballot_sync(FULL, pass);
-            if (pass) {
-                const int pos = nF + __popc(m & lanemask_lt());
-                if (pos < max_first) ws.first[pos] = Cand{xh, j, 0};
-            }
-            nF += __popc(m);
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    int inc = v;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const int t = __shfl_up_sync(0xffffffffu, inc, d);
+        if (lane >= d) inc += t;
+    }
+    if (lane == 31) warp_sums[wid] = inc;
+    __syncthreads();
+    if (wid == 0) {
+        const int ws = lane < kTrackWarps ? warp_sums[lane] : 0;
+        int wi = ws;
+#pragma unroll
+        for (int d = 1; d < kTrackWarps; d <<= 1) {
+            const int t = __shfl_up_sync(0xffffffffu, wi, d);
+            if (lane >= d) wi += t;
         }
+        if (lane < kTrackWarps) warp_sums[lane] = wi - ws;
     }
-    if (nF == 0) {
-        if (lane == 0) write_not_found(out, s);
-        return;
-    }
-    if (nF > max_first) {
-        // more hits in the window than are tried: keep the max_first closest by (distance, id)
-        double last_d = -1.0;
-        int last_id = INT32_MIN;
-        for (int k = 0; k < max_first; ++k) {
-            double bd = 1e300, bxh = 0.0;
-            int bid = INT32_MAX, bj = -1;
+    __syncthreads();
+    return inc + warp_sums[wid];
+}
+
+// All seeds of one event.  Every thread of the block runs this with the same arguments.
+__device__ __forceinline__ void track_event(const DevConst &c, TrackShared &sh, const EventHits &H, const ds_seeds &seeds,
+                                            int s_begin, int s_end, const ds_tracks &out)
+{
+    const int tid = threadIdx.x;
+    const int max_first = c.max_first;
+    const int *tab = sh.tab;
+    int s_base = s_begin;
+    while (s_base < s_end) {
+        // ---- phase A: thread per seed -- S2, S3 ------------------------------------------------------------------------
+        const int s = s_base + tid;
+        const bool act = s < s_end;
+        S2 s2;
+        int s_lo = 0, s_hi = -1, nF = 0;
+        double off3 = 0.0, lo3 = 0.0, hi3 = 0.0;
+        if (act) {
+            const float fx = seeds.x[s], fy = seeds.y[s], ftx = seeds.tx[s], fty = seeds.ty[s], fq = seeds.qop[s];
+            sh.sx[tid] = fx; sh.sy[tid] = fy; sh.stx[tid] = ftx; sh.sty[tid] = fty; sh.sqop[tid] = fq;
+            s2 = extrapolate_seed(c, fx, fy, ftx, fty, fq);
+            sector_range(c, s2.y3, s_lo, s_hi);
+            off3 = c.dxdy[3] * s2.y3;
+            lo3 = s2.xc3 - off3 - s2.w0;
+            hi3 = s2.xc3 - off3 + s2.w0;
             for (int sec = s_lo; sec <= s_hi; ++sec) {
                 int a, b;
                 slice_range(c, tab, 3, sec, lo3, hi3, a, b);
-                for (int j = a + lane; j < b; j += 32) {
+                for (int j = a; j < b; ++j) {
                     const double xh = (double)H.x0[j] + off3;
-                    const double d = fabs(xh - s2.xc3);
-                    if (d <= s2.w0 && y_compatible(c, H, j, s2.y3)) {
-                        const int id = H.id[j];
-                        if (key_less(last_d, last_id, d, id) && key_less(d, id, bd, bid)) {
-                            bd = d; bid = id; bj = j; bxh = xh;
+                    nF += (fabs(xh - s2.xc3) <= s2.w0 && y_compatible(c, H, j, s2.y3)) ? 1 : 0;
+                }
+            }
+        }
+        const int nFc = min(nF, max_first);
+        const int incl = block_inclusive_scan(nFc, sh.warp_sums);
+        // the seeds taken this round are the longest prefix whose first hits fit the list
+        const bool take = act && incl <= kFirstCap;
+        const int n_take = __syncthreads_count(take);
+        if (take && tid == n_take - 1) sh.n_first = incl;
+        if (take) {
+            int pos = incl - nFc;
+            sh.foff[tid] = pos;
+            sh.fn[tid] = (unsigned char)nFc;
+            if (nF <= max_first) {
+                for (int sec = s_lo; sec <= s_hi; ++sec) {
+                    int a, b;
+                    slice_range(c, tab, 3, sec, lo3, hi3, a, b);
+                    for (int j = a; j < b; ++j) {
+                        const double xh = (double)H.x0[j] + off3;
+                        if (fabs(xh - s2.xc3) <= s2.w0 && y_compatible(c, H, j, s2.y3)) {
+                            sh.fj[pos] = j;
+                            sh.fs[pos] = (unsigned short)tid;
+                            ++pos;
                         }
                     }
                 }
-            }
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) {
-                const double od = __shfl_xor_sync(FULL, bd, o), oxh = __shfl_xor_sync(FULL, bxh, o);
-                const int oid = __shfl_xor_sync(FULL, bid, o), oj = __shfl_xor_sync(FULL, bj, o);
-                if (key_less(od, oid, bd, bid)) { bd = od; bid = oid; bj = oj; bxh = oxh; }
-            }
-            if (lane == 0) ws.first[k] = Cand{bxh, bj, bid};
-            last_d = bd;
-            last_id = bid;
-        }
-        nF = max_first;
-    }
-    __syncwarp();
-
-    // ---- S4: refined windows, lanes over (first hit, layer) -----------------------------------------------------------
-    const int nT = 3 * nF;
-    if (lane < nT) {
-        const int f = lane / 3, l = lane - 3 * f;
-        const Cand fh = ws.first[f];
-        const double zf = (double)H.z[fh.idx];
-        const double txc = (fh.xh - s2.xm) / (zf - s2.zm);
-        const double xp = s2.xm + txc * (c.z_layer[l] - s2.zm);
-        const double y = l == 0 ? s2.y0 : (l == 1 ? s2.y1 : s2.y2);
-        const double off = c.dxdy[l] * y;
-        const double lo = xp - off - s2.w1, hi = xp - off + s2.w1;
-        const int keepn = l == 0 ? 1 : 2;
-        double d0 = 1e300, d1 = 1e300;
-        Cand c0 = Cand{0.0, -1, INT32_MAX}, c1 = c0;
-        int n = 0, tl, th;
-        sector_range(c, y, tl, th);
-        for (int sec = tl; sec <= th; ++sec) {
-            int a, b;
-            slice_range(c, tab, l, sec, lo, hi, a, b);
-            for (int j = a; j < b; ++j) {
-                const double xh = (double)H.x0[j] + off;
-                const double d = fabs(xh - xp);
-                if (d <= s2.w1 && y_compatible(c, H, j, y)) {
-                    const int id = H.id[j];
-                    if (key_less(d, id, d0, c0.id)) {
-                        d1 = d0; c1 = c0;
-                        d0 = d; c0 = Cand{xh, j, id};
-                    } else if (key_less(d, id, d1, c1.id)) {
-                        d1 = d; c1 = Cand{xh, j, id};
+            } else {
+                // more hits in the window than are tried: the max_first closest by (distance, id)
+                double last_d = -1.0;
+                int last_j = -1;
+                for (int k = 0; k < max_first; ++k) {
+                    double bd = 1e300;
+                    int bj = -1;
+                    for (int sec = s_lo; sec <= s_hi; ++sec) {
+                        int a, b;
+                        slice_range(c, tab, 3, sec, lo3, hi3, a, b);
+                        for (int j = a; j < b; ++j) {
+                            const double xh = (double)H.x0[j] + off3;
+                            const double d = fabs(xh - s2.xc3);
+                            if (d <= s2.w0 && y_compatible(c, H, j, s2.y3)) {
+                                // strictly after the previous pick, and before the best so far
+                                const bool after = last_j < 0 || (j != last_j && closer(H, last_d, last_j, d, j));
+                                if (after && closer(H, d, j, bd, bj)) { bd = d; bj = j; }
+                            }
+                        }
                     }
-                    ++n;
+                    sh.fj[pos] = bj;
+                    sh.fs[pos] = (unsigned short)tid;
+                    ++pos;
+                    last_d = bd;
+                    last_j = bj;
                 }
             }
         }
-        ws.tn[lane] = min(n, keepn);
-        ws.task[lane][0] = c0;
-        ws.task[lane][1] = c1;
-    }
-    __syncwarp();
-
-    // ---- S5: lanes over combinations (first hit f, i1, i2); S6: best by (score, more hits, id3, id0, id1, id2) -----------------
-    double b_score = 1e300, b_a = 0.0, b_b = 0.0, b_chi2 = 0.0;
-    int b_nh = 0, b_i0 = -1, b_i1 = -1, b_i2 = -1, b_i3 = -1;
-    int b_id0 = INT32_MAX, b_id1 = INT32_MAX, b_id2 = INT32_MAX, b_id3 = INT32_MAX;
-    bool b_ok = false;
-    for (int cb = lane; cb < 4 * nF; cb += 32) {
-        const int f = cb >> 2, i1 = (cb >> 1) & 1, i2 = cb & 1;
-        const int n0 = ws.tn[3 * f], n1 = ws.tn[3 * f + 1], n2 = ws.tn[3 * f + 2];
-        if (i1 >= max(n1, 1) || i2 >= max(n2, 1)) continue;
-        const int nh = 1 + (n0 > 0) + (n1 > 0) + (n2 > 0);
-        if (nh < c.min_hits) continue;
-        Cand h[4];
-        h[0] = ws.task[3 * f][0];
-        h[1] = ws.task[3 * f + 1][i1];
-        h[2] = ws.task[3 * f + 2][i2];
-        h[3] = ws.first[f];
-        if (n0 == 0) h[0].idx = -1;
-        if (n1 == 0) h[1].idx = -1;
-        if (n2 == 0) h[2].idx = -1;
-        double pz[5], px[5], pw[5];
-        double S = 0, Sz = 0, Szz = 0, Sx = 0, Sxz = 0;
-#pragma unroll
-        for (int k = 0; k < 5; ++k) {
-            bool use = true;
-            if (k < 4) {
-                use = h[k].idx >= 0;
-                const int j = use ? h[k].idx : 0;
-                pz[k] = (double)H.z[j] - c.z_ref;
-                px[k] = h[k].xh;
-                pw[k] = use ? (double)H.w[j] : 0.0;
-            } else {   // magnet point pseudo-measurement (A-8)
-                pz[k] = s2.zm - c.z_ref;
-                px[k] = s2.xm;
-                pw[k] = c.w_mag;
+        __syncthreads();
+        // ---- phase B: thread per first hit -- S4, S5 ---------------------------------------------------------------
+        const int n_first = sh.n_first;
+        for (int f = tid; f < n_first; f += kTrackThreads) {
+            const int o = sh.fs[f];
+            const S2 t2 = extrapolate_seed(c, sh.sx[o], sh.sy[o], sh.stx[o], sh.sty[o], sh.sqop[o]);
+            sh.fscore[f] = eval_first_hit(c, H, tab, t2, sh.fj[f]).score;
+        }
+        __syncthreads();
+        // ---- phase C: thread per seed -- S6 and the track record ------------------------------------------------------
+        if (take) {
+            const int f0 = sh.foff[tid];
+            int fbest = -1;
+            double sbest = kNoScore;
+            bool tied = false;
+            for (int k = 0; k < nFc; ++k) {
+                const double sc = sh.fscore[f0 + k];
+                if (sc < sbest) { sbest = sc; fbest = f0 + k; tied = false; }
+                else if (sc == sbest && sc != kNoScore) tied = true;
             }
-            if (!use) px[k] = 0.0;
-            S += pw[k];
-            Sz += pw[k] * pz[k];
-            Szz += pw[k] * pz[k] * pz[k];
-            Sx += pw[k] * px[k];
-            Sxz += pw[k] * px[k] * pz[k];
+            if (fbest < 0) {
+                write_not_found(out, s);
+            } else {
+                FirstBest w = eval_first_hit(c, H, tab, s2, sh.fj[fbest]);
+                if (tied) {   // equal scores in different first hits (duplicate hits): more hits, then ids (A-9)
+                    for (int k = 0; k < nFc; ++k) {
+                        if (f0 + k == fbest || sh.fscore[f0 + k] != sbest) continue;
+                        const FirstBest q = eval_first_hit(c, H, tab, s2, sh.fj[f0 + k]);
+                        if (tie_better(H, q, w)) w = q;
+                    }
+                }
+                const double ys = (double)sh.sy[tid], txs = (double)sh.stx[tid], tys = (double)sh.sty[tid];
+                out.x[s] = (float)w.a;
+                out.y[s] = (float)(ys + tys * (c.z_ref - c.z_seed));
+                out.tx[s] = (float)w.b;
+                out.ty[s] = (float)tys;
+                out.qop[s] = (float)((txs - w.b) / c.kick);
+                out.chi2[s] = (float)w.chi2;
+                out.nhits[s] = w.nh;
+                out.found[s] = 1;
+                int4 hv;
+                hv.x = w.j0 >= 0 ? H.perm[w.j0] : -1;
+                hv.y = w.j1 >= 0 ? H.perm[w.j1] : -1;
+                hv.z = w.j2 >= 0 ? H.perm[w.j2] : -1;
+                hv.w = H.perm[w.j3];
+                reinterpret_cast<int4 *>(out.hit)[s] = hv;
+            }
         }
-        const double D = S * Szz - Sz * Sz;
-        const double fb = (S * Sxz - Sz * Sx) / D;
-        const double fa = (Szz * Sx - Sz * Sxz) / D;
-        double chi2 = 0.0;
-#pragma unroll
-        for (int k = 0; k < 5; ++k) {
-            const double r = px[k] - fa - fb * pz[k];
-            chi2 += pw[k] * r * r;
-        }
-        const double ndf = (double)(nh - 1);
-        if (!(chi2 / ndf <= c.chi2ndf_max)) continue;
-        const double score = chi2 + c.miss_penalty * (double)(4 - nh);
-        const int id0 = h[0].idx >= 0 ? h[0].id : INT32_MAX;
-        const int id1 = h[1].idx >= 0 ? h[1].id : INT32_MAX;
-        const int id2 = h[2].idx >= 0 ? h[2].id : INT32_MAX;
-        const int id3 = H.id[h[3].idx];
-        bool better = !b_ok;
-        if (b_ok) {
-            if (score != b_score) better = score < b_score;
-            else if (nh != b_nh) better = nh > b_nh;
-            else if (id3 != b_id3) better = id3 < b_id3;
-            else if (id0 != b_id0) better = id0 < b_id0;
-            else if (id1 != b_id1) better = id1 < b_id1;
-            else better = id2 < b_id2;
-        }
-        if (better) {
-            b_ok = true; b_score = score; b_a = fa; b_b = fb; b_chi2 = chi2; b_nh = nh;
-            b_i0 = h[0].idx; b_i1 = h[1].idx; b_i2 = h[2].idx; b_i3 = h[3].idx;
-            b_id0 = id0; b_id1 = id1; b_id2 = id2; b_id3 = id3;
-        }
-    }
-    // warp argmin
-    double smin = b_ok ? b_score : 1e300;
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) smin = fmin(smin, __shfl_xor_sync(FULL, smin, o));
-    unsigned tied = __ballot_sync(FULL, b_ok && b_score == smin);
-    if (tied == 0) {
-        if (lane == 0) write_not_found(out, s);
-        return;
-    }
-    int win = __ffs(tied) - 1;
-    unsigned rest = tied & (tied - 1);
-    while (rest) {   // equal scores (duplicate hits): more hits, then (id3, id0, id1, id2)
-        const int t = __ffs(rest) - 1;
-        rest &= rest - 1;
-        const int nh_t = __shfl_sync(FULL, b_nh, t), nh_w = __shfl_sync(FULL, b_nh, win);
-        const int a3 = __shfl_sync(FULL, b_id3, t), w3 = __shfl_sync(FULL, b_id3, win);
-        const int a0 = __shfl_sync(FULL, b_id0, t), w0 = __shfl_sync(FULL, b_id0, win);
-        const int a1 = __shfl_sync(FULL, b_id1, t), w1 = __shfl_sync(FULL, b_id1, win);
-        const int a2 = __shfl_sync(FULL, b_id2, t), w2 = __shfl_sync(FULL, b_id2, win);
-        bool better;
-        if (nh_t != nh_w) better = nh_t > nh_w;
-        else if (a3 != w3) better = a3 < w3;
-        else if (a0 != w0) better = a0 < w0;
-        else if (a1 != w1) better = a1 < w1;
-        else better = a2 < w2;
-        if (better) win = t;
-    }
-    if (lane == win) {
-        out.x[s] = (float)b_a;
-        out.y[s] = (float)(ys + tys * (c.z_ref - c.z_seed));
-        out.tx[s] = (float)b_b;
-        out.ty[s] = (float)tys;
-        out.qop[s] = (float)((txs - b_b) / c.kick);
-        out.chi2[s] = (float)b_chi2;
-        out.nhits[s] = b_nh;
-        out.found[s] = 1;
-        int4 hv;
-        hv.x = b_i0 >= 0 ? H.perm[b_i0] : -1;
-        hv.y = b_i1 >= 0 ? H.perm[b_i1] : -1;
-        hv.z = b_i2 >= 0 ? H.perm[b_i2] : -1;
-        hv.w = H.perm[b_i3];
-        reinterpret_cast<int4 *>(out.hit)[s] = hv;
+        s_base += n_take;
+        __syncthreads();   // the lists are rewritten by the next round
     }
 }
 
 __global__ void __launch_bounds__(kTrackThreads)
 k_track(const __grid_constant__ DevConst c, const LayoutPtrs L, const ds_seeds seeds,
-        const int32_t *__restrict__ hit_offsets, const int32_t *__restrict__ seed_offsets, const ds_tracks out)
+        const int32_t *__restrict__ hit_offsets, const int32_t *__restrict__ seed_offsets, const ds_tracks out, int cap)
 {
-    __shared__ int tab[kMaxBins + 1];
-    __shared__ int queue[kTrackThreads];
-    __shared__ int n_queue;
-    __shared__ WarpScratch scratch[kTrackWarps];
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    TrackShared &sh = *reinterpret_cast<TrackShared *>(smem_raw);
+    constexpr size_t kHitsAt = (sizeof(TrackShared) + 15) & ~(size_t)15;
+    float *st_x0 = reinterpret_cast<float *>(smem_raw + kHitsAt);   // [cap], then ymin [cap], ymax [cap]
+    float *st_ymin = st_x0 + cap, *st_ymax = st_ymin + cap;
 
     const int e = blockIdx.x;
-    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
-    const int h0 = hit_offsets[e];
+    const int tid = threadIdx.x;
     const int s_begin = seed_offsets[e], s_end = seed_offsets[e + 1];
     if (s_begin == s_end) return;
+    const int h0 = hit_offsets[e], h1 = hit_offsets[e + 1];
+    // staged range: the event's slice widened to 16-byte boundaries (the sorted arrays are 256-byte aligned and padded)
+    const int h0a = h0 & ~3, cnt = ((h1 + 3) & ~3) - h0a;
+    const bool staged = cnt <= cap;
+    if (tid == 0 && staged) {
+        mbar_init(&sh.bar, 1);
+        const uint32_t bytes = 4u * (uint32_t)cnt;
+        mbar_expect_tx(&sh.bar, 3u * bytes);
+        if (bytes) {
+            bulk_g2s(st_x0, L.sx0 + h0a, bytes, &sh.bar);
+            bulk_g2s(st_ymin, L.symin + h0a, bytes, &sh.bar);
+            bulk_g2s(st_ymax, L.symax + h0a, bytes, &sh.bar);
+        }
+    }
     const int nb = c.n_bins;
     const int32_t *gtab = L.bin_offsets + (size_t)e * (nb + 1);
-    for (int b = tid; b <= nb; b += kTrackThreads) tab[b] = gtab[b];
-    SortedHits H;
-    H.x0 = L.sx0 + h0; H.z = L.sz + h0; H.ymin = L.symin + h0; H.ymax = L.symax + h0; H.w = L.sw + h0;
-    H.id = L.sid + h0; H.perm = L.perm + h0;
+    for (int b = tid; b <= nb; b += kTrackThreads) sh.tab[b] = gtab[b];
+    __syncthreads();
 
-    for (int chunk = s_begin; chunk < s_end; chunk += kTrackThreads) {
-        if (tid == 0) n_queue = 0;
-        __syncthreads();   // also orders the table load before its first use
-        // ---- prefilter: thread per seed (S2 + any hit in the slices of the first window?) ----------------------------
-        const int s = chunk + tid;
-        if (s < s_end) {
-            const S2 s2 = extrapolate_seed(c, seeds.x[s], seeds.y[s], seeds.tx[s], seeds.ty[s], seeds.qop[s]);
-            int s_lo, s_hi, cnt = 0;
-            sector_range(c, s2.y3, s_lo, s_hi);
-            const double off3 = c.dxdy[3] * s2.y3;
-            for (int sec = s_lo; sec <= s_hi; ++sec) {
-                int a, b;
-                slice_range(c, tab, 3, sec, s2.xc3 - off3 - s2.w0, s2.xc3 - off3 + s2.w0, a, b);
-                cnt += b - a;
-            }
-            if (cnt > 0) queue[atomicAdd(&n_queue, 1)] = s;
-            else write_not_found(out, s);
-        }
-        __syncthreads();
-        // ---- warp per queued seed ------------------------------------------------------------------------------------
-        const int nq = n_queue;
-        for (int q = wid; q < nq; q += kTrackWarps) {
-            const int sq = queue[q];
-            const double xs = seeds.x[sq], ys = seeds.y[sq], txs = seeds.tx[sq], tys = seeds.ty[sq], qop = seeds.qop[sq];
-            const S2 s2 = extrapolate_seed(c, xs, ys, txs, tys, qop);
-            reconstruct_seed(c, H, tab, scratch[wid], s2, ys, txs, tys, sq, out);
-            __syncwarp();
-        }
-        __syncthreads();
+    EventHits H;
+    H.z = L.sz + h0; H.w = L.sw + h0; H.id = L.sid + h0; H.perm = L.perm + h0;
+    if (staged) {
+        mbar_wait(&sh.bar, 0);
+        const int d = h0 - h0a;
+        H.x0 = st_x0 + d; H.ymin = st_ymin + d; H.ymax = st_ymax + d;
+        track_event(c, sh, H, seeds, s_begin, s_end, out);
+    } else {
+        H.x0 = L.sx0 + h0; H.ymin = L.symin + h0; H.ymax = L.symax + h0;
+        track_event(c, sh, H, seeds, s_begin, s_end, out);
     }
-    (void)lane;
 }
 
+static int g_track_smem_set = -1;
+
 cudaError_t launch_track(const DevConst &c, const LayoutPtrs &lay, const ds_seeds &seeds, const int32_t *hit_offsets,
-                         const int32_t *seed_offsets, int n_events, const ds_tracks &out, cudaStream_t st, Prof &prof)
+                         const int32_t *seed_offsets, int n_events, int max_event_hits_hint, const ds_tracks &out,
+                         cudaStream_t st, Prof &prof)
 {
     if (n_events <= 0) return cudaSuccess;
+    // staging capacity in hits (a multiple of 4, with room for the alignment slack): 12 bytes each
+    const int hint = max_event_hits_hint > 0 ? max_event_hits_hint : 4096;
+    const size_t fixed = ((sizeof(TrackShared) + 15) & ~(size_t)15);
+    const int cap_max = (int)((227 * 1024 - fixed) / 12) & ~3;
+    int cap = ((hint + 3) & ~3) + 8;
+    if (cap > cap_max) cap = cap_max;
+    const size_t smem = fixed + (size_t)cap * 12;
+    if ((int)smem > g_track_smem_set) {
+        cudaError_t err = cudaFuncSetAttribute(k_track, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (err != cudaSuccess) return err;
+        g_track_smem_set = (int)smem;
+    }
     prof.begin(DS_K_TRACK, st);
-    k_track<<<n_events, kTrackThreads, 0, st>>>(c, lay, seeds, hit_offsets, seed_offsets, out);
+    k_track<<<n_events, kTrackThreads, smem, st>>>(c, lay, seeds, hit_offsets, seed_offsets, out, cap);
     prof.end(st);
     return cudaGetLastError();
 }
