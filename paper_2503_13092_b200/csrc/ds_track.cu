@@ -128,20 +128,21 @@ __device__ __forceinline__ void mbar_wait(unsigned long long *bar, uint32_t pari
     }
 }
 
-constexpr int kFirstCap = 768;   // first hits handled per round (>= DS_MAX_FIRST_HITS)
+
+constexpr int kFirstCap = 512;   // first hits handled per round (>= DS_MAX_FIRST_HITS)
 constexpr double kNoScore = 1e300;
 
 // Block-shared state of k_track (carved from dynamic shared memory, followed by the staged hit arrays).
 struct TrackShared {
     unsigned long long bar;
-    double fscore[kFirstCap];             // phase B: best score of the first hit (kNoScore = no candidate)
+    int2 near[3 * kFirstCap];             // phase B: closest / second closest hit of (first hit, layer), -1 = none
     int tab[kMaxBins + 1];                // the event's bin table
-    int fj[kFirstCap];                    // first-hit list: position of the UTbX hit in the event's sorted slice
+    int slot[kTrackThreads * kMaxFirst];  // phase A: the seed's first hits (positions in the event's sorted slice)
     float sx[kTrackThreads], sy[kTrackThreads], stx[kTrackThreads], sty[kTrackThreads], sqop[kTrackThreads];
-    int foff[kTrackThreads];              // where the seed's first hits start in the list
+    int foff[kTrackThreads];              // where the seed's first hits start in the round's list
     int warp_sums[kTrackWarps + 1];
     int n_first;                          // entries of the first-hit list this round
-    unsigned short fs[kFirstCap];         // first-hit list: owning seed (thread index of this round)
+    unsigned short fs[kFirstCap];         // first-hit list: index into slot[]
     unsigned char fn[kTrackThreads];      // number of first hits of the seed
 };
 
@@ -153,10 +154,11 @@ struct EventHits {
     const int32_t *id, *perm;        // global
 };
 
-// y-compatibility of hit j (O-S3: ymin - y_tol <= y <= ymax + y_tol)
+// y-compatibility of hit j (O-S3: ymin - y_tol <= y <= ymax + y_tol); no short circuit: both loads are always issued
 __device__ __forceinline__ bool y_compatible(const DevConst &c, const EventHits &H, int j, double y)
 {
-    return ((double)H.ymin[j] - c.y_tol <= y) && (y <= (double)H.ymax[j] + c.y_tol);
+    const double lo = (double)H.ymin[j] - c.y_tol, hi = (double)H.ymax[j] + c.y_tol;
+    return (lo <= y) & (y <= hi);
 }
 
 // (distance, id) order of the "closest hits" rules; ids are only read on an exact distance tie
@@ -167,55 +169,93 @@ __device__ __forceinline__ bool closer(const EventHits &H, double d1, int j1, do
     return H.id[j1] < H.id[j2];
 }
 
-// Result of one refined-window search: the closest and second closest hit
-struct Near {
-    int n;          // hits kept (0..keepn)
-    int j0, j1;     // positions, -1 = none
-    double x0, x1;  // measured x at the track's y
-};
-
-// S4: closest `keepn` y-compatible hits of layer l within w1 of the prediction xp
-__device__ __forceinline__ Near search_layer(const DevConst &c, const EventHits &H, const int *tab, int l, double xp,
-                                             double y, double w1, int keepn)
+// S4: closest and second closest y-compatible hit of layer l within w1 of the prediction xp; -1 = none
+__device__ __forceinline__ int2 search_layer(const DevConst &c, const EventHits &H, const int *tab, int l, double xp,
+                                             double y, double w1)
 {
-    Near r;
-    r.n = 0; r.j0 = -1; r.j1 = -1; r.x0 = 0.0; r.x1 = 0.0;
+    int j0 = -1, j1 = -1;
     double d0 = 1e300, d1 = 1e300;
     const double off = c.dxdy[l] * y;
     const double lo = xp - off - w1, hi = xp - off + w1;
-    int tl, th, n = 0;
+    int tl, th;
     sector_range(c, y, tl, th);
     for (int sec = tl; sec <= th; ++sec) {
         int a, b;
         slice_range(c, tab, l, sec, lo, hi, a, b);
         for (int j = a; j < b; ++j) {
-            const double xh = (double)H.x0[j] + off;
-            const double d = fabs(xh - xp);
-            if (d <= w1 && y_compatible(c, H, j, y)) {
-                if (closer(H, d, j, d0, r.j0)) {
-                    d1 = d0; r.j1 = r.j0; r.x1 = r.x0;
-                    d0 = d; r.j0 = j; r.x0 = xh;
-                } else if (closer(H, d, j, d1, r.j1)) {
-                    d1 = d; r.j1 = j; r.x1 = xh;
+            const double d = fabs(((double)H.x0[j] + off) - xp);
+            const bool pass = (d <= w1) & y_compatible(c, H, j, y);
+            if (pass) {
+                if (closer(H, d, j, d0, j0)) {
+                    d1 = d0; j1 = j0;
+                    d0 = d; j0 = j;
+                } else if (closer(H, d, j, d1, j1)) {
+                    d1 = d; j1 = j;
                 }
-                ++n;
             }
         }
     }
-    r.n = min(n, keepn);
-    if (r.n < 2) r.j1 = -1;
-    if (r.n < 1) r.j0 = -1;
-    return r;
+    return make_int2(j0, j1);
 }
 
-// Best candidate of one first hit (S4 + S5 and the part of S6 that stays inside the first hit).
-struct FirstBest {
-    double score, a, b, chi2;   // score = kNoScore: no candidate
-    int nh, j0, j1, j2, j3;     // chosen hits (positions in the event's sorted slice), -1 = layer missing
+// The max_first closest of the more than max_first hits in the first window, by (distance, id), for a window
+// that lies in one sector [A, B) of the x0-sorted slice: walk outwards from the window centre.  Returns false (nothing
+// valid written) if it meets equal x0 on the left side, where the walk order is not the id order.
+__device__ bool select_first_walk(const DevConst &c, const EventHits &H, int A, int B, double off3, double xc, double w0,
+                                  double y, int max_first, int *dst)
+{
+    int lo = A, hi = B;   // first j in [A, B) with x0[j] + off3 >= xc
+    while (lo < hi) {
+        const int mid = (lo + hi) >> 1;
+        if ((double)H.x0[mid] + off3 >= xc) hi = mid; else lo = mid + 1;
+    }
+    int l = lo - 1, r = lo;
+    double dl = 1e300, dr = 1e300;
+    auto settle_left = [&]() {
+        for (; l >= A; --l) {
+            dl = fabs(((double)H.x0[l] + off3) - xc);
+            if (dl > w0) { l = A - 1; break; }
+            if (y_compatible(c, H, l, y)) break;
+        }
+    };
+    auto settle_right = [&]() {
+        for (; r < B; ++r) {
+            dr = fabs(((double)H.x0[r] + off3) - xc);
+            if (dr > w0) { r = B; break; }
+            if (y_compatible(c, H, r, y)) break;
+        }
+    };
+    settle_left();
+    settle_right();
+    for (int k = 0; k < max_first; ++k) {
+        const bool has_l = l >= A, has_r = r < B;
+        if (!has_l && !has_r) return false;   // fewer hits than the caller counted: cannot happen
+        bool take_left;
+        if (!has_r) take_left = true;
+        else if (!has_l) take_left = false;
+        else take_left = closer(H, dl, l, dr, r);
+        if (take_left) {
+            if (l - 1 >= A && H.x0[l - 1] == H.x0[l]) return false;
+            dst[k] = l;
+            --l;
+            settle_left();
+        } else {
+            dst[k] = r;
+            ++r;
+            settle_right();
+        }
+    }
+    return true;
+}
+
+// A candidate: fit result and chosen hits (positions in the event's sorted slice, -1 = layer missing)
+struct Candidate {
+    double score, a, b, chi2;   // score = kNoScore: none
+    int nh, j0, j1, j2, j3;
 };
 
 // A-9 order of two candidates with the same score: more hits, then smaller (id3, id0, id1, id2); missing = INT32_MAX
-__device__ __forceinline__ bool tie_better(const EventHits &H, const FirstBest &p, const FirstBest &q)
+__device__ __noinline__ bool tie_better(const EventHits &H, const Candidate &p, const Candidate &q)
 {
     if (p.nh != q.nh) return p.nh > q.nh;
     const int pj[4] = {p.j3, p.j0, p.j1, p.j2}, qj[4] = {q.j3, q.j0, q.j1, q.j2};
@@ -227,37 +267,34 @@ __device__ __forceinline__ bool tie_better(const EventHits &H, const FirstBest &
     return false;
 }
 
-__device__ FirstBest eval_first_hit(const DevConst &c, const EventHits &H, const int *tab, const S2 &s2, int j3)
+// S5 for the <= 4 combinations of one first hit j3 with the refined-window hits n0, n1, n2 (S4); S6: `best` is
+// replaced by every combination that beats it.
+__device__ __forceinline__ void fit_first_hit(const DevConst &c, const EventHits &H, const S2 &s2, int j3, int2 n0,
+                                              int2 n1, int2 n2, Candidate &best)
 {
-    FirstBest best;
-    best.score = kNoScore; best.a = 0.0; best.b = 0.0; best.chi2 = 0.0;
-    best.nh = 0; best.j0 = -1; best.j1 = -1; best.j2 = -1; best.j3 = j3;
-
-    // S4: trajectory through (first hit, magnet point), refined windows
+    const int nh = 1 + (n0.x >= 0) + (n1.x >= 0) + (n2.x >= 0);
+    if (nh < c.min_hits) return;
+    // weighted line through the hits and the magnet point (A-8)
     const double x3 = (double)H.x0[j3] + c.dxdy[3] * s2.y3;
-    const double z3 = (double)H.z[j3];
-    const double txc = (x3 - s2.xm) / (z3 - s2.zm);
-    const Near n0 = search_layer(c, H, tab, 0, s2.xm + txc * (c.z_layer[0] - s2.zm), s2.y0, s2.w1, 1);
-    const Near n1 = search_layer(c, H, tab, 1, s2.xm + txc * (c.z_layer[1] - s2.zm), s2.y1, s2.w1, 2);
-    const Near n2 = search_layer(c, H, tab, 2, s2.xm + txc * (c.z_layer[2] - s2.zm), s2.y2, s2.w1, 2);
-    const int nh = 1 + (n0.n > 0) + (n1.n > 0) + (n2.n > 0);
-    if (nh < c.min_hits) return best;
-
-    // S5: weighted line through the hits and the magnet point (A-8); terms shared by all combinations first
-    const double w3 = (double)H.w[j3];
-    const double pz3 = z3 - c.z_ref, pzm = s2.zm - c.z_ref;
+    const double pz3 = (double)H.z[j3] - c.z_ref, w3 = (double)H.w[j3], pzm = s2.zm - c.z_ref;
     double pz0 = 0.0, pw0 = 0.0, px0 = 0.0;
-    if (n0.n > 0) { pz0 = (double)H.z[n0.j0] - c.z_ref; pw0 = (double)H.w[n0.j0]; px0 = n0.x0; }
+    if (n0.x >= 0) {
+        pz0 = (double)H.z[n0.x] - c.z_ref; pw0 = (double)H.w[n0.x]; px0 = (double)H.x0[n0.x] + c.dxdy[0] * s2.y0;
+    }
     const double ndf = (double)(nh - 1);
-    const int m1 = max(n1.n, 1), m2 = max(n2.n, 1);
+    const int m1 = n1.y >= 0 ? 2 : 1, m2 = n2.y >= 0 ? 2 : 1;
     for (int i1 = 0; i1 < m1; ++i1) {
-        const int j1 = n1.n > 0 ? (i1 ? n1.j1 : n1.j0) : -1;
+        const int j1 = i1 ? n1.y : n1.x;
         double pz1 = 0.0, pw1 = 0.0, px1 = 0.0;
-        if (j1 >= 0) { pz1 = (double)H.z[j1] - c.z_ref; pw1 = (double)H.w[j1]; px1 = i1 ? n1.x1 : n1.x0; }
+        if (j1 >= 0) {
+            pz1 = (double)H.z[j1] - c.z_ref; pw1 = (double)H.w[j1]; px1 = (double)H.x0[j1] + c.dxdy[1] * s2.y1;
+        }
         for (int i2 = 0; i2 < m2; ++i2) {
-            const int j2 = n2.n > 0 ? (i2 ? n2.j1 : n2.j0) : -1;
+            const int j2 = i2 ? n2.y : n2.x;
             double pz2 = 0.0, pw2 = 0.0, px2 = 0.0;
-            if (j2 >= 0) { pz2 = (double)H.z[j2] - c.z_ref; pw2 = (double)H.w[j2]; px2 = i2 ? n2.x1 : n2.x0; }
+            if (j2 >= 0) {
+                pz2 = (double)H.z[j2] - c.z_ref; pw2 = (double)H.w[j2]; px2 = (double)H.x0[j2] + c.dxdy[2] * s2.y2;
+            }
             const double pz[5] = {pz0, pz1, pz2, pz3, pzm};
             const double px[5] = {px0, px1, px2, x3, s2.xm};
             const double pw[5] = {pw0, pw1, pw2, w3, c.w_mag};
@@ -280,16 +317,13 @@ __device__ FirstBest eval_first_hit(const DevConst &c, const EventHits &H, const
                 chi2 += pw[k] * r * r;
             }
             if (!(chi2 / ndf <= c.chi2ndf_max)) continue;
-            FirstBest cand;
+            Candidate cand;
             cand.score = chi2 + c.miss_penalty * (double)(4 - nh);
             cand.a = fa; cand.b = fb; cand.chi2 = chi2;
-            cand.nh = nh; cand.j0 = n0.j0; cand.j1 = j1; cand.j2 = j2; cand.j3 = j3;
-            if (best.score == kNoScore || cand.score < best.score ||
-                (cand.score == best.score && tie_better(H, cand, best)))
-                best = cand;
+            cand.nh = nh; cand.j0 = n0.x; cand.j1 = j1; cand.j2 = j2; cand.j3 = j3;
+            if (cand.score < best.score || (cand.score == best.score && tie_better(H, cand, best))) best = cand;
         }
     }
-    return best;
 }
 
 __device__ __forceinline__ void write_not_found(const ds_tracks &out, int64_t s)
@@ -332,28 +366,62 @@ __device__ __forceinline__ void track_event(const DevConst &c, TrackShared &sh, 
     const int tid = threadIdx.x;
     const int max_first = c.max_first;
     const int *tab = sh.tab;
+    int *my_slot = sh.slot + tid * kMaxFirst;
     int s_base = s_begin;
     while (s_base < s_end) {
         // ---- phase A: thread per seed -- S2, S3 ------------------------------------------------------------------------
         const int s = s_base + tid;
         const bool act = s < s_end;
-        S2 s2;
-        int s_lo = 0, s_hi = -1, nF = 0;
-        double off3 = 0.0, lo3 = 0.0, hi3 = 0.0;
+        int nF = 0;
         if (act) {
             const float fx = seeds.x[s], fy = seeds.y[s], ftx = seeds.tx[s], fty = seeds.ty[s], fq = seeds.qop[s];
             sh.sx[tid] = fx; sh.sy[tid] = fy; sh.stx[tid] = ftx; sh.sty[tid] = fty; sh.sqop[tid] = fq;
-            s2 = extrapolate_seed(c, fx, fy, ftx, fty, fq);
+            const S2 s2 = extrapolate_seed(c, fx, fy, ftx, fty, fq);
+            int s_lo, s_hi;
             sector_range(c, s2.y3, s_lo, s_hi);
-            off3 = c.dxdy[3] * s2.y3;
-            lo3 = s2.xc3 - off3 - s2.w0;
-            hi3 = s2.xc3 - off3 + s2.w0;
+            const double off3 = c.dxdy[3] * s2.y3;
+            const double lo3 = s2.xc3 - off3 - s2.w0, hi3 = s2.xc3 - off3 + s2.w0;
             for (int sec = s_lo; sec <= s_hi; ++sec) {
                 int a, b;
                 slice_range(c, tab, 3, sec, lo3, hi3, a, b);
                 for (int j = a; j < b; ++j) {
-                    const double xh = (double)H.x0[j] + off3;
-                    nF += (fabs(xh - s2.xc3) <= s2.w0 && y_compatible(c, H, j, s2.y3)) ? 1 : 0;
+                    const double d = fabs(((double)H.x0[j] + off3) - s2.xc3);
+                    if ((d <= s2.w0) & y_compatible(c, H, j, s2.y3)) {
+                        if (nF < max_first) my_slot[nF] = j;
+                        ++nF;
+                    }
+                }
+            }
+            if (nF > max_first) {
+                // more hits in the window than are tried: the max_first closest by (distance, id) (P:105)
+                bool done = false;
+                if (s_lo == s_hi) {
+                    const int base = (3 * c.n_sectors + s_lo) * kXBins;
+                    done = select_first_walk(c, H, tab[base], tab[base + kXBins], off3, s2.xc3, s2.w0, s2.y3, max_first,
+                                             my_slot);
+                }
+                if (!done) {
+                    double last_d = -1.0;
+                    int last_j = -1;
+                    for (int k = 0; k < max_first; ++k) {
+                        double bd = 1e300;
+                        int bj = -1;
+                        for (int sec = s_lo; sec <= s_hi; ++sec) {
+                            int a, b;
+                            slice_range(c, tab, 3, sec, lo3, hi3, a, b);
+                            for (int j = a; j < b; ++j) {
+                                const double d = fabs(((double)H.x0[j] + off3) - s2.xc3);
+                                if ((d <= s2.w0) & y_compatible(c, H, j, s2.y3)) {
+                                    // strictly after the previous pick, and before the best so far
+                                    const bool after = last_j < 0 || (j != last_j && closer(H, last_d, last_j, d, j));
+                                    if (after && closer(H, d, j, bd, bj)) { bd = d; bj = j; }
+                                }
+                            }
+                        }
+                        my_slot[k] = bj;
+                        last_d = bd;
+                        last_j = bj;
+                    }
                 }
             }
         }
@@ -362,97 +430,58 @@ __device__ __forceinline__ void track_event(const DevConst &c, TrackShared &sh, 
         // the seeds taken this round are the longest prefix whose first hits fit the list
         const bool take = act && incl <= kFirstCap;
         const int n_take = __syncthreads_count(take);
-        if (take && tid == n_take - 1) sh.n_first = incl;
         if (take) {
-            int pos = incl - nFc;
+            const int pos = incl - nFc;
+            if (tid == n_take - 1) sh.n_first = incl;
             sh.foff[tid] = pos;
-            sh.fn[tid] = (unsigned char)nFc;
-            if (nF <= max_first) {
-                for (int sec = s_lo; sec <= s_hi; ++sec) {
-                    int a, b;
-                    slice_range(c, tab, 3, sec, lo3, hi3, a, b);
-                    for (int j = a; j < b; ++j) {
-                        const double xh = (double)H.x0[j] + off3;
-                        if (fabs(xh - s2.xc3) <= s2.w0 && y_compatible(c, H, j, s2.y3)) {
-                            sh.fj[pos] = j;
-                            sh.fs[pos] = (unsigned short)tid;
-                            ++pos;
-                        }
-                    }
-                }
-            } else {
-                // more hits in the window than are tried: the max_first closest by (distance, id) (P:105)
-                double last_d = -1.0;
-                int last_j = -1;
-                for (int k = 0; k < max_first; ++k) {
-                    double bd = 1e300;
-                    int bj = -1;
-                    for (int sec = s_lo; sec <= s_hi; ++sec) {
-                        int a, b;
-                        slice_range(c, tab, 3, sec, lo3, hi3, a, b);
-                        for (int j = a; j < b; ++j) {
-                            const double xh = (double)H.x0[j] + off3;
-                            const double d = fabs(xh - s2.xc3);
-                            if (d <= s2.w0 && y_compatible(c, H, j, s2.y3)) {
-                                // strictly after the previous pick, and before the best so far
-                                const bool after = last_j < 0 || (j != last_j && closer(H, last_d, last_j, d, j));
-                                if (after && closer(H, d, j, bd, bj)) { bd = d; bj = j; }
-                            }
-                        }
-                    }
-                    sh.fj[pos] = bj;
-                    sh.fs[pos] = (unsigned short)tid;
-                    ++pos;
-                    last_d = bd;
-                    last_j = bj;
-                }
-            }
+            for (int k = 0; k < nFc; ++k) sh.fs[pos + k] = (unsigned short)(tid * kMaxFirst + k);
         }
         __syncthreads();
-        // ---- phase B: thread per first hit -- S4, S5 ---------------------------------------------------------------
-        const int n_first = sh.n_first;
-        for (int f = tid; f < n_first; f += kTrackThreads) {
-            const int o = sh.fs[f];
+        // ---- phase B: thread per (first hit, layer) -- S4 ----------------------------------------------------------------
+        const int n_task = 3 * sh.n_first;
+        for (int t = tid; t < n_task; t += kTrackThreads) {
+            const int f = t / 3, l = t - 3 * f;
+            const int sl = sh.fs[f], o = sl / kMaxFirst;
+            const int j3 = sh.slot[sl];
             const S2 t2 = extrapolate_seed(c, sh.sx[o], sh.sy[o], sh.stx[o], sh.sty[o], sh.sqop[o]);
-            sh.fscore[f] = eval_first_hit(c, H, tab, t2, sh.fj[f]).score;
+            // trajectory through (first hit, magnet point), refined window in layer l
+            const double x3 = (double)H.x0[j3] + c.dxdy[3] * t2.y3;
+            const double txc = (x3 - t2.xm) / ((double)H.z[j3] - t2.zm);
+            const double xp = t2.xm + txc * (c.z_layer[l] - t2.zm);
+            const double y = l == 0 ? t2.y0 : (l == 1 ? t2.y1 : t2.y2);
+            int2 r = search_layer(c, H, tab, l, xp, y, t2.w1);
+            if (l == 0) r.y = -1;   // UTaX keeps the closest hit only
+            sh.near[t] = r;
         }
         __syncthreads();
-        // ---- phase C: thread per seed -- S6 and the track record ------------------------------------------------------
+        // ---- phase C: thread per seed -- S5, S6 and the track record ----------------------------------------------------
         if (take) {
+            Candidate best;
+            best.score = kNoScore; best.a = 0.0; best.b = 0.0; best.chi2 = 0.0;
+            best.nh = 0; best.j0 = -1; best.j1 = -1; best.j2 = -1; best.j3 = -1;
+            const S2 s2 = extrapolate_seed(c, sh.sx[tid], sh.sy[tid], sh.stx[tid], sh.sty[tid], sh.sqop[tid]);
             const int f0 = sh.foff[tid];
-            int fbest = -1;
-            double sbest = kNoScore;
-            bool tied = false;
             for (int k = 0; k < nFc; ++k) {
-                const double sc = sh.fscore[f0 + k];
-                if (sc < sbest) { sbest = sc; fbest = f0 + k; tied = false; }
-                else if (sc == sbest && sc != kNoScore) tied = true;
+                const int t = 3 * (f0 + k);
+                fit_first_hit(c, H, s2, my_slot[k], sh.near[t], sh.near[t + 1], sh.near[t + 2], best);
             }
-            if (fbest < 0) {
+            if (best.score == kNoScore) {
                 write_not_found(out, s);
             } else {
-                FirstBest w = eval_first_hit(c, H, tab, s2, sh.fj[fbest]);
-                if (tied) {   // equal scores in different first hits (duplicate hits): more hits, then ids (A-9)
-                    for (int k = 0; k < nFc; ++k) {
-                        if (f0 + k == fbest || sh.fscore[f0 + k] != sbest) continue;
-                        const FirstBest q = eval_first_hit(c, H, tab, s2, sh.fj[f0 + k]);
-                        if (tie_better(H, q, w)) w = q;
-                    }
-                }
                 const double ys = (double)sh.sy[tid], txs = (double)sh.stx[tid], tys = (double)sh.sty[tid];
-                out.x[s] = (float)w.a;
+                out.x[s] = (float)best.a;
                 out.y[s] = (float)(ys + tys * (c.z_ref - c.z_seed));
-                out.tx[s] = (float)w.b;
+                out.tx[s] = (float)best.b;
                 out.ty[s] = (float)tys;
-                out.qop[s] = (float)((txs - w.b) / c.kick);
-                out.chi2[s] = (float)w.chi2;
-                out.nhits[s] = w.nh;
+                out.qop[s] = (float)((txs - best.b) / c.kick);
+                out.chi2[s] = (float)best.chi2;
+                out.nhits[s] = best.nh;
                 out.found[s] = 1;
                 int4 hv;
-                hv.x = w.j0 >= 0 ? H.perm[w.j0] : -1;
-                hv.y = w.j1 >= 0 ? H.perm[w.j1] : -1;
-                hv.z = w.j2 >= 0 ? H.perm[w.j2] : -1;
-                hv.w = H.perm[w.j3];
+                hv.x = best.j0 >= 0 ? H.perm[best.j0] : -1;
+                hv.y = best.j1 >= 0 ? H.perm[best.j1] : -1;
+                hv.z = best.j2 >= 0 ? H.perm[best.j2] : -1;
+                hv.w = H.perm[best.j3];
                 reinterpret_cast<int4 *>(out.hit)[s] = hv;
             }
         }
