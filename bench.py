@@ -25,6 +25,8 @@ import sys
 import threading
 import time
 
+import numpy as np
+
 ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
@@ -225,7 +227,10 @@ def main():
 
     # ---- pinned host copies (e2e inputs) and device-resident copies (kernel-path inputs) --------------------------------
     mlp_w = gen.mlp_weights(0)
-    ds = pk.Downstream(C.GEOMETRY, mlp_w, C.PARAMS, device=local)
+    # max_event_hits_hint = the largest event of the workload (sizes the kernels' per-event staging buffers)
+    max_event_hits = max(int(np.diff(d["hit_offsets"]).max()) for d in subs)
+    params = dict(C.PARAMS, max_event_hits_hint=max_event_hits)
+    ds = pk.Downstream(C.GEOMETRY, mlp_w, params, device=local)
     host, devd = [], []
     for d in subs:
         hp = dict(hits={k: torch.from_numpy(v).pin_memory() for k, v in d["hits"].items()},
@@ -326,7 +331,7 @@ def main():
     # ---- end to end: pinned host buffers in, pinned host buffers out, through ds_process_host ----------------------------
     e2e = None
     if not args.no_e2e:
-        handles = [pk.Downstream(C.GEOMETRY, mlp_w, C.PARAMS, device=local) for _ in range(n_streams)]
+        handles = [pk.Downstream(C.GEOMETRY, mlp_w, params, device=local) for _ in range(n_streams)]
         vcap = 1 << 18
         out_t = [pk.host_tracks(max(n_seeds), pinned=True) for _ in range(n_streams)]
         out_v = [pk.host_vertices(vcap, args.subbatch, pinned=True) for _ in range(n_streams)]

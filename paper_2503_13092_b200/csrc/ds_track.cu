@@ -129,22 +129,36 @@ __device__ __forceinline__ void mbar_wait(unsigned long long *bar, uint32_t pari
 }
 
 
-constexpr int kFirstCap = 512;   // first hits handled per round (>= DS_MAX_FIRST_HITS)
+constexpr int kFirstCap = 384;   // first hits handled per round (>= DS_MAX_FIRST_HITS)
+constexpr int kFitCap = 256;     // fits handled by the fit phase per round; the rest are fitted by the seed's thread
 constexpr double kNoScore = 1e300;
+constexpr unsigned short kFitNone = 0xffffu, kFitInline = 0xfffeu;
 
-// Block-shared state of k_track (carved from dynamic shared memory, followed by the staged hit arrays).
+struct FitRes {
+    double score, a, b, chi2;   // score = kNoScore: the combination fails the chi2/ndf cut
+};
+
+// Block-shared state of k_track (carved from dynamic shared memory, followed by the staged hit arrays).  Idx is the
+// type hit positions inside the event are stored in: uint16_t when the event is staged (it then has < 65535 hits),
+// int otherwise.  (Idx)-1 = none.
+template <typename Idx>
 struct TrackShared {
     unsigned long long bar;
-    int2 near[3 * kFirstCap];             // phase B: closest / second closest hit of (first hit, layer), -1 = none
+    FitRes res[kFitCap];                  // fit phase: result of fit task i
+    float2 zw3[kFirstCap];                // (z, w) of the first hit
     int tab[kMaxBins + 1];                // the event's bin table
-    int slot[kTrackThreads * kMaxFirst];  // phase A: the seed's first hits (positions in the event's sorted slice)
     float sx[kTrackThreads], sy[kTrackThreads], stx[kTrackThreads], sty[kTrackThreads], sqop[kTrackThreads];
-    int foff[kTrackThreads];              // where the seed's first hits start in the round's list
     int warp_sums[kTrackWarps + 1];
     int n_first;                          // entries of the first-hit list this round
+    int n_fit;                            // fit tasks appended this round (may exceed kFitCap)
+    Idx slot[kTrackThreads * kMaxFirst];  // phase A: the seed's first hits (positions in the event's sorted slice)
+    Idx near[3 * kFirstCap][2];           // phase B: closest / second closest hit of (first hit, layer)
+    unsigned short foff[kTrackThreads];   // where the seed's first hits start in the round's list
     unsigned short fs[kFirstCap];         // first-hit list: index into slot[]
-    unsigned char fn[kTrackThreads];      // number of first hits of the seed
+    unsigned short ffit[kFirstCap];       // first fit task of the first hit, kFitNone or kFitInline
+    unsigned short task[kFitCap];         // fit task: first hit | i1 << 9 | i2 << 10
 };
+static_assert(kFirstCap <= 512, "fit task packs the first hit in 9 bits");
 
 // The event's hits as the searches see them: x0 / ymin / ymax from the staging buffer (or global for an oversize
 // event), the rest always from global memory.  Indices are relative to the event's sorted slice.
@@ -153,6 +167,9 @@ struct EventHits {
     const float *z, *w;              // global
     const int32_t *id, *perm;        // global
 };
+
+template <typename Idx>
+__device__ __forceinline__ int idx_get(Idx v) { return v == (Idx)-1 ? -1 : (int)v; }
 
 // y-compatibility of hit j (O-S3: ymin - y_tol <= y <= ymax + y_tol); no short circuit: both loads are always issued
 __device__ __forceinline__ bool y_compatible(const DevConst &c, const EventHits &H, int j, double y)
@@ -199,50 +216,57 @@ __device__ __forceinline__ int2 search_layer(const DevConst &c, const EventHits 
 }
 
 // The max_first closest of the more than max_first hits in the first window, by (distance, id), for a window
-// that lies in one sector [A, B) of the x0-sorted slice: walk outwards from the window centre.  Returns false (nothing
-// valid written) if it meets equal x0 on the left side, where the walk order is not the id order.
-__device__ bool select_first_walk(const DevConst &c, const EventHits &H, int A, int B, double off3, double xc, double w0,
-                                  double y, int max_first, int *dst)
+// that touches one or two sectors: every sector is an x0-sorted range, so the closest hits are found by walking
+// outwards from the window centre, one left and one right head per sector, always taking the closest head.  Returns
+// false (dst not valid) when it meets equal x0 on a left side, where the walk order is not the id order.
+template <typename Idx>
+__device__ __noinline__ bool select_first_walk(const DevConst &c, const EventHits &H, const int *tab, int s_lo, int s_hi,
+                                               double off3, double xc, double w0, double y, int max_first, Idx *dst)
 {
-    int lo = A, hi = B;   // first j in [A, B) with x0[j] + off3 >= xc
-    while (lo < hi) {
-        const int mid = (lo + hi) >> 1;
-        if ((double)H.x0[mid] + off3 >= xc) hi = mid; else lo = mid + 1;
+    int hj[4], hend[4];
+    double hd[4];
+#pragma unroll
+    for (int k = 0; k < 2; ++k) {
+        int A = 0, B = 0;
+        if (s_lo + k <= s_hi) {
+            const int base = (3 * c.n_sectors + s_lo + k) * kXBins;
+            A = tab[base];
+            B = tab[base + kXBins];
+        }
+        int lo = A, hi = B;   // first j in [A, B) with x0[j] + off3 >= xc
+        while (lo < hi) {
+            const int mid = (lo + hi) >> 1;
+            if ((double)H.x0[mid] + off3 >= xc) hi = mid; else lo = mid + 1;
+        }
+        hj[2 * k] = lo - 1; hend[2 * k] = A - 1;
+        hj[2 * k + 1] = lo; hend[2 * k + 1] = B;
     }
-    int l = lo - 1, r = lo;
-    double dl = 1e300, dr = 1e300;
-    auto settle_left = [&]() {
-        for (; l >= A; --l) {
-            dl = fabs(((double)H.x0[l] + off3) - xc);
-            if (dl > w0) { l = A - 1; break; }
-            if (y_compatible(c, H, l, y)) break;
+    // move head h to the next y-compatible hit inside the window (or to its end)
+    auto settle = [&](int &j, int end, int step, double &d) {
+        for (; j != end; j += step) {
+            d = fabs(((double)H.x0[j] + off3) - xc);
+            if (d > w0) { j = end; break; }
+            if (y_compatible(c, H, j, y)) break;
         }
     };
-    auto settle_right = [&]() {
-        for (; r < B; ++r) {
-            dr = fabs(((double)H.x0[r] + off3) - xc);
-            if (dr > w0) { r = B; break; }
-            if (y_compatible(c, H, r, y)) break;
-        }
-    };
-    settle_left();
-    settle_right();
+#pragma unroll
+    for (int h = 0; h < 4; ++h) { hd[h] = 1e300; settle(hj[h], hend[h], (h & 1) ? 1 : -1, hd[h]); }
     for (int k = 0; k < max_first; ++k) {
-        const bool has_l = l >= A, has_r = r < B;
-        if (!has_l && !has_r) return false;   // fewer hits than the caller counted: cannot happen
-        bool take_left;
-        if (!has_r) take_left = true;
-        else if (!has_l) take_left = false;
-        else take_left = closer(H, dl, l, dr, r);
-        if (take_left) {
-            if (l - 1 >= A && H.x0[l - 1] == H.x0[l]) return false;
-            dst[k] = l;
-            --l;
-            settle_left();
-        } else {
-            dst[k] = r;
-            ++r;
-            settle_right();
+        int pick = -1, pj = -1;
+        double pd = 1e300;
+#pragma unroll
+        for (int h = 0; h < 4; ++h) {
+            if (hj[h] != hend[h] && (pick < 0 || closer(H, hd[h], hj[h], pd, pj))) { pick = h; pj = hj[h]; pd = hd[h]; }
+        }
+        if (pick < 0) return false;   // fewer hits than the caller counted: cannot happen
+        dst[k] = (Idx)pj;
+#pragma unroll
+        for (int h = 0; h < 4; ++h) {
+            if (h == pick) {
+                if (!(h & 1) && pj - 1 != hend[h] && H.x0[pj - 1] == H.x0[pj]) return false;
+                hj[h] += (h & 1) ? 1 : -1;
+                settle(hj[h], hend[h], (h & 1) ? 1 : -1, hd[h]);
+            }
         }
     }
     return true;
@@ -267,63 +291,45 @@ __device__ __noinline__ bool tie_better(const EventHits &H, const Candidate &p, 
     return false;
 }
 
-// S5 for the <= 4 combinations of one first hit j3 with the refined-window hits n0, n1, n2 (S4); S6: `best` is
-// replaced by every combination that beats it.
-__device__ __forceinline__ void fit_first_hit(const DevConst &c, const EventHits &H, const S2 &s2, int j3, int2 n0,
-                                              int2 n1, int2 n2, Candidate &best)
+// S5: weighted straight line x(z - z_ref) through the first hit (z3, w3 given), the refined-window hits j0, j1, j2
+// (-1 = missing) and the magnet point as pseudo-measurement (A-8); chi2; chi2/ndf cut and score (A-9)
+__device__ __forceinline__ FitRes fit_combo(const DevConst &c, const EventHits &H, const S2 &s2, int j0, int j1, int j2,
+                                            int j3, double z3, double w3)
 {
-    const int nh = 1 + (n0.x >= 0) + (n1.x >= 0) + (n2.x >= 0);
-    if (nh < c.min_hits) return;
-    // weighted line through the hits and the magnet point (A-8)
-    const double x3 = (double)H.x0[j3] + c.dxdy[3] * s2.y3;
-    const double pz3 = (double)H.z[j3] - c.z_ref, w3 = (double)H.w[j3], pzm = s2.zm - c.z_ref;
-    double pz0 = 0.0, pw0 = 0.0, px0 = 0.0;
-    if (n0.x >= 0) {
-        pz0 = (double)H.z[n0.x] - c.z_ref; pw0 = (double)H.w[n0.x]; px0 = (double)H.x0[n0.x] + c.dxdy[0] * s2.y0;
+    // all loads first (z, w come from global memory)
+    const int k0 = max(j0, 0), k1 = max(j1, 0), k2 = max(j2, 0);
+    const float fz0 = H.z[k0], fw0 = H.w[k0], fz1 = H.z[k1], fw1 = H.w[k1], fz2 = H.z[k2], fw2 = H.w[k2];
+    const float fx0 = H.x0[k0], fx1 = H.x0[k1], fx2 = H.x0[k2], fx3 = H.x0[j3];
+    const bool u0 = j0 >= 0, u1 = j1 >= 0, u2 = j2 >= 0;
+    const int nh = 1 + u0 + u1 + u2;
+    const double pz[5] = {u0 ? (double)fz0 - c.z_ref : 0.0, u1 ? (double)fz1 - c.z_ref : 0.0,
+                          u2 ? (double)fz2 - c.z_ref : 0.0, z3 - c.z_ref, s2.zm - c.z_ref};
+    const double px[5] = {u0 ? (double)fx0 + c.dxdy[0] * s2.y0 : 0.0, u1 ? (double)fx1 + c.dxdy[1] * s2.y1 : 0.0,
+                          u2 ? (double)fx2 + c.dxdy[2] * s2.y2 : 0.0, (double)fx3 + c.dxdy[3] * s2.y3, s2.xm};
+    const double pw[5] = {u0 ? (double)fw0 : 0.0, u1 ? (double)fw1 : 0.0, u2 ? (double)fw2 : 0.0, w3, c.w_mag};
+    double S = 0, Sz = 0, Szz = 0, Sx = 0, Sxz = 0;
+#pragma unroll
+    for (int k = 0; k < 5; ++k) {
+        S += pw[k];
+        Sz += pw[k] * pz[k];
+        Szz += pw[k] * pz[k] * pz[k];
+        Sx += pw[k] * px[k];
+        Sxz += pw[k] * px[k] * pz[k];
     }
+    const double D = S * Szz - Sz * Sz;
+    FitRes r;
+    r.b = (S * Sxz - Sz * Sx) / D;
+    r.a = (Szz * Sx - Sz * Sxz) / D;
+    double chi2 = 0.0;
+#pragma unroll
+    for (int k = 0; k < 5; ++k) {
+        const double e = px[k] - r.a - r.b * pz[k];
+        chi2 += pw[k] * e * e;
+    }
+    r.chi2 = chi2;
     const double ndf = (double)(nh - 1);
-    const int m1 = n1.y >= 0 ? 2 : 1, m2 = n2.y >= 0 ? 2 : 1;
-    for (int i1 = 0; i1 < m1; ++i1) {
-        const int j1 = i1 ? n1.y : n1.x;
-        double pz1 = 0.0, pw1 = 0.0, px1 = 0.0;
-        if (j1 >= 0) {
-            pz1 = (double)H.z[j1] - c.z_ref; pw1 = (double)H.w[j1]; px1 = (double)H.x0[j1] + c.dxdy[1] * s2.y1;
-        }
-        for (int i2 = 0; i2 < m2; ++i2) {
-            const int j2 = i2 ? n2.y : n2.x;
-            double pz2 = 0.0, pw2 = 0.0, px2 = 0.0;
-            if (j2 >= 0) {
-                pz2 = (double)H.z[j2] - c.z_ref; pw2 = (double)H.w[j2]; px2 = (double)H.x0[j2] + c.dxdy[2] * s2.y2;
-            }
-            const double pz[5] = {pz0, pz1, pz2, pz3, pzm};
-            const double px[5] = {px0, px1, px2, x3, s2.xm};
-            const double pw[5] = {pw0, pw1, pw2, w3, c.w_mag};
-            double S = 0, Sz = 0, Szz = 0, Sx = 0, Sxz = 0;
-#pragma unroll
-            for (int k = 0; k < 5; ++k) {
-                S += pw[k];
-                Sz += pw[k] * pz[k];
-                Szz += pw[k] * pz[k] * pz[k];
-                Sx += pw[k] * px[k];
-                Sxz += pw[k] * px[k] * pz[k];
-            }
-            const double D = S * Szz - Sz * Sz;
-            const double fb = (S * Sxz - Sz * Sx) / D;
-            const double fa = (Szz * Sx - Sz * Sxz) / D;
-            double chi2 = 0.0;
-#pragma unroll
-            for (int k = 0; k < 5; ++k) {
-                const double r = px[k] - fa - fb * pz[k];
-                chi2 += pw[k] * r * r;
-            }
-            if (!(chi2 / ndf <= c.chi2ndf_max)) continue;
-            Candidate cand;
-            cand.score = chi2 + c.miss_penalty * (double)(4 - nh);
-            cand.a = fa; cand.b = fb; cand.chi2 = chi2;
-            cand.nh = nh; cand.j0 = n0.x; cand.j1 = j1; cand.j2 = j2; cand.j3 = j3;
-            if (cand.score < best.score || (cand.score == best.score && tie_better(H, cand, best))) best = cand;
-        }
-    }
+    r.score = (chi2 / ndf <= c.chi2ndf_max) ? chi2 + c.miss_penalty * (double)(4 - nh) : kNoScore;
+    return r;
 }
 
 __device__ __forceinline__ void write_not_found(const ds_tracks &out, int64_t s)
@@ -360,19 +366,21 @@ __device__ __forceinline__ int block_inclusive_scan(int v, int *warp_sums)
 }
 
 // All seeds of one event.  Every thread of the block runs this with the same arguments.
-__device__ __forceinline__ void track_event(const DevConst &c, TrackShared &sh, const EventHits &H, const ds_seeds &seeds,
-                                            int s_begin, int s_end, const ds_tracks &out)
+template <typename Idx>
+__device__ __forceinline__ void track_event(const DevConst &c, TrackShared<Idx> &sh, const EventHits &H,
+                                            const ds_seeds &seeds, int s_begin, int s_end, const ds_tracks &out)
 {
-    const int tid = threadIdx.x;
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const int max_first = c.max_first;
     const int *tab = sh.tab;
-    int *my_slot = sh.slot + tid * kMaxFirst;
+    Idx *my_slot = sh.slot + tid * kMaxFirst;
     int s_base = s_begin;
     while (s_base < s_end) {
         // ---- phase A: thread per seed -- S2, S3 ------------------------------------------------------------------------
         const int s = s_base + tid;
         const bool act = s < s_end;
         int nF = 0;
+        if (tid == 0) sh.n_fit = 0;
         if (act) {
             const float fx = seeds.x[s], fy = seeds.y[s], ftx = seeds.tx[s], fty = seeds.ty[s], fq = seeds.qop[s];
             sh.sx[tid] = fx; sh.sy[tid] = fy; sh.stx[tid] = ftx; sh.sty[tid] = fty; sh.sqop[tid] = fq;
@@ -387,7 +395,7 @@ __device__ __forceinline__ void track_event(const DevConst &c, TrackShared &sh, 
                 for (int j = a; j < b; ++j) {
                     const double d = fabs(((double)H.x0[j] + off3) - s2.xc3);
                     if ((d <= s2.w0) & y_compatible(c, H, j, s2.y3)) {
-                        if (nF < max_first) my_slot[nF] = j;
+                        if (nF < max_first) my_slot[nF] = (Idx)j;
                         ++nF;
                     }
                 }
@@ -395,12 +403,9 @@ __device__ __forceinline__ void track_event(const DevConst &c, TrackShared &sh, 
             if (nF > max_first) {
                 // more hits in the window than are tried: the max_first closest by (distance, id)
                 bool done = false;
-                if (s_lo == s_hi) {
-                    const int base = (3 * c.n_sectors + s_lo) * kXBins;
-                    done = select_first_walk(c, H, tab[base], tab[base + kXBins], off3, s2.xc3, s2.w0, s2.y3, max_first,
-                                             my_slot);
-                }
-                if (!done) {
+                if (s_hi - s_lo <= 1)
+                    done = select_first_walk<Idx>(c, H, tab, s_lo, s_hi, off3, s2.xc3, s2.w0, s2.y3, max_first, my_slot);
+                if (!done) {   // general case: max_first selection passes over the window
                     double last_d = -1.0;
                     int last_j = -1;
                     for (int k = 0; k < max_first; ++k) {
@@ -418,7 +423,7 @@ __device__ __forceinline__ void track_event(const DevConst &c, TrackShared &sh, 
                                 }
                             }
                         }
-                        my_slot[k] = bj;
+                        my_slot[k] = (Idx)bj;
                         last_d = bd;
                         last_j = bj;
                     }
@@ -433,37 +438,99 @@ __device__ __forceinline__ void track_event(const DevConst &c, TrackShared &sh, 
         if (take) {
             const int pos = incl - nFc;
             if (tid == n_take - 1) sh.n_first = incl;
-            sh.foff[tid] = pos;
-            for (int k = 0; k < nFc; ++k) sh.fs[pos + k] = (unsigned short)(tid * kMaxFirst + k);
+            sh.foff[tid] = (unsigned short)pos;
+            for (int k = 0; k < nFc; ++k) {
+                const int j = (int)my_slot[k];
+                sh.fs[pos + k] = (unsigned short)(tid * kMaxFirst + k);
+                sh.zw3[pos + k] = make_float2(H.z[j], H.w[j]);
+            }
         }
         __syncthreads();
-        // ---- phase B: thread per (first hit, layer) -- S4 ----------------------------------------------------------------
-        const int n_task = 3 * sh.n_first;
-        for (int t = tid; t < n_task; t += kTrackThreads) {
-            const int f = t / 3, l = t - 3 * f;
+        // ---- phase B: three lanes per first hit, one per layer -- S4; lane 0 of the three queues the fits ----------------
+        const int n_first = sh.n_first;
+        for (int fb = 0; fb < n_first; fb += kTrackWarps * 10) {
+            const int g = lane / 3, l = lane - 3 * g;
+            const int f = fb + wid * 10 + g;
+            const bool on = lane < 30 && f < n_first;
+            int2 r = make_int2(-1, -1);
+            if (on) {
+                const int sl = sh.fs[f], o = sl / kMaxFirst;
+                const int j3 = (int)sh.slot[sl];
+                const S2 t2 = extrapolate_seed(c, sh.sx[o], sh.sy[o], sh.stx[o], sh.sty[o], sh.sqop[o]);
+                // trajectory through (first hit, magnet point), refined window in layer l
+                const double x3 = (double)H.x0[j3] + c.dxdy[3] * t2.y3;
+                const double txc = (x3 - t2.xm) / ((double)sh.zw3[f].x - t2.zm);
+                const double xp = t2.xm + txc * (c.z_layer[l] - t2.zm);
+                const double y = l == 0 ? t2.y0 : (l == 1 ? t2.y1 : t2.y2);
+                r = search_layer(c, H, tab, l, xp, y, t2.w1);
+                if (l == 0) r.y = -1;   // UTaX keeps the closest hit only
+                sh.near[3 * f + l][0] = (Idx)r.x;
+                sh.near[3 * f + l][1] = (Idx)r.y;
+            }
+            const int g3 = min(3 * g, 29);
+            const unsigned has1 = __ballot_sync(0xffffffffu, r.x >= 0), has2 = __ballot_sync(0xffffffffu, r.y >= 0);
+            if (on && l == 0) {
+                const int nh = 1 + ((has1 >> g3) & 1) + ((has1 >> (g3 + 1)) & 1) + ((has1 >> (g3 + 2)) & 1);
+                unsigned short ff = kFitNone;
+                if (nh >= c.min_hits) {
+                    const int m1 = 1 + ((has2 >> (g3 + 1)) & 1), m2 = 1 + ((has2 >> (g3 + 2)) & 1);
+                    const int base = atomicAdd(&sh.n_fit, m1 * m2);
+                    if (base + m1 * m2 <= kFitCap) {
+                        ff = (unsigned short)base;
+                        for (int i1 = 0; i1 < m1; ++i1)
+                            for (int i2 = 0; i2 < m2; ++i2)
+                                sh.task[base + i1 * m2 + i2] = (unsigned short)(f | (i1 << 9) | (i2 << 10));
+                    } else {
+                        ff = kFitInline;
+                    }
+                }
+                sh.ffit[f] = ff;
+            }
+        }
+        __syncthreads();
+        // ---- fit phase: thread per queued combination -- S5 ------------------------------------------------------------
+        const int n_fit = min(sh.n_fit, kFitCap);
+        for (int t = tid; t < n_fit; t += kTrackThreads) {
+            const int tk = sh.task[t], f = tk & 511, i1 = (tk >> 9) & 1, i2 = (tk >> 10) & 1;
             const int sl = sh.fs[f], o = sl / kMaxFirst;
-            const int j3 = sh.slot[sl];
             const S2 t2 = extrapolate_seed(c, sh.sx[o], sh.sy[o], sh.stx[o], sh.sty[o], sh.sqop[o]);
-            // trajectory through (first hit, magnet point), refined window in layer l
-            const double x3 = (double)H.x0[j3] + c.dxdy[3] * t2.y3;
-            const double txc = (x3 - t2.xm) / ((double)H.z[j3] - t2.zm);
-            const double xp = t2.xm + txc * (c.z_layer[l] - t2.zm);
-            const double y = l == 0 ? t2.y0 : (l == 1 ? t2.y1 : t2.y2);
-            int2 r = search_layer(c, H, tab, l, xp, y, t2.w1);
-            if (l == 0) r.y = -1;   // UTaX keeps the closest hit only
-            sh.near[t] = r;
+            const float2 zw = sh.zw3[f];
+            sh.res[t] = fit_combo(c, H, t2, idx_get(sh.near[3 * f][0]), idx_get(sh.near[3 * f + 1][i1]),
+                                  idx_get(sh.near[3 * f + 2][i2]), (int)sh.slot[sl], (double)zw.x, (double)zw.y);
         }
         __syncthreads();
-        // ---- phase C: thread per seed -- S5, S6 and the track record ----------------------------------------------------
+        // ---- phase C: thread per seed -- S6 and the track record ---------------------------------------------------------
         if (take) {
             Candidate best;
             best.score = kNoScore; best.a = 0.0; best.b = 0.0; best.chi2 = 0.0;
             best.nh = 0; best.j0 = -1; best.j1 = -1; best.j2 = -1; best.j3 = -1;
-            const S2 s2 = extrapolate_seed(c, sh.sx[tid], sh.sy[tid], sh.stx[tid], sh.sty[tid], sh.sqop[tid]);
             const int f0 = sh.foff[tid];
             for (int k = 0; k < nFc; ++k) {
-                const int t = 3 * (f0 + k);
-                fit_first_hit(c, H, s2, my_slot[k], sh.near[t], sh.near[t + 1], sh.near[t + 2], best);
+                const int f = f0 + k;
+                const unsigned short ff = sh.ffit[f];
+                if (ff == kFitNone) continue;
+                const int j0 = idx_get(sh.near[3 * f][0]), j3 = (int)my_slot[k];
+                const int j1a = idx_get(sh.near[3 * f + 1][0]), j1b = idx_get(sh.near[3 * f + 1][1]);
+                const int j2a = idx_get(sh.near[3 * f + 2][0]), j2b = idx_get(sh.near[3 * f + 2][1]);
+                const int m1 = j1b >= 0 ? 2 : 1, m2 = j2b >= 0 ? 2 : 1;
+                const int nh = 1 + (j0 >= 0) + (j1a >= 0) + (j2a >= 0);
+                for (int i1 = 0; i1 < m1; ++i1) {
+                    for (int i2 = 0; i2 < m2; ++i2) {
+                        const int j1 = i1 ? j1b : j1a, j2 = i2 ? j2b : j2a;
+                        FitRes r;
+                        if (ff != kFitInline) {
+                            r = sh.res[ff + i1 * m2 + i2];
+                        } else {   // the round queued more fits than the fit phase takes
+                            const S2 s2 = extrapolate_seed(c, sh.sx[tid], sh.sy[tid], sh.stx[tid], sh.sty[tid], sh.sqop[tid]);
+                            r = fit_combo(c, H, s2, j0, j1, j2, j3, (double)sh.zw3[f].x, (double)sh.zw3[f].y);
+                        }
+                        if (r.score == kNoScore) continue;
+                        Candidate cand;
+                        cand.score = r.score; cand.a = r.a; cand.b = r.b; cand.chi2 = r.chi2;
+                        cand.nh = nh; cand.j0 = j0; cand.j1 = j1; cand.j2 = j2; cand.j3 = j3;
+                        if (cand.score < best.score || (cand.score == best.score && tie_better(H, cand, best))) best = cand;
+                    }
+                }
             }
             if (best.score == kNoScore) {
                 write_not_found(out, s);
@@ -490,13 +557,14 @@ __device__ __forceinline__ void track_event(const DevConst &c, TrackShared &sh, 
     }
 }
 
-__global__ void __launch_bounds__(kTrackThreads)
+__global__ void __launch_bounds__(kTrackThreads, 3)
 k_track(const __grid_constant__ DevConst c, const LayoutPtrs L, const ds_seeds seeds,
         const int32_t *__restrict__ hit_offsets, const int32_t *__restrict__ seed_offsets, const ds_tracks out, int cap)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    TrackShared &sh = *reinterpret_cast<TrackShared *>(smem_raw);
-    constexpr size_t kHitsAt = (sizeof(TrackShared) + 15) & ~(size_t)15;
+    using Staged = TrackShared<uint16_t>;
+    using Direct = TrackShared<int>;
+    constexpr size_t kHitsAt = (sizeof(Staged) + 15) & ~(size_t)15;
     float *st_x0 = reinterpret_cast<float *>(smem_raw + kHitsAt);   // [cap], then ymin [cap], ymax [cap]
     float *st_ymin = st_x0 + cap, *st_ymax = st_ymin + cap;
 
@@ -507,32 +575,34 @@ k_track(const __grid_constant__ DevConst c, const LayoutPtrs L, const ds_seeds s
     const int h0 = hit_offsets[e], h1 = hit_offsets[e + 1];
     // staged range: the event's slice widened to 16-byte boundaries (the sorted arrays are 256-byte aligned and padded)
     const int h0a = h0 & ~3, cnt = ((h1 + 3) & ~3) - h0a;
-    const bool staged = cnt <= cap;
+    const bool staged = cnt <= cap;   // cap < 65535 (see launch_track)
+    unsigned long long *bar = reinterpret_cast<unsigned long long *>(smem_raw);   // first member of both layouts
+    int *tab = staged ? reinterpret_cast<Staged *>(smem_raw)->tab : reinterpret_cast<Direct *>(smem_raw)->tab;
     if (tid == 0 && staged) {
-        mbar_init(&sh.bar, 1);
+        mbar_init(bar, 1);
         const uint32_t bytes = 4u * (uint32_t)cnt;
-        mbar_expect_tx(&sh.bar, 3u * bytes);
+        mbar_expect_tx(bar, 3u * bytes);
         if (bytes) {
-            bulk_g2s(st_x0, L.sx0 + h0a, bytes, &sh.bar);
-            bulk_g2s(st_ymin, L.symin + h0a, bytes, &sh.bar);
-            bulk_g2s(st_ymax, L.symax + h0a, bytes, &sh.bar);
+            bulk_g2s(st_x0, L.sx0 + h0a, bytes, bar);
+            bulk_g2s(st_ymin, L.symin + h0a, bytes, bar);
+            bulk_g2s(st_ymax, L.symax + h0a, bytes, bar);
         }
     }
     const int nb = c.n_bins;
     const int32_t *gtab = L.bin_offsets + (size_t)e * (nb + 1);
-    for (int b = tid; b <= nb; b += kTrackThreads) sh.tab[b] = gtab[b];
+    for (int b = tid; b <= nb; b += kTrackThreads) tab[b] = gtab[b];
     __syncthreads();
 
     EventHits H;
     H.z = L.sz + h0; H.w = L.sw + h0; H.id = L.sid + h0; H.perm = L.perm + h0;
     if (staged) {
-        mbar_wait(&sh.bar, 0);
+        mbar_wait(bar, 0);
         const int d = h0 - h0a;
         H.x0 = st_x0 + d; H.ymin = st_ymin + d; H.ymax = st_ymax + d;
-        track_event(c, sh, H, seeds, s_begin, s_end, out);
+        track_event<uint16_t>(c, *reinterpret_cast<Staged *>(smem_raw), H, seeds, s_begin, s_end, out);
     } else {
         H.x0 = L.sx0 + h0; H.ymin = L.symin + h0; H.ymax = L.symax + h0;
-        track_event(c, sh, H, seeds, s_begin, s_end, out);
+        track_event<int>(c, *reinterpret_cast<Direct *>(smem_raw), H, seeds, s_begin, s_end, out);
     }
 }
 
@@ -543,13 +613,16 @@ cudaError_t launch_track(const DevConst &c, const LayoutPtrs &lay, const ds_seed
                          cudaStream_t st, Prof &prof)
 {
     if (n_events <= 0) return cudaSuccess;
-    // staging capacity in hits (a multiple of 4, with room for the alignment slack): 12 bytes each
+    // staging capacity in hits (a multiple of 4, with room for the alignment slack): 12 bytes each; positions of a
+    // staged event are stored as uint16_t with 0xffff = none
     const int hint = max_event_hits_hint > 0 ? max_event_hits_hint : 4096;
-    const size_t fixed = ((sizeof(TrackShared) + 15) & ~(size_t)15);
-    const int cap_max = (int)((227 * 1024 - fixed) / 12) & ~3;
+    const size_t fixed = ((sizeof(TrackShared<uint16_t>) + 15) & ~(size_t)15);
+    int cap_max = (int)((227 * 1024 - fixed) / 12) & ~3;
+    if (cap_max > 65528) cap_max = 65528;
     int cap = ((hint + 3) & ~3) + 8;
     if (cap > cap_max) cap = cap_max;
-    const size_t smem = fixed + (size_t)cap * 12;
+    size_t smem = fixed + (size_t)cap * 12;
+    if (smem < sizeof(TrackShared<int>)) smem = sizeof(TrackShared<int>);   // the layout of an event that is not staged
     if ((int)smem > g_track_smem_set) {
         cudaError_t err = cudaFuncSetAttribute(k_track, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (err != cudaSuccess) return err;
