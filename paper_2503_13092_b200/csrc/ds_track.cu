@@ -151,6 +151,7 @@ struct TrackShared {
     int warp_sums[kTrackWarps + 1];
     int n_first;                          // entries of the first-hit list this round
     int n_fit;                            // fit tasks appended this round (may exceed kFitCap)
+    int fit_end;                          // tasks [0, fit_end) are queued; later appends did not fit the queue
     Idx slot[kTrackThreads * kMaxFirst];  // phase A: the seed's first hits (positions in the event's sorted slice)
     Idx near[3 * kFirstCap][2];           // phase B: closest / second closest hit of (first hit, layer)
     unsigned short foff[kTrackThreads];   // where the seed's first hits start in the round's list
@@ -186,6 +187,20 @@ __device__ __forceinline__ bool closer(const EventHits &H, double d1, int j1, do
     return H.id[j1] < H.id[j2];
 }
 
+// fp32 superset test of "|x0 + off - x| <= w" (decided in fp64 afterwards): |x0 - t| <= w', with t = (float)(x - off)
+// and w' = w widened by far more than the fp32 rounding of the difference (a few ulp of |t|)
+struct Prefilter {
+    float t, w;
+};
+
+__device__ __forceinline__ Prefilter make_prefilter(double target_x0, double w)
+{
+    Prefilter p;
+    p.t = (float)target_x0;
+    p.w = (float)w * 1.0001f + 0.01f + 2e-6f * fabsf(p.t);
+    return p;
+}
+
 // S4: closest and second closest y-compatible hit of layer l within w1 of the prediction xp; -1 = none
 __device__ __forceinline__ int2 search_layer(const DevConst &c, const EventHits &H, const int *tab, int l, double xp,
                                              double y, double w1)
@@ -194,12 +209,14 @@ __device__ __forceinline__ int2 search_layer(const DevConst &c, const EventHits 
     double d0 = 1e300, d1 = 1e300;
     const double off = c.dxdy[l] * y;
     const double lo = xp - off - w1, hi = xp - off + w1;
+    const Prefilter pf = make_prefilter(xp - off, w1);
     int tl, th;
     sector_range(c, y, tl, th);
     for (int sec = tl; sec <= th; ++sec) {
         int a, b;
         slice_range(c, tab, l, sec, lo, hi, a, b);
         for (int j = a; j < b; ++j) {
+            if (!(fabsf(H.x0[j] - pf.t) <= pf.w)) continue;
             const double d = fabs(((double)H.x0[j] + off) - xp);
             const bool pass = (d <= w1) & y_compatible(c, H, j, y);
             if (pass) {
@@ -365,6 +382,41 @@ __device__ __forceinline__ int block_inclusive_scan(int v, int *warp_sums)
     return inc + warp_sums[wid];
 }
 
+// S6 in full for one seed (first hits f0 .. f0+nF-1 of the round's list): every combination in turn, equal scores
+// resolved by (more hits, ids) (A-9), combinations that the fit phase did not take fitted here.
+template <typename Idx>
+__device__ __noinline__ Candidate choose_general(const DevConst &c, const TrackShared<Idx> &sh, const EventHits &H, int f0,
+                                                 int nF, int o)
+{
+    Candidate best;
+    best.score = kNoScore; best.a = 0.0; best.b = 0.0; best.chi2 = 0.0;
+    best.nh = 0; best.j0 = -1; best.j1 = -1; best.j2 = -1; best.j3 = -1;
+    const S2 s2 = extrapolate_seed(c, sh.sx[o], sh.sy[o], sh.stx[o], sh.sty[o], sh.sqop[o]);
+    for (int k = 0; k < nF; ++k) {
+        const int f = f0 + k;
+        const unsigned short ff = sh.ffit[f];
+        if (ff == kFitNone) continue;
+        const int j0 = idx_get(sh.near[3 * f][0]), j3 = (int)sh.slot[sh.fs[f]];
+        const int j1a = idx_get(sh.near[3 * f + 1][0]), j1b = idx_get(sh.near[3 * f + 1][1]);
+        const int j2a = idx_get(sh.near[3 * f + 2][0]), j2b = idx_get(sh.near[3 * f + 2][1]);
+        const int m1 = j1b >= 0 ? 2 : 1, m2 = j2b >= 0 ? 2 : 1;
+        const int nh = 1 + (j0 >= 0) + (j1a >= 0) + (j2a >= 0);
+        for (int i1 = 0; i1 < m1; ++i1) {
+            for (int i2 = 0; i2 < m2; ++i2) {
+                const int j1 = i1 ? j1b : j1a, j2 = i2 ? j2b : j2a;
+                const FitRes r = ff != kFitInline ? sh.res[(ff & 0xfff) + i1 * m2 + i2]
+                                                  : fit_combo(c, H, s2, j0, j1, j2, j3, (double)sh.zw3[f].x, (double)sh.zw3[f].y);
+                if (r.score == kNoScore) continue;
+                Candidate cand;
+                cand.score = r.score; cand.a = r.a; cand.b = r.b; cand.chi2 = r.chi2;
+                cand.nh = nh; cand.j0 = j0; cand.j1 = j1; cand.j2 = j2; cand.j3 = j3;
+                if (cand.score < best.score || (cand.score == best.score && tie_better(H, cand, best))) best = cand;
+            }
+        }
+    }
+    return best;
+}
+
 // All seeds of one event.  Every thread of the block runs this with the same arguments.
 template <typename Idx>
 __device__ __forceinline__ void track_event(const DevConst &c, TrackShared<Idx> &sh, const EventHits &H,
@@ -380,7 +432,7 @@ __device__ __forceinline__ void track_event(const DevConst &c, TrackShared<Idx> 
         const int s = s_base + tid;
         const bool act = s < s_end;
         int nF = 0;
-        if (tid == 0) sh.n_fit = 0;
+        if (tid == 0) { sh.n_fit = 0; sh.fit_end = kFitCap; }
         if (act) {
             const float fx = seeds.x[s], fy = seeds.y[s], ftx = seeds.tx[s], fty = seeds.ty[s], fq = seeds.qop[s];
             sh.sx[tid] = fx; sh.sy[tid] = fy; sh.stx[tid] = ftx; sh.sty[tid] = fty; sh.sqop[tid] = fq;
@@ -389,10 +441,12 @@ __device__ __forceinline__ void track_event(const DevConst &c, TrackShared<Idx> 
             sector_range(c, s2.y3, s_lo, s_hi);
             const double off3 = c.dxdy[3] * s2.y3;
             const double lo3 = s2.xc3 - off3 - s2.w0, hi3 = s2.xc3 - off3 + s2.w0;
+            const Prefilter pf = make_prefilter(s2.xc3 - off3, s2.w0);
             for (int sec = s_lo; sec <= s_hi; ++sec) {
                 int a, b;
                 slice_range(c, tab, 3, sec, lo3, hi3, a, b);
                 for (int j = a; j < b; ++j) {
+                    if (!(fabsf(H.x0[j] - pf.t) <= pf.w)) continue;
                     const double d = fabs(((double)H.x0[j] + off3) - s2.xc3);
                     if ((d <= s2.w0) & y_compatible(c, H, j, s2.y3)) {
                         if (nF < max_first) my_slot[nF] = (Idx)j;
@@ -476,12 +530,13 @@ __device__ __forceinline__ void track_event(const DevConst &c, TrackShared<Idx> 
                     const int m1 = 1 + ((has2 >> (g3 + 1)) & 1), m2 = 1 + ((has2 >> (g3 + 2)) & 1);
                     const int base = atomicAdd(&sh.n_fit, m1 * m2);
                     if (base + m1 * m2 <= kFitCap) {
-                        ff = (unsigned short)base;
+                        ff = (unsigned short)(base | ((m1 * m2) << 12));
                         for (int i1 = 0; i1 < m1; ++i1)
                             for (int i2 = 0; i2 < m2; ++i2)
                                 sh.task[base + i1 * m2 + i2] = (unsigned short)(f | (i1 << 9) | (i2 << 10));
                     } else {
                         ff = kFitInline;
+                        atomicMin(&sh.fit_end, base);
                     }
                 }
                 sh.ffit[f] = ff;
@@ -489,7 +544,7 @@ __device__ __forceinline__ void track_event(const DevConst &c, TrackShared<Idx> 
         }
         __syncthreads();
         // ---- fit phase: thread per queued combination -- S5 ------------------------------------------------------------
-        const int n_fit = min(sh.n_fit, kFitCap);
+        const int n_fit = min(sh.n_fit, sh.fit_end);
         for (int t = tid; t < n_fit; t += kTrackThreads) {
             const int tk = sh.task[t], f = tk & 511, i1 = (tk >> 9) & 1, i2 = (tk >> 10) & 1;
             const int sl = sh.fs[f], o = sl / kMaxFirst;
@@ -501,36 +556,38 @@ __device__ __forceinline__ void track_event(const DevConst &c, TrackShared<Idx> 
         __syncthreads();
         // ---- phase C: thread per seed -- S6 and the track record ---------------------------------------------------------
         if (take) {
-            Candidate best;
-            best.score = kNoScore; best.a = 0.0; best.b = 0.0; best.chi2 = 0.0;
-            best.nh = 0; best.j0 = -1; best.j1 = -1; best.j2 = -1; best.j3 = -1;
             const int f0 = sh.foff[tid];
+            // best score over the fit results of the seed's first hits; exact ties and fits that were not queued go
+            // through the general comparison below
+            double bscore = kNoScore;
+            int bf = -1, bq = 0;
+            bool general = false;
             for (int k = 0; k < nFc; ++k) {
-                const int f = f0 + k;
-                const unsigned short ff = sh.ffit[f];
+                const unsigned short ff = sh.ffit[f0 + k];
                 if (ff == kFitNone) continue;
-                const int j0 = idx_get(sh.near[3 * f][0]), j3 = (int)my_slot[k];
-                const int j1a = idx_get(sh.near[3 * f + 1][0]), j1b = idx_get(sh.near[3 * f + 1][1]);
-                const int j2a = idx_get(sh.near[3 * f + 2][0]), j2b = idx_get(sh.near[3 * f + 2][1]);
-                const int m1 = j1b >= 0 ? 2 : 1, m2 = j2b >= 0 ? 2 : 1;
-                const int nh = 1 + (j0 >= 0) + (j1a >= 0) + (j2a >= 0);
-                for (int i1 = 0; i1 < m1; ++i1) {
-                    for (int i2 = 0; i2 < m2; ++i2) {
-                        const int j1 = i1 ? j1b : j1a, j2 = i2 ? j2b : j2a;
-                        FitRes r;
-                        if (ff != kFitInline) {
-                            r = sh.res[ff + i1 * m2 + i2];
-                        } else {   // the round queued more fits than the fit phase takes
-                            const S2 s2 = extrapolate_seed(c, sh.sx[tid], sh.sy[tid], sh.stx[tid], sh.sty[tid], sh.sqop[tid]);
-                            r = fit_combo(c, H, s2, j0, j1, j2, j3, (double)sh.zw3[f].x, (double)sh.zw3[f].y);
-                        }
-                        if (r.score == kNoScore) continue;
-                        Candidate cand;
-                        cand.score = r.score; cand.a = r.a; cand.b = r.b; cand.chi2 = r.chi2;
-                        cand.nh = nh; cand.j0 = j0; cand.j1 = j1; cand.j2 = j2; cand.j3 = j3;
-                        if (cand.score < best.score || (cand.score == best.score && tie_better(H, cand, best))) best = cand;
-                    }
+                if (ff == kFitInline) { general = true; continue; }
+                const int base = ff & 0xfff, m = ff >> 12;
+                for (int q = 0; q < m; ++q) {
+                    const double sc = sh.res[base + q].score;
+                    if (sc < bscore) { bscore = sc; bf = f0 + k; bq = q; }
+                    else if (sc == bscore && sc != kNoScore) general = true;
                 }
+            }
+            Candidate best;
+            best.score = kNoScore;
+            if (general) {
+                best = choose_general<Idx>(c, sh, H, f0, nFc, tid);
+            } else if (bf >= 0) {
+                const int base = sh.ffit[bf] & 0xfff;
+                const FitRes r = sh.res[base + bq];
+                const int m2 = sh.near[3 * bf + 2][1] != (Idx)-1 ? 2 : 1;
+                const int i1 = bq / m2, i2 = bq - i1 * m2;
+                best.score = r.score; best.a = r.a; best.b = r.b; best.chi2 = r.chi2;
+                best.j0 = idx_get(sh.near[3 * bf][0]);
+                best.j1 = idx_get(sh.near[3 * bf + 1][i1]);
+                best.j2 = idx_get(sh.near[3 * bf + 2][i2]);
+                best.j3 = (int)sh.slot[sh.fs[bf]];
+                best.nh = 1 + (best.j0 >= 0) + (best.j1 >= 0) + (best.j2 >= 0);
             }
             if (best.score == kNoScore) {
                 write_not_found(out, s);
