@@ -30,7 +30,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if not force and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in deps):
         return LIB
     tmp = LIB + f".tmp{os.getpid()}"
-    cmd = [_nvcc()] + NVCC_FLAGS + ["-o", tmp] + srcs
+    cmd = [_nvcc()] + NVCC_FLAGS + os.environ.get("DS_NVCC_EXTRA", "").split() + ["-o", tmp] + srcs
     r = subprocess.run(cmd, capture_output=True, text=True)
     if verbose or r.returncode != 0:
         sys.stderr.write(r.stdout + r.stderr)

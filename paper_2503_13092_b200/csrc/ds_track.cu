@@ -20,7 +20,10 @@
 
 namespace ds {
 
-constexpr int kTrackThreads = 256;
+#ifndef DS_TRACK_THREADS
+#define DS_TRACK_THREADS 256
+#endif
+constexpr int kTrackThreads = DS_TRACK_THREADS;
 constexpr int kTrackWarps = kTrackThreads / 32;
 constexpr int kMaxBins = 4 * DS_MAX_SECTORS * kXBins;
 
@@ -129,8 +132,8 @@ __device__ __forceinline__ void mbar_wait(unsigned long long *bar, uint32_t pari
 }
 
 
-constexpr int kFirstCap = 384;   // first hits handled per round (>= DS_MAX_FIRST_HITS)
-constexpr int kFitCap = 256;     // fits handled by the fit phase per round; the rest are fitted by the seed's thread
+constexpr int kFirstCap = 64;    // first hits a warp handles per round (>= DS_MAX_FIRST_HITS)
+constexpr int kFitCap = 32;      // fits of the warp's fit phase per round; the rest are fitted by the seed's thread
 constexpr double kNoScore = 1e300;
 constexpr unsigned short kFitNone = 0xffffu, kFitInline = 0xfffeu;
 
@@ -138,28 +141,32 @@ struct FitRes {
     double score, a, b, chi2;   // score = kNoScore: the combination fails the chi2/ndf cut
 };
 
-// Block-shared state of k_track (carved from dynamic shared memory, followed by the staged hit arrays).  Idx is the
+// State of one warp of k_track: the warp takes up to 32 seeds of the event through all phases on its own.  Idx is the
 // type hit positions inside the event are stored in: uint16_t when the event is staged (it then has < 65535 hits),
 // int otherwise.  (Idx)-1 = none.
 template <typename Idx>
-struct TrackShared {
-    unsigned long long bar;
+struct WarpShared {
     FitRes res[kFitCap];                  // fit phase: result of fit task i
     float2 zw3[kFirstCap];                // (z, w) of the first hit
-    int tab[kMaxBins + 1];                // the event's bin table
-    float sx[kTrackThreads], sy[kTrackThreads], stx[kTrackThreads], sty[kTrackThreads], sqop[kTrackThreads];
-    int warp_sums[kTrackWarps + 1];
-    int n_first;                          // entries of the first-hit list this round
+    float sx[32], sy[32], stx[32], sty[32], sqop[32];
     int n_fit;                            // fit tasks appended this round (may exceed kFitCap)
     int fit_end;                          // tasks [0, fit_end) are queued; later appends did not fit the queue
-    Idx slot[kTrackThreads * kMaxFirst];  // phase A: the seed's first hits (positions in the event's sorted slice)
+    Idx slot[32 * kMaxFirst];             // phase A: the seed's first hits (positions in the event's sorted slice)
     Idx near[3 * kFirstCap][2];           // phase B: closest / second closest hit of (first hit, layer)
-    unsigned short foff[kTrackThreads];   // where the seed's first hits start in the round's list
+    unsigned short foff[32];              // where the seed's first hits start in the round's list
     unsigned short fs[kFirstCap];         // first-hit list: index into slot[]
-    unsigned short ffit[kFirstCap];       // first fit task of the first hit, kFitNone or kFitInline
+    unsigned short ffit[kFirstCap];       // first fit task of the first hit (| combinations << 12), kFitNone or kFitInline
     unsigned short task[kFitCap];         // fit task: first hit | i1 << 9 | i2 << 10
 };
-static_assert(kFirstCap <= 512, "fit task packs the first hit in 9 bits");
+
+// Block-shared state of k_track (carved from dynamic shared memory, followed by the staged hit arrays).
+template <typename Idx>
+struct TrackShared {
+    unsigned long long bar;
+    int tab[kMaxBins + 1];                // the event's bin table
+    WarpShared<Idx> warp[kTrackWarps];
+};
+static_assert(kFirstCap <= 512 && kFitCap < 0xfff, "packing of task[] and ffit[]");
 
 // The event's hits as the searches see them: x0 / ymin / ymax from the staging buffer (or global for an oversize
 // event), the rest always from global memory.  Indices are relative to the event's sorted slice.
@@ -356,36 +363,10 @@ __device__ __forceinline__ void write_not_found(const ds_tracks &out, int64_t s)
     reinterpret_cast<int4 *>(out.hit)[s] = make_int4(-1, -1, -1, -1);
 }
 
-// inclusive scan of one int per thread over the block; every thread of the block calls it
-__device__ __forceinline__ int block_inclusive_scan(int v, int *warp_sums)
-{
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    int inc = v;
-#pragma unroll
-    for (int d = 1; d < 32; d <<= 1) {
-        const int t = __shfl_up_sync(0xffffffffu, inc, d);
-        if (lane >= d) inc += t;
-    }
-    if (lane == 31) warp_sums[wid] = inc;
-    __syncthreads();
-    if (wid == 0) {
-        const int ws = lane < kTrackWarps ? warp_sums[lane] : 0;
-        int wi = ws;
-#pragma unroll
-        for (int d = 1; d < kTrackWarps; d <<= 1) {
-            const int t = __shfl_up_sync(0xffffffffu, wi, d);
-            if (lane >= d) wi += t;
-        }
-        if (lane < kTrackWarps) warp_sums[lane] = wi - ws;
-    }
-    __syncthreads();
-    return inc + warp_sums[wid];
-}
-
-// S6 in full for one seed (first hits f0 .. f0+nF-1 of the round's list): every combination in turn, equal scores
-// resolved by (more hits, ids) (A-9), combinations that the fit phase did not take fitted here.
+// S6 in full for one seed (first hits f0 .. f0+nF-1 of the warp's list, seed in lane o): every combination in turn,
+// equal scores resolved by (more hits, ids) (A-9), combinations that the fit phase did not take fitted here.
 template <typename Idx>
-__device__ __noinline__ Candidate choose_general(const DevConst &c, const TrackShared<Idx> &sh, const EventHits &H, int f0,
+__device__ __noinline__ Candidate choose_general(const DevConst &c, const WarpShared<Idx> &sh, const EventHits &H, int f0,
                                                  int nF, int o)
 {
     Candidate best;
@@ -417,25 +398,30 @@ __device__ __noinline__ Candidate choose_general(const DevConst &c, const TrackS
     return best;
 }
 
-// All seeds of one event.  Every thread of the block runs this with the same arguments.
+// Seeds [cb, ce) (at most 32) of one event, by one warp on its own: rounds of
+//   A  lane per seed:       S2, first window in UTbX (S3) -> the seed's <= max_first first hits; warp scan of the counts
+//   B  three lanes per first hit, one per layer: refined windows (S4); the first lane of the three queues the fits
+//   F  lane per queued combination: fit (S5)
+//   C  lane per seed:       best candidate (S6), track record
+// A round takes the longest prefix of the remaining seeds whose first hits fit the warp's list.
 template <typename Idx>
-__device__ __forceinline__ void track_event(const DevConst &c, TrackShared<Idx> &sh, const EventHits &H,
-                                            const ds_seeds &seeds, int s_begin, int s_end, const ds_tracks &out)
+__device__ __forceinline__ void track_chunk(const DevConst &c, WarpShared<Idx> &sh, const int *tab, const EventHits &H,
+                                            const ds_seeds &seeds, int cb, int ce, const ds_tracks &out)
 {
-    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    const unsigned FULL = 0xffffffffu;
+    const int lane = threadIdx.x & 31;
     const int max_first = c.max_first;
-    const int *tab = sh.tab;
-    Idx *my_slot = sh.slot + tid * kMaxFirst;
-    int s_base = s_begin;
-    while (s_base < s_end) {
-        // ---- phase A: thread per seed -- S2, S3 ------------------------------------------------------------------------
-        const int s = s_base + tid;
-        const bool act = s < s_end;
+    Idx *my_slot = sh.slot + lane * kMaxFirst;
+    int s_base = cb;
+    while (s_base < ce) {
+        // ---- phase A: lane per seed -- S2, S3 ----------------------------------------------------------------------------
+        const int s = s_base + lane;
+        const bool act = s < ce;
         int nF = 0;
-        if (tid == 0) { sh.n_fit = 0; sh.fit_end = kFitCap; }
+        if (lane == 0) { sh.n_fit = 0; sh.fit_end = kFitCap; }
         if (act) {
             const float fx = seeds.x[s], fy = seeds.y[s], ftx = seeds.tx[s], fty = seeds.ty[s], fq = seeds.qop[s];
-            sh.sx[tid] = fx; sh.sy[tid] = fy; sh.stx[tid] = ftx; sh.sty[tid] = fty; sh.sqop[tid] = fq;
+            sh.sx[lane] = fx; sh.sy[lane] = fy; sh.stx[lane] = ftx; sh.sty[lane] = fty; sh.sqop[lane] = fq;
             const S2 s2 = extrapolate_seed(c, fx, fy, ftx, fty, fq);
             int s_lo, s_hi;
             sector_range(c, s2.y3, s_lo, s_hi);
@@ -485,26 +471,31 @@ __device__ __forceinline__ void track_event(const DevConst &c, TrackShared<Idx> 
             }
         }
         const int nFc = min(nF, max_first);
-        const int incl = block_inclusive_scan(nFc, sh.warp_sums);
+        int incl = nFc;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const int t = __shfl_up_sync(FULL, incl, d);
+            if (lane >= d) incl += t;
+        }
         // the seeds taken this round are the longest prefix whose first hits fit the list
         const bool take = act && incl <= kFirstCap;
-        const int n_take = __syncthreads_count(take);
+        const unsigned take_mask = __ballot_sync(FULL, take);
+        const int n_take = __popc(take_mask);
+        const int n_first = __shfl_sync(FULL, incl, n_take - 1);
         if (take) {
             const int pos = incl - nFc;
-            if (tid == n_take - 1) sh.n_first = incl;
-            sh.foff[tid] = (unsigned short)pos;
+            sh.foff[lane] = (unsigned short)pos;
             for (int k = 0; k < nFc; ++k) {
                 const int j = (int)my_slot[k];
-                sh.fs[pos + k] = (unsigned short)(tid * kMaxFirst + k);
+                sh.fs[pos + k] = (unsigned short)(lane * kMaxFirst + k);
                 sh.zw3[pos + k] = make_float2(H.z[j], H.w[j]);
             }
         }
-        __syncthreads();
+        __syncwarp();
         // ---- phase B: three lanes per first hit, one per layer -- S4; lane 0 of the three queues the fits ----------------
-        const int n_first = sh.n_first;
-        for (int fb = 0; fb < n_first; fb += kTrackWarps * 10) {
+        for (int fb = 0; fb < n_first; fb += 10) {
             const int g = lane / 3, l = lane - 3 * g;
-            const int f = fb + wid * 10 + g;
+            const int f = fb + g;
             const bool on = lane < 30 && f < n_first;
             int2 r = make_int2(-1, -1);
             if (on) {
@@ -522,7 +513,7 @@ __device__ __forceinline__ void track_event(const DevConst &c, TrackShared<Idx> 
                 sh.near[3 * f + l][1] = (Idx)r.y;
             }
             const int g3 = min(3 * g, 29);
-            const unsigned has1 = __ballot_sync(0xffffffffu, r.x >= 0), has2 = __ballot_sync(0xffffffffu, r.y >= 0);
+            const unsigned has1 = __ballot_sync(FULL, r.x >= 0), has2 = __ballot_sync(FULL, r.y >= 0);
             if (on && l == 0) {
                 const int nh = 1 + ((has1 >> g3) & 1) + ((has1 >> (g3 + 1)) & 1) + ((has1 >> (g3 + 2)) & 1);
                 unsigned short ff = kFitNone;
@@ -542,23 +533,23 @@ __device__ __forceinline__ void track_event(const DevConst &c, TrackShared<Idx> 
                 sh.ffit[f] = ff;
             }
         }
-        __syncthreads();
-        // ---- fit phase: thread per queued combination -- S5 ------------------------------------------------------------
+        __syncwarp();
+        // ---- fit phase: lane per queued combination -- S5 ----------------------------------------------------------------
         const int n_fit = min(sh.n_fit, sh.fit_end);
-        for (int t = tid; t < n_fit; t += kTrackThreads) {
-            const int tk = sh.task[t], f = tk & 511, i1 = (tk >> 9) & 1, i2 = (tk >> 10) & 1;
+        if (lane < n_fit) {
+            const int tk = sh.task[lane], f = tk & 511, i1 = (tk >> 9) & 1, i2 = (tk >> 10) & 1;
             const int sl = sh.fs[f], o = sl / kMaxFirst;
             const S2 t2 = extrapolate_seed(c, sh.sx[o], sh.sy[o], sh.stx[o], sh.sty[o], sh.sqop[o]);
             const float2 zw = sh.zw3[f];
-            sh.res[t] = fit_combo(c, H, t2, idx_get(sh.near[3 * f][0]), idx_get(sh.near[3 * f + 1][i1]),
-                                  idx_get(sh.near[3 * f + 2][i2]), (int)sh.slot[sl], (double)zw.x, (double)zw.y);
+            sh.res[lane] = fit_combo(c, H, t2, idx_get(sh.near[3 * f][0]), idx_get(sh.near[3 * f + 1][i1]),
+                                     idx_get(sh.near[3 * f + 2][i2]), (int)sh.slot[sl], (double)zw.x, (double)zw.y);
         }
-        __syncthreads();
-        // ---- phase C: thread per seed -- S6 and the track record ---------------------------------------------------------
+        __syncwarp();
+        // ---- phase C: lane per seed -- S6 and the track record -----------------------------------------------------------
         if (take) {
-            const int f0 = sh.foff[tid];
+            const int f0 = sh.foff[lane];
             // best score over the fit results of the seed's first hits; exact ties and fits that were not queued go
-            // through the general comparison below
+            // through the general comparison
             double bscore = kNoScore;
             int bf = -1, bq = 0;
             bool general = false;
@@ -576,7 +567,7 @@ __device__ __forceinline__ void track_event(const DevConst &c, TrackShared<Idx> 
             Candidate best;
             best.score = kNoScore;
             if (general) {
-                best = choose_general<Idx>(c, sh, H, f0, nFc, tid);
+                best = choose_general<Idx>(c, sh, H, f0, nFc, lane);
             } else if (bf >= 0) {
                 const int base = sh.ffit[bf] & 0xfff;
                 const FitRes r = sh.res[base + bq];
@@ -592,7 +583,7 @@ __device__ __forceinline__ void track_event(const DevConst &c, TrackShared<Idx> 
             if (best.score == kNoScore) {
                 write_not_found(out, s);
             } else {
-                const double ys = (double)sh.sy[tid], txs = (double)sh.stx[tid], tys = (double)sh.sty[tid];
+                const double ys = (double)sh.sy[lane], txs = (double)sh.stx[lane], tys = (double)sh.sty[lane];
                 out.x[s] = (float)best.a;
                 out.y[s] = (float)(ys + tys * (c.z_ref - c.z_seed));
                 out.tx[s] = (float)best.b;
@@ -610,11 +601,25 @@ __device__ __forceinline__ void track_event(const DevConst &c, TrackShared<Idx> 
             }
         }
         s_base += n_take;
-        __syncthreads();   // the lists are rewritten by the next round
+        __syncwarp();   // the lists are rewritten by the next round
     }
 }
 
-__global__ void __launch_bounds__(kTrackThreads, 3)
+// All seeds of one event: every warp of the block takes an equal share (at most 32 at a time).
+template <typename Idx>
+__device__ __forceinline__ void track_event(const DevConst &c, TrackShared<Idx> &sh, const EventHits &H,
+                                            const ds_seeds &seeds, int s_begin, int s_end, const ds_tracks &out)
+{
+    const int wid = threadIdx.x >> 5;
+    const int chunk = min(32, (s_end - s_begin + kTrackWarps - 1) / kTrackWarps);
+    for (int cb = s_begin + wid * chunk; cb < s_end; cb += kTrackWarps * chunk)
+        track_chunk<Idx>(c, sh.warp[wid], sh.tab, H, seeds, cb, min(cb + chunk, s_end), out);
+}
+
+#ifndef DS_TRACK_MINBLOCKS
+#define DS_TRACK_MINBLOCKS 3
+#endif
+__global__ void __launch_bounds__(kTrackThreads, DS_TRACK_MINBLOCKS)
 k_track(const __grid_constant__ DevConst c, const LayoutPtrs L, const ds_seeds seeds,
         const int32_t *__restrict__ hit_offsets, const int32_t *__restrict__ seed_offsets, const ds_tracks out, int cap)
 {
