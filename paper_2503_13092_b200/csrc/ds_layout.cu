@@ -3,12 +3,15 @@
 // inside a sector and the x0 slices are this library's own layout (BASELINE north_star (1)).
 //
 // One thread block per event.  The sort is a counting sort on the fine bin (layer, sector, x0 slice) followed by a
-// rank inside each fine bin (a handful of hits), so there is no comparison network and no global scratch:
-//   A  histogram of the fine bins in shared memory (atomicAdd returns the hit's arrival slot in its bin)
+// rank inside each fine bin (a handful of hits), so there is no comparison network and no global scratch.  The
+// event's six input arrays are brought into shared memory by 1-D bulk async copies (cp.async.bulk + mbarrier), each
+// exactly once: x0 and id up front (they make the sort key), z while the sort runs, ymin / ymax / w into buffers as
+// they fall free, so that every load is in flight behind the work on the previous array:
+//   A  histogram of the fine bins (atomicAdd returns the hit's arrival slot in its bin)
 //   B  block-wide exclusive scan -> bin starts (= the bin table that is written out)
-//   C  arrival-ordered member list per bin
-//   D  rank of every hit among the members of its bin by (x0, id, original index) -> final position q
-//   E  field by field: scatter in[i] -> smem[q], then coalesced copy smem -> out (double buffered)
+//   C  orderable x0 keys and hit indices laid out bin by bin, in arrival order
+//   D  rank of every hit among the keys of its bin (ties: id, then original index) -> final position q; src[q] = hit
+//   E  per array: out[q] = staged[src[q]], coalesced stores
 // Events larger than the shared-memory capacity chosen from the caller's hint take an O(n^2) rank over global
 // memory (phase A/B identical), which yields the same permutation.
 #include "ds_common.cuh"
@@ -61,51 +64,79 @@ __device__ void block_exclusive_scan(int *v, int n, int *warp_sums)
     __syncthreads();
 }
 
+// Stage global src[h0 .. h0+n) into a shared buffer so that element i sits at buf[(h0 & 3) + i]: the part of the slice
+// between 16-byte boundaries by one bulk async copy that completes on `bar` (issued by thread 0, which also arms the
+// barrier), the up to three elements after the last boundary by ordinary loads (threads 32..34).  With `bulk` false
+// (a source pointer that is not 16-byte aligned) everything is loaded by ordinary loads and the barrier only armed.
+// Every thread of the block calls it; the buffer must be free (a __syncthreads after its last reader), and a
+// __syncthreads plus mbar_wait(bar) must precede the first read.
 template <typename T>
-__device__ __forceinline__ void scatter_field(const T *__restrict__ in, T *buf, const uint32_t *q, int n)
+__device__ __forceinline__ void stage_field(T *buf, const T *__restrict__ src, int h0, int n, unsigned long long *bar,
+                                            bool bulk)
 {
-    for (int i = threadIdx.x; i < n; i += blockDim.x) buf[q[i]] = in[i];
-}
-
-template <typename T>
-__device__ __forceinline__ void copy_out(const T *buf, T *__restrict__ out, int n)
-{
-    for (int i = threadIdx.x; i < n; i += blockDim.x) out[i] = buf[i];
+    const int d = h0 & 3, h0a = h0 - d, h1 = h0 + n;
+    const int h1dn = bulk ? max(h1 & ~3, h0a) : h0a;          // bulk part: [h0a, h1dn); it may start before h0
+    if (threadIdx.x == 0) {
+        const uint32_t bytes = 4u * (uint32_t)(h1dn - h0a);
+        mbar_expect_tx(bar, bytes);
+        if (bytes) bulk_g2s(buf, src + h0a, bytes, bar);
+    }
+    if (bulk) {
+        const int t = (int)threadIdx.x - 32;
+        if (t >= 0 && h1dn + t < h1 && h1dn + t >= h0) buf[h1dn + t - h0a] = src[h1dn + t];
+    } else {
+        for (int i = threadIdx.x; i < n; i += blockDim.x) buf[d + i] = src[h0 + i];
+    }
 }
 
 __global__ void __launch_bounds__(kLayoutThreads)
-k_layout(const __grid_constant__ DevConst c, const LayoutPtrs p, const int32_t *__restrict__ hit_offsets, int cap)
+k_layout(const __grid_constant__ DevConst c, const LayoutPtrs p, const int32_t *__restrict__ hit_offsets, int cap, bool bulk)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ int warp_sums[33];
+    __shared__ __align__(8) unsigned long long bars[3];
     const int nb = c.n_bins;
-    int *hist = reinterpret_cast<int *>(smem_raw);                    // [nb + 1]
-    uint32_t *keyx = reinterpret_cast<uint32_t *>(hist + kMaxBins + 1); // [cap] orderable x0
-    uint32_t *pk = keyx + cap;                                         // [cap] bin << 20 | slot, later q
-    uint32_t *bufA = pk + cap, *bufB = bufA + cap;                     // [cap] staging
-    uint16_t *lst = reinterpret_cast<uint16_t *>(bufB + cap);          // [cap] members of each bin, arrival order
+    // cap is a multiple of 4, so every array starts on a 16-byte boundary
+    float *s_x0 = reinterpret_cast<float *>(smem_raw);                 // [cap] x0, later ymin
+    int32_t *s_id = reinterpret_cast<int32_t *>(s_x0 + cap);           // [cap] id, later ymax
+    uint32_t *s_pk = reinterpret_cast<uint32_t *>(s_id + cap);         // [cap] bin << 20 | slot, later q
+    uint32_t *s_buf = s_pk + cap;                                      // [cap] keys in bin order, later z, later w
+    uint16_t *s_src = reinterpret_cast<uint16_t *>(s_buf + cap);       // [cap] hits in bin order, later src[q]
+    int *hist = reinterpret_cast<int *>(s_src + cap);                  // [nb + 1]
+    unsigned long long *bar_x = &bars[0], *bar_i = &bars[1], *bar_b = &bars[2];
 
     const int e = blockIdx.x;
     const int h0 = hit_offsets[e];
     const int n = hit_offsets[e + 1] - h0;
     const int tid = threadIdx.x;
-    const bool fast = n <= cap;
-    const float *x0 = p.x0 + h0;
-    const int32_t *hid = p.id + h0;
+    const int d = h0 & 3;
+    const bool fast = n + 3 <= cap;
 
+    if (tid == 0) {
+        mbar_init(bar_x, 1);
+        mbar_init(bar_i, 1);
+        mbar_init(bar_b, 1);
+    }
     for (int b = tid; b <= nb; b += blockDim.x) hist[b] = 0;
     __syncthreads();
-    // A
-    for (int i = tid; i < n; i += blockDim.x) {
-        float x = x0[i];
-        int b = fine_bin(c, hid[i], x);
-        int slot = atomicAdd(&hist[b], 1);
-        if (fast) {
-            keyx[i] = float_key(x);
-            pk[i] = ((uint32_t)b << 20) | (uint32_t)slot;
+
+    if (fast) {
+        stage_field(s_x0, p.x0, h0, n, bar_x, bulk);
+        stage_field(s_id, p.id, h0, n, bar_i, bulk);
+        __syncthreads();
+        mbar_wait(bar_x, 0);
+        mbar_wait(bar_i, 0);
+        // A
+        for (int i = tid; i < n; i += blockDim.x) {
+            const int b = fine_bin(c, s_id[d + i], s_x0[d + i]);
+            const int slot = atomicAdd(&hist[b], 1);
+            s_pk[i] = ((uint32_t)b << 20) | (uint32_t)slot;
         }
+        __syncthreads();
+    } else {
+        for (int i = tid; i < n; i += blockDim.x) atomicAdd(&hist[fine_bin(c, p.id[h0 + i], p.x0[h0 + i])], 1);
+        __syncthreads();
     }
-    __syncthreads();
     // B
     block_exclusive_scan(hist, nb, warp_sums);
     int32_t *tab = p.bin_offsets + (size_t)e * (nb + 1);
@@ -114,53 +145,67 @@ k_layout(const __grid_constant__ DevConst c, const LayoutPtrs p, const int32_t *
     if (fast) {
         // C
         for (int i = tid; i < n; i += blockDim.x) {
-            uint32_t v = pk[i];
-            lst[hist[v >> 20] + (v & 0xfffffu)] = (uint16_t)i;
+            const uint32_t v = s_pk[i];
+            const int pos = hist[v >> 20] + (int)(v & 0xfffffu);
+            s_buf[pos] = float_key(s_x0[d + i]);
+            s_src[pos] = (uint16_t)i;
         }
         __syncthreads();
         // D
         for (int i = tid; i < n; i += blockDim.x) {
-            const int b = pk[i] >> 20;
-            const uint32_t ki = keyx[i];
+            const int b = s_pk[i] >> 20;
+            const uint32_t ki = float_key(s_x0[d + i]);
             const int jb = hist[b], je = hist[b + 1];
-            int rank = 0;
+            int rank = 0, eq = 0;
             for (int j = jb; j < je; ++j) {
-                const int m = lst[j];
-                const uint32_t km = keyx[m];
-                bool less = km < ki;
-                if (km == ki && m != i) {
-                    const int im = hid[m], ii = hid[i];
-                    less = im < ii || (im == ii && m < i);
-                }
-                rank += less ? 1 : 0;
+                const uint32_t km = s_buf[j];
+                rank += km < ki ? 1 : 0;
+                eq += km == ki ? 1 : 0;
             }
-            pk[i] = (uint32_t)(jb + rank);   // q (pk[i] is only ever touched by the thread that owns hit i)
+            if (eq > 1) {   // equal x0 inside the bin: order by (id, original index)
+                const int ii = s_id[d + i];
+                for (int j = jb; j < je; ++j) {
+                    const int m = s_src[j];
+                    if (s_buf[j] == ki && m != i) {
+                        const int im = s_id[d + m];
+                        rank += (im < ii || (im == ii && m < i)) ? 1 : 0;
+                    }
+                }
+            }
+            s_pk[i] = (uint32_t)(jb + rank);   // q
         }
         __syncthreads();
-        // E: perm, x0, z, ymin, ymax, w, id
-        for (int i = tid; i < n; i += blockDim.x) bufA[pk[i]] = (uint32_t)(h0 + i);
+        for (int i = tid; i < n; i += blockDim.x) s_src[s_pk[i]] = (uint16_t)i;
         __syncthreads();
-        scatter_field(x0, reinterpret_cast<float *>(bufB), pk, n);
-        copy_out(reinterpret_cast<int32_t *>(bufA), p.perm + h0, n);
+        // E: z is loaded while perm, x0 and id go out; ymin, ymax, w follow into the buffers that fall free
+        stage_field(reinterpret_cast<float *>(s_buf), p.z, h0, n, bar_b, bulk);
+        for (int q = tid; q < n; q += blockDim.x) {
+            const int i = s_src[q];
+            p.perm[h0 + q] = h0 + i;
+            p.sx0[h0 + q] = s_x0[d + i];
+            p.sid[h0 + q] = s_id[d + i];
+        }
         __syncthreads();
-        scatter_field(p.z + h0, reinterpret_cast<float *>(bufA), pk, n);
-        copy_out(reinterpret_cast<float *>(bufB), p.sx0 + h0, n);
+        stage_field(s_x0, p.ymin, h0, n, bar_x, bulk);
+        stage_field(reinterpret_cast<float *>(s_id), p.ymax, h0, n, bar_i, bulk);
+        mbar_wait(bar_b, 0);
+        for (int q = tid; q < n; q += blockDim.x) p.sz[h0 + q] = reinterpret_cast<float *>(s_buf)[d + s_src[q]];
         __syncthreads();
-        scatter_field(p.ymin + h0, reinterpret_cast<float *>(bufB), pk, n);
-        copy_out(reinterpret_cast<float *>(bufA), p.sz + h0, n);
+        stage_field(reinterpret_cast<float *>(s_buf), p.w, h0, n, bar_b, bulk);
+        mbar_wait(bar_x, 1);
+        mbar_wait(bar_i, 1);
+        for (int q = tid; q < n; q += blockDim.x) {
+            const int i = d + s_src[q];
+            p.symin[h0 + q] = s_x0[i];
+            p.symax[h0 + q] = reinterpret_cast<float *>(s_id)[i];
+        }
         __syncthreads();
-        scatter_field(p.ymax + h0, reinterpret_cast<float *>(bufA), pk, n);
-        copy_out(reinterpret_cast<float *>(bufB), p.symin + h0, n);
-        __syncthreads();
-        scatter_field(p.w + h0, reinterpret_cast<float *>(bufB), pk, n);
-        copy_out(reinterpret_cast<float *>(bufA), p.symax + h0, n);
-        __syncthreads();
-        scatter_field(hid, reinterpret_cast<int32_t *>(bufA), pk, n);
-        copy_out(reinterpret_cast<float *>(bufB), p.sw + h0, n);
-        __syncthreads();
-        copy_out(reinterpret_cast<int32_t *>(bufA), p.sid + h0, n);
+        mbar_wait(bar_b, 1);
+        for (int q = tid; q < n; q += blockDim.x) p.sw[h0 + q] = reinterpret_cast<float *>(s_buf)[d + s_src[q]];
     } else {
         // oversize event: rank over the whole event straight from global memory, scattered writes
+        const float *x0 = p.x0 + h0;
+        const int32_t *hid = p.id + h0;
         for (int i = tid; i < n; i += blockDim.x) {
             const float xi = x0[i];
             const int ii = hid[i];
@@ -188,22 +233,35 @@ k_layout(const __grid_constant__ DevConst c, const LayoutPtrs p, const int32_t *
     }
 }
 
-static size_t layout_smem_bytes(int cap) { return sizeof(int) * (kMaxBins + 1) + (size_t)cap * (4 * 4 + 2) + 16; }
+
+static size_t layout_smem_bytes(int cap) { return (size_t)cap * 18 + sizeof(int) * (kMaxBins + 1) + 16; }
+
+static int g_layout_smem_set = -1;
 
 cudaError_t launch_layout(const DevConst &c, const LayoutPtrs &p, const int32_t *hit_offsets, int n_events,
                           int max_event_hits_hint, cudaStream_t st, Prof &prof)
 {
     if (n_events <= 0) return cudaSuccess;
-    int hint = max_event_hits_hint > 0 ? max_event_hits_hint : 4096;
-    int cap = (hint + 255) & ~255;
-    const int cap_max = (int)((227 * 1024 - sizeof(int) * (kMaxBins + 1) - 512) / 18) & ~255;   // 227 KB per CTA
+    // staging capacity in hits: a multiple of 4 with room for the alignment slack, 18 bytes each; hit indices inside an
+    // event are kept as uint16_t
+    const int hint = max_event_hits_hint > 0 ? max_event_hits_hint : 4096;
+    int cap = ((hint + 3) & ~3) + 8;
+    int cap_max = (int)((227 * 1024 - sizeof(int) * (kMaxBins + 1) - 512) / 18) & ~3;   // 227 KB per CTA
+    if (cap_max > 65532) cap_max = 65532;
     if (cap > cap_max) cap = cap_max;
-    if (cap > 65536) cap = 65536;   // lst holds uint16 indices
     const size_t smem = layout_smem_bytes(cap);
-    cudaError_t err = cudaFuncSetAttribute(k_layout, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (err != cudaSuccess) return err;
+    if ((int)smem > g_layout_smem_set) {
+        cudaError_t err = cudaFuncSetAttribute(k_layout, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (err != cudaSuccess) return err;
+        g_layout_smem_set = (int)smem;
+    }
+    // the bulk copies need 16-byte aligned sources (offsets inside the arrays are handled by the kernel)
+    const uintptr_t bits = reinterpret_cast<uintptr_t>(p.x0) | reinterpret_cast<uintptr_t>(p.z) |
+                           reinterpret_cast<uintptr_t>(p.ymin) | reinterpret_cast<uintptr_t>(p.ymax) |
+                           reinterpret_cast<uintptr_t>(p.w) | reinterpret_cast<uintptr_t>(p.id);
+    const bool bulk = (bits & 15) == 0;
     prof.begin(DS_K_LAYOUT, st);
-    k_layout<<<n_events, kLayoutThreads, smem, st>>>(c, p, hit_offsets, cap);
+    k_layout<<<n_events, kLayoutThreads, smem, st>>>(c, p, hit_offsets, cap, bulk);
     prof.end(st);
     return cudaGetLastError();
 }
