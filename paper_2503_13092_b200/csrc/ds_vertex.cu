@@ -6,7 +6,9 @@
 //
 // Three launches, all deterministic (count -> scan -> write, BASELINE north_star (5)):
 //   k_vertex_count  block per event: ordered compaction of the kept positive / negative tracks into a per-event list
-//                   (workspace), then all (pos, neg) pairs, lanes over pairs; number of passing pairs per event
+//                   (workspace) and, with the per-track terms of the masses (|d|, p/|d|, E_pi, E_p), into shared
+//                   memory; then all (pos, neg) pairs, lanes over pairs, masses only for pairs that pass the DOCA and
+//                   z cuts; number of passing pairs per event
 //   k_vertex_scan   one block: exclusive scan of the per-event counts -> offsets (int64), overflow count
 //   k_vertex_write  block per event: the pairs again, block-ordered compaction of the passing ones -> (ia, ib) order
 // Pair arithmetic is fp64 in registers (cuts decide list membership); results are stored as fp32.
@@ -14,122 +16,185 @@
 
 namespace ds {
 
-constexpr int kVtxThreads = 256;
+constexpr int kVtxThreads = 128;
 constexpr int kVtxWarps = kVtxThreads / 32;
+constexpr int kVtxCap = 512;   // seeds of an event whose kept tracks are staged in shared memory
 
 struct VtxOut {
     double x, y, z, doca, m_pipi, m_ppi;
     int flags;
 };
 
-__device__ __forceinline__ double inv_mass(double tx1, double ty1, double p1, double m1, double tx2, double ty2,
-                                           double p2, double m2)
+// A kept track as the pair loop sees it: state at z_ref and the per-track terms of the invariant masses
+// (|d| = sqrt(tx^2 + ty^2 + 1), p in MeV, k = p / |d|, E under the pion and the proton hypothesis).
+struct VtxTrack {
+    double x, y, tx, ty, p, k, e_pi, e_p;
+};
+
+__device__ __forceinline__ VtxTrack make_track(const DevConst &c, const ds_tracks &t, int i)
 {
-    const double n1 = sqrt(tx1 * tx1 + ty1 * ty1 + 1.0), n2 = sqrt(tx2 * tx2 + ty2 * ty2 + 1.0);
-    const double k1 = p1 / n1, k2 = p2 / n2;
-    const double px = k1 * tx1 + k2 * tx2, py = k1 * ty1 + k2 * ty2, pz = k1 + k2;
-    const double E = sqrt(p1 * p1 + m1 * m1) + sqrt(p2 * p2 + m2 * m2);
-    const double M2 = E * E - (px * px + py * py + pz * pz);
-    return M2 > 0.0 ? sqrt(M2) : 0.0;
+    VtxTrack r;
+    r.x = t.x[i]; r.y = t.y[i]; r.tx = t.tx[i]; r.ty = t.ty[i];
+    const double q = t.qop[i];
+    r.p = 1000.0 / fabs(q);   // MeV
+    r.k = r.p / sqrt(r.tx * r.tx + r.ty * r.ty + 1.0);
+    r.e_pi = sqrt(r.p * r.p + c.m_pi * c.m_pi);
+    r.e_p = sqrt(r.p * r.p + c.m_p * c.m_p);
+    return r;
 }
 
-// a = positive track, b = negative track.  Returns true iff the pair passes every cut.
-__device__ __forceinline__ bool vertex_pair(const DevConst &c, double xa, double ya, double txa, double tya, double qa,
-                                            double xb, double yb, double txb, double tyb, double qb, VtxOut &o)
+// Kept tracks of one event in shared memory (positive tracks from the front, negative tracks from the back).
+struct VtxShared {
+    float x[kVtxCap], y[kVtxCap], tx[kVtxCap], ty[kVtxCap];
+    double p[kVtxCap], k[kVtxCap], e_pi[kVtxCap], e_p[kVtxCap];
+    __device__ __forceinline__ void put(int pos, const VtxTrack &r)
+    {
+        x[pos] = (float)r.x; y[pos] = (float)r.y; tx[pos] = (float)r.tx; ty[pos] = (float)r.ty;   // exact: they were fp32
+        p[pos] = r.p; k[pos] = r.k; e_pi[pos] = r.e_pi; e_p[pos] = r.e_p;
+    }
+    __device__ __forceinline__ VtxTrack get(int pos) const
+    {
+        VtxTrack r;
+        r.x = x[pos]; r.y = y[pos]; r.tx = tx[pos]; r.ty = ty[pos];
+        r.p = p[pos]; r.k = k[pos]; r.e_pi = e_pi[pos]; r.e_p = e_p[pos];
+        return r;
+    }
+};
+
+// a = positive track, b = negative track.  Returns true iff the pair passes every cut; o is complete only then.
+__device__ __forceinline__ bool vertex_pair(const DevConst &c, const VtxTrack &a, const VtxTrack &b, VtxOut &o)
 {
     // n = d_a x d_b with d = (tx, ty, 1): built from slope differences; |n|^2 = A*C - B^2 (Lagrange) without cancellation
-    const double nx = tya - tyb, ny = txb - txa, nz = txa * tyb - tya * txb;
+    const double nx = a.ty - b.ty, ny = b.tx - a.tx, nz = a.tx * b.ty - a.ty * b.tx;
     const double n2 = nx * nx + ny * ny + nz * nz;
     if (n2 < c.n2_min) return false;
-    const double A = txa * txa + tya * tya + 1.0, B = txa * txb + tya * tyb + 1.0, C = txb * txb + tyb * tyb + 1.0;
-    const double rx = xa - xb, ry = ya - yb;
-    const double Dd = txa * rx + tya * ry, Ee = txb * rx + tyb * ry;
+    const double A = a.tx * a.tx + a.ty * a.ty + 1.0, B = a.tx * b.tx + a.ty * b.ty + 1.0, C = b.tx * b.tx + b.ty * b.ty + 1.0;
+    const double rx = a.x - b.x, ry = a.y - b.y;
+    const double Dd = a.tx * rx + a.ty * ry, Ee = b.tx * rx + b.ty * ry;
     const double sa = (B * Ee - C * Dd) / n2, sb = (A * Ee - B * Dd) / n2;
-    const double qax = xa + sa * txa, qay = ya + sa * tya, qaz = c.z_ref + sa;
-    const double qbx = xb + sb * txb, qby = yb + sb * tyb, qbz = c.z_ref + sb;
+    const double qax = a.x + sa * a.tx, qay = a.y + sa * a.ty, qaz = c.z_ref + sa;
+    const double qbx = b.x + sb * b.tx, qby = b.y + sb * b.ty, qbz = c.z_ref + sb;
     const double dx = qax - qbx, dy = qay - qby, dz = qaz - qbz;
     o.x = 0.5 * (qax + qbx);
     o.y = 0.5 * (qay + qby);
     o.z = 0.5 * (qaz + qbz);
     o.doca = sqrt(dx * dx + dy * dy + dz * dz);
-    const double pa = 1000.0 / fabs(qa), pb = 1000.0 / fabs(qb);   // MeV
-    o.m_pipi = inv_mass(txa, tya, pa, c.m_pi, txb, tyb, pb, c.m_pi);
-    o.m_ppi = pa >= pb ? inv_mass(txa, tya, pa, c.m_p, txb, tyb, pb, c.m_pi)
-                       : inv_mass(txa, tya, pa, c.m_pi, txb, tyb, pb, c.m_p);
+    if (!(o.doca < c.doca_max && c.zv_min <= o.z && o.z <= c.zv_max)) return false;
+    // invariant masses: same momentum sum under both hypotheses; proton = larger momentum (A-15)
+    const double px = a.k * a.tx + b.k * b.tx, py = a.k * a.ty + b.k * b.ty, pz = a.k + b.k;
+    const double p2 = px * px + py * py + pz * pz;
+    const double e1 = a.e_pi + b.e_pi, e2 = a.p >= b.p ? a.e_p + b.e_pi : a.e_pi + b.e_p;
+    const double m1 = e1 * e1 - p2, m2 = e2 * e2 - p2;
+    o.m_pipi = m1 > 0.0 ? sqrt(m1) : 0.0;
+    o.m_ppi = m2 > 0.0 ? sqrt(m2) : 0.0;
     o.flags = (fabs(o.m_pipi - c.m_ks) < c.dm_ks ? 1 : 0) | (fabs(o.m_ppi - c.m_lambda) < c.dm_lambda ? 2 : 0);
-    return o.doca < c.doca_max && c.zv_min <= o.z && o.z <= c.zv_max && o.flags != 0;
-}
-
-// Exclusive offset of this thread's flag inside the block (thread order) and the block total.
-__device__ __forceinline__ int block_ordered_offset(bool flag, int *warp_cnt, int &total)
-{
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    const unsigned m = __ballot_sync(0xffffffffu, flag);
-    if (lane == 0) warp_cnt[wid] = __popc(m);
-    __syncthreads();
-    int before = 0, tot = 0;
-#pragma unroll
-    for (int w = 0; w < kVtxWarps; ++w) {
-        const int cw = warp_cnt[w];
-        if (w < wid) before += cw;
-        tot += cw;
-    }
-    __syncthreads();
-    total = tot;
-    return before + __popc(m & lanemask_lt());
+    return o.flags != 0;
 }
 
 struct PairLists {
-    int32_t *list;   // [n_seeds]: event e keeps its positive tracks at [s0, s0+npos), negative at [s0+npos, s0+npos+nneg)
+    int32_t *list;   // [n_seeds]: event e (seeds [s0, s1)) keeps its positive tracks at s0, s0+1, ... and its negative
+                     // tracks at s1-1, s1-2, ..., both in seed order
     int32_t *npos;   // [n_events]
     int32_t *nneg;   // [n_events]
 };
 
-__device__ __forceinline__ void load_pair(const ds_tracks &t, int ia, int ib, double &xa, double &ya, double &txa,
-                                          double &tya, double &qa, double &xb, double &yb, double &txb, double &tyb,
-                                          double &qb)
+// Track of pair k = a * nneg + b of the event: from shared memory if the event is staged, else from global memory.
+struct PairSource {
+    const VtxShared *sh;   // nullptr: not staged
+    const int32_t *list;   // the event's slice of PairLists::list
+    int n_seeds, nneg;
+};
+
+__device__ __forceinline__ void pair_tracks(const DevConst &c, const ds_tracks &t, const PairSource &ps, int64_t k,
+                                            VtxTrack &ta, VtxTrack &tb, int &ia, int &ib)
 {
-    xa = t.x[ia]; ya = t.y[ia]; txa = t.tx[ia]; tya = t.ty[ia]; qa = t.qop[ia];
-    xb = t.x[ib]; yb = t.y[ib]; txb = t.tx[ib]; tyb = t.ty[ib]; qb = t.qop[ib];
+    int pa, pb;
+    if (k <= 0xffffffffLL) {   // 32-bit division when it fits
+        const unsigned a = (unsigned)k / (unsigned)ps.nneg;
+        pa = (int)a;
+        pb = ps.n_seeds - 1 - (int)((unsigned)k - a * (unsigned)ps.nneg);
+    } else {
+        const int64_t a = k / ps.nneg;
+        pa = (int)a;
+        pb = ps.n_seeds - 1 - (int)(k - a * ps.nneg);
+    }
+    ia = ps.list[pa];
+    ib = ps.list[pb];
+    if (ps.sh) {
+        ta = ps.sh->get(pa);
+        tb = ps.sh->get(pb);
+    } else {
+        ta = make_track(c, t, ia);
+        tb = make_track(c, t, ib);
+    }
+}
+
+// Exclusive offsets of this thread's two flags inside the block (thread order) and the block totals.
+__device__ __forceinline__ void block_ordered_offsets(bool f0, bool f1, int (*warp_cnt)[2], int &off0, int &off1,
+                                                      int &tot0, int &tot1)
+{
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const unsigned m0 = __ballot_sync(0xffffffffu, f0), m1 = __ballot_sync(0xffffffffu, f1);
+    if (lane == 0) { warp_cnt[wid][0] = __popc(m0); warp_cnt[wid][1] = __popc(m1); }
+    __syncthreads();
+    int b0 = 0, b1 = 0, t0 = 0, t1 = 0;
+#pragma unroll
+    for (int w = 0; w < kVtxWarps; ++w) {
+        const int c0 = warp_cnt[w][0], c1 = warp_cnt[w][1];
+        if (w < wid) { b0 += c0; b1 += c1; }
+        t0 += c0; t1 += c1;
+    }
+    __syncthreads();
+    tot0 = t0; tot1 = t1;
+    off0 = b0 + __popc(m0 & lanemask_lt());
+    off1 = b1 + __popc(m1 & lanemask_lt());
 }
 
 __global__ void __launch_bounds__(kVtxThreads)
 k_vertex_count(const __grid_constant__ DevConst c, const ds_tracks trk, const int32_t *__restrict__ seed_offsets,
                PairLists pl, int32_t *__restrict__ n_per_event)
 {
-    __shared__ int warp_cnt[kVtxWarps];
+    __shared__ VtxShared sh;
+    __shared__ int warp_cnt[kVtxWarps][2];
     __shared__ int red[kVtxWarps];
     const int e = blockIdx.x, tid = threadIdx.x;
     const int s0 = seed_offsets[e], s1 = seed_offsets[e + 1];
-    // pass 1: positive tracks to the front of the event's list slice, in seed order
+    const int n_seeds = s1 - s0;
+    const bool staged = n_seeds <= kVtxCap;
+    int32_t *list = pl.list + s0;
+    // S8: kept tracks, positive to the front and negative to the back of the event's list slice, both in seed order
     int npos = 0, nneg = 0;
-    for (int sign = 0; sign < 2; ++sign) {
-        int base = sign == 0 ? s0 : s0 + npos, cnt = 0;
-        for (int chunk = s0; chunk < s1; chunk += kVtxThreads) {
-            const int s = chunk + tid;
-            bool f = false;
-            if (s < s1 && trk.keep[s]) {
-                const float q = trk.qop[s];
-                f = sign == 0 ? q > 0.f : q < 0.f;
-            }
-            int tot;
-            const int off = block_ordered_offset(f, warp_cnt, tot);
-            if (f) pl.list[base + cnt + off] = s;
-            cnt += tot;
+    for (int chunk = s0; chunk < s1; chunk += kVtxThreads) {
+        const int s = chunk + tid;
+        bool fp = false, fn = false;
+        if (s < s1 && trk.keep[s]) {
+            const float q = trk.qop[s];
+            fp = q > 0.f;
+            fn = q < 0.f;
         }
-        if (sign == 0) npos = cnt; else nneg = cnt;
+        int op, on, tp, tn;
+        block_ordered_offsets(fp, fn, warp_cnt, op, on, tp, tn);
+        if (fp | fn) {
+            const int pos = fp ? npos + op : n_seeds - 1 - (nneg + on);
+            list[pos] = s;
+            if (staged) sh.put(pos, make_track(c, trk, s));
+        }
+        npos += tp;
+        nneg += tn;
     }
     if (tid == 0) { pl.npos[e] = npos; pl.nneg[e] = nneg; }
-    __syncthreads();   // list writes of this block are visible to this block
+    __syncthreads();   // list and shared-memory writes of this block are visible to this block
+    // S9: all (positive, negative) pairs, lanes over pairs
+    PairSource ps;
+    ps.sh = staged ? &sh : nullptr; ps.list = list; ps.n_seeds = n_seeds; ps.nneg = nneg;
     const int64_t npairs = (int64_t)npos * nneg;
     int mine = 0;
     for (int64_t k = tid; k < npairs; k += kVtxThreads) {
-        const int a = (int)(k / nneg), b = (int)(k - (int64_t)a * nneg);
-        const int ia = pl.list[s0 + a], ib = pl.list[s0 + npos + b];
-        double xa, ya, txa, tya, qa, xb, yb, txb, tyb, qb;
-        load_pair(trk, ia, ib, xa, ya, txa, tya, qa, xb, yb, txb, tyb, qb);
+        VtxTrack ta, tb;
+        int ia, ib;
+        pair_tracks(c, trk, ps, k, ta, tb, ia, ib);
         VtxOut o;
-        mine += vertex_pair(c, xa, ya, txa, tya, qa, xb, yb, txb, tyb, qb, o) ? 1 : 0;
+        mine += vertex_pair(c, ta, tb, o) ? 1 : 0;
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) mine += __shfl_xor_sync(0xffffffffu, mine, o);
@@ -191,29 +256,39 @@ __global__ void __launch_bounds__(kVtxThreads)
 k_vertex_write(const __grid_constant__ DevConst c, const ds_tracks trk, const int32_t *__restrict__ seed_offsets,
                PairLists pl, const ds_vertices out)
 {
-    __shared__ int warp_cnt[kVtxWarps];
+    __shared__ VtxShared sh;
+    __shared__ int warp_cnt[kVtxWarps][2];
     const int e = blockIdx.x, tid = threadIdx.x;
     const int64_t o0 = out.offsets[e];
     if (out.offsets[e + 1] == o0) return;
-    const int s0 = seed_offsets[e];
+    const int s0 = seed_offsets[e], n_seeds = seed_offsets[e + 1] - s0;
     const int npos = pl.npos[e], nneg = pl.nneg[e];
+    const bool staged = n_seeds <= kVtxCap;
+    const int32_t *list = pl.list + s0;
+    if (staged) {
+        for (int t = tid; t < npos + nneg; t += kVtxThreads) {
+            const int pos = t < npos ? t : n_seeds - 1 - (t - npos);
+            sh.put(pos, make_track(c, trk, list[pos]));
+        }
+        __syncthreads();
+    }
+    PairSource ps;
+    ps.sh = staged ? &sh : nullptr; ps.list = list; ps.n_seeds = n_seeds; ps.nneg = nneg;
     const int64_t npairs = (int64_t)npos * nneg;
     int64_t written = 0;
+    // S9 again, S10: block-ordered compaction of the passing pairs -> (ia, ib) order
     for (int64_t tile = 0; tile < npairs; tile += kVtxThreads) {
         const int64_t k = tile + tid;
         bool pass = false;
         VtxOut o;
         int ia = 0, ib = 0;
         if (k < npairs) {
-            const int a = (int)(k / nneg), b = (int)(k - (int64_t)a * nneg);
-            ia = pl.list[s0 + a];
-            ib = pl.list[s0 + npos + b];
-            double xa, ya, txa, tya, qa, xb, yb, txb, tyb, qb;
-            load_pair(trk, ia, ib, xa, ya, txa, tya, qa, xb, yb, txb, tyb, qb);
-            pass = vertex_pair(c, xa, ya, txa, tya, qa, xb, yb, txb, tyb, qb, o);
+            VtxTrack ta, tb;
+            pair_tracks(c, trk, ps, k, ta, tb, ia, ib);
+            pass = vertex_pair(c, ta, tb, o);
         }
-        int tot;
-        const int off = block_ordered_offset(pass, warp_cnt, tot);
+        int off, off1, tot, tot1;
+        block_ordered_offsets(pass, false, warp_cnt, off, off1, tot, tot1);
         const int64_t pos = o0 + written + off;
         if (pass && pos < out.capacity) {
             out.evt[pos] = e; out.ia[pos] = ia; out.ib[pos] = ib; out.flags[pos] = o.flags;
