@@ -80,7 +80,8 @@ __device__ __forceinline__ void sector_range(const DevConst &c, double y, int &s
 }
 
 // Positions [a, b) (relative to the event) of the x0 slices of (layer, sector) that the x0 interval [lo, hi] touches.
-__device__ __forceinline__ void slice_range(const DevConst &c, const int *tab, int layer, int sector, double lo,
+template <typename Tab>
+__device__ __forceinline__ void slice_range(const DevConst &c, const Tab *tab, int layer, int sector, double lo,
                                             double hi, int &a, int &b)
 {
     const int base = (layer * c.n_sectors + sector) * kXBins;
@@ -103,11 +104,19 @@ struct FitRes {
 // State of one warp of k_track: the warp takes up to 32 seeds of the event through all phases on its own.  Idx is the
 // type hit positions inside the event are stored in: uint16_t when the event is staged (it then has < 65535 hits),
 // int otherwise.  (Idx)-1 = none.
+// What the later phases need of a seed (S2, computed once in phase A): magnet point, y at the four planes, refined
+// window half-width, and the y-sector range of the refined window in UTaX, UTaU, UTbV (lo > hi: none).
+struct SeedRec {
+    double xm, zm, w1, y[4];
+    unsigned char sec[3][2];
+    unsigned char pad_[2];
+};
+
 template <typename Idx>
 struct WarpShared {
     FitRes res[kFitCap];                  // fit phase: result of fit task i
+    SeedRec rec[32];
     float2 zw3[kFirstCap];                // (z, w) of the first hit
-    float sx[32], sy[32], stx[32], sty[32], sqop[32];
     int n_fit;                            // fit tasks appended this round (may exceed kFitCap)
     int fit_end;                          // tasks [0, fit_end) are queued; later appends did not fit the queue
     Idx slot[32 * kMaxFirst];             // phase A: the seed's first hits (positions in the event's sorted slice)
@@ -122,8 +131,8 @@ struct WarpShared {
 template <typename Idx>
 struct TrackShared {
     unsigned long long bar;
-    int tab[kMaxBins + 1];                // the event's bin table
     WarpShared<Idx> warp[kTrackWarps];
+    Idx tab[kMaxBins + 1];                // the event's bin table
 };
 static_assert(kFirstCap <= 512 && kFitCap < 0xfff, "packing of task[] and ffit[]");
 
@@ -167,22 +176,33 @@ __device__ __forceinline__ Prefilter make_prefilter(double target_x0, double w)
     return p;
 }
 
-// S4: closest and second closest y-compatible hit of layer l within w1 of the prediction xp; -1 = none
-__device__ __forceinline__ int2 search_layer(const DevConst &c, const EventHits &H, const int *tab, int l, double xp,
-                                             double y, double w1)
+// First position in [a, b) of the x0-sorted slice whose x0 is not below xl
+__device__ __forceinline__ int lower_bound_x0(const float *x0, int a, int b, float xl)
+{
+    while (a < b) {
+        const int mid = (a + b) >> 1;
+        if (x0[mid] < xl) a = mid + 1; else b = mid;
+    }
+    return a;
+}
+
+// S4: closest and second closest y-compatible hit of layer l (sectors tl..th) within w1 of the prediction xp;
+// -1 = none.  Inside a sector the hits are x0-sorted: binary search to the lower edge of the (fp32, widened) window,
+// then only the hits inside it are looked at in fp64.
+template <typename Tab>
+__device__ __forceinline__ int2 search_layer(const DevConst &c, const EventHits &H, const Tab *tab, int l, double xp,
+                                             double y, double w1, int tl, int th)
 {
     int j0 = -1, j1 = -1;
     double d0 = 1e300, d1 = 1e300;
     const double off = c.dxdy[l] * y;
     const double lo = xp - off - w1, hi = xp - off + w1;
     const Prefilter pf = make_prefilter(xp - off, w1);
-    int tl, th;
-    sector_range(c, y, tl, th);
+    const float xl = pf.t - pf.w, xh = pf.t + pf.w;
     for (int sec = tl; sec <= th; ++sec) {
         int a, b;
         slice_range(c, tab, l, sec, lo, hi, a, b);
-        for (int j = a; j < b; ++j) {
-            if (!(fabsf(H.x0[j] - pf.t) <= pf.w)) continue;
+        for (int j = lower_bound_x0(H.x0, a, b, xl); j < b && H.x0[j] <= xh; ++j) {
             const double d = fabs(((double)H.x0[j] + off) - xp);
             const bool pass = (d <= w1) & y_compatible(c, H, j, y);
             if (pass) {
@@ -203,7 +223,7 @@ __device__ __forceinline__ int2 search_layer(const DevConst &c, const EventHits 
 // outwards from the window centre, one left and one right head per sector, always taking the closest head.  Returns
 // false (dst not valid) when it meets equal x0 on a left side, where the walk order is not the id order.
 template <typename Idx>
-__device__ __noinline__ bool select_first_walk(const DevConst &c, const EventHits &H, const int *tab, int s_lo, int s_hi,
+__device__ __noinline__ bool select_first_walk(const DevConst &c, const EventHits &H, const Idx *tab, int s_lo, int s_hi,
                                                double off3, double xc, double w0, double y, int max_first, Idx *dst)
 {
     int hj[4], hend[4];
@@ -276,7 +296,7 @@ __device__ __noinline__ bool tie_better(const EventHits &H, const Candidate &p, 
 
 // S5: weighted straight line x(z - z_ref) through the first hit (z3, w3 given), the refined-window hits j0, j1, j2
 // (-1 = missing) and the magnet point as pseudo-measurement (A-8); chi2; chi2/ndf cut and score (A-9)
-__device__ __forceinline__ FitRes fit_combo(const DevConst &c, const EventHits &H, const S2 &s2, int j0, int j1, int j2,
+__device__ __forceinline__ FitRes fit_combo(const DevConst &c, const EventHits &H, const SeedRec &s2, int j0, int j1, int j2,
                                             int j3, double z3, double w3)
 {
     // all loads first (z, w come from global memory)
@@ -287,8 +307,8 @@ __device__ __forceinline__ FitRes fit_combo(const DevConst &c, const EventHits &
     const int nh = 1 + u0 + u1 + u2;
     const double pz[5] = {u0 ? (double)fz0 - c.z_ref : 0.0, u1 ? (double)fz1 - c.z_ref : 0.0,
                           u2 ? (double)fz2 - c.z_ref : 0.0, z3 - c.z_ref, s2.zm - c.z_ref};
-    const double px[5] = {u0 ? (double)fx0 + c.dxdy[0] * s2.y0 : 0.0, u1 ? (double)fx1 + c.dxdy[1] * s2.y1 : 0.0,
-                          u2 ? (double)fx2 + c.dxdy[2] * s2.y2 : 0.0, (double)fx3 + c.dxdy[3] * s2.y3, s2.xm};
+    const double px[5] = {u0 ? (double)fx0 + c.dxdy[0] * s2.y[0] : 0.0, u1 ? (double)fx1 + c.dxdy[1] * s2.y[1] : 0.0,
+                          u2 ? (double)fx2 + c.dxdy[2] * s2.y[2] : 0.0, (double)fx3 + c.dxdy[3] * s2.y[3], s2.xm};
     const double pw[5] = {u0 ? (double)fw0 : 0.0, u1 ? (double)fw1 : 0.0, u2 ? (double)fw2 : 0.0, w3, c.w_mag};
     double S = 0, Sz = 0, Szz = 0, Sx = 0, Sxz = 0;
 #pragma unroll
@@ -331,7 +351,7 @@ __device__ __noinline__ Candidate choose_general(const DevConst &c, const WarpSh
     Candidate best;
     best.score = kNoScore; best.a = 0.0; best.b = 0.0; best.chi2 = 0.0;
     best.nh = 0; best.j0 = -1; best.j1 = -1; best.j2 = -1; best.j3 = -1;
-    const S2 s2 = extrapolate_seed(c, sh.sx[o], sh.sy[o], sh.stx[o], sh.sty[o], sh.sqop[o]);
+    const SeedRec &s2 = sh.rec[o];
     for (int k = 0; k < nF; ++k) {
         const int f = f0 + k;
         const unsigned short ff = sh.ffit[f];
@@ -364,7 +384,7 @@ __device__ __noinline__ Candidate choose_general(const DevConst &c, const WarpSh
 //   C  lane per seed:       best candidate (S6), track record
 // A round takes the longest prefix of the remaining seeds whose first hits fit the warp's list.
 template <typename Idx>
-__device__ __forceinline__ void track_chunk(const DevConst &c, WarpShared<Idx> &sh, const int *tab, const EventHits &H,
+__device__ __forceinline__ void track_chunk(const DevConst &c, WarpShared<Idx> &sh, const Idx *tab, const EventHits &H,
                                             const ds_seeds &seeds, int cb, int ce, const ds_tracks &out)
 {
     const unsigned FULL = 0xffffffffu;
@@ -377,21 +397,34 @@ __device__ __forceinline__ void track_chunk(const DevConst &c, WarpShared<Idx> &
         const int s = s_base + lane;
         const bool act = s < ce;
         int nF = 0;
+        float fy = 0.f, ftx = 0.f, fty = 0.f;   // kept for the track record (phase C)
         if (lane == 0) { sh.n_fit = 0; sh.fit_end = kFitCap; }
         if (act) {
-            const float fx = seeds.x[s], fy = seeds.y[s], ftx = seeds.tx[s], fty = seeds.ty[s], fq = seeds.qop[s];
-            sh.sx[lane] = fx; sh.sy[lane] = fy; sh.stx[lane] = ftx; sh.sty[lane] = fty; sh.sqop[lane] = fq;
+            const float fx = seeds.x[s], fq = seeds.qop[s];
+            fy = seeds.y[s]; ftx = seeds.tx[s]; fty = seeds.ty[s];
             const S2 s2 = extrapolate_seed(c, fx, fy, ftx, fty, fq);
+            {
+                SeedRec &r = sh.rec[lane];
+                r.xm = s2.xm; r.zm = s2.zm; r.w1 = s2.w1;
+                r.y[0] = s2.y0; r.y[1] = s2.y1; r.y[2] = s2.y2; r.y[3] = s2.y3;
+#pragma unroll
+                for (int l = 0; l < 3; ++l) {
+                    int tl, th;
+                    sector_range(c, l == 0 ? s2.y0 : (l == 1 ? s2.y1 : s2.y2), tl, th);
+                    r.sec[l][0] = (unsigned char)(th < tl ? 1 : tl);
+                    r.sec[l][1] = (unsigned char)(th < tl ? 0 : th);
+                }
+            }
             int s_lo, s_hi;
             sector_range(c, s2.y3, s_lo, s_hi);
             const double off3 = c.dxdy[3] * s2.y3;
             const double lo3 = s2.xc3 - off3 - s2.w0, hi3 = s2.xc3 - off3 + s2.w0;
             const Prefilter pf = make_prefilter(s2.xc3 - off3, s2.w0);
+            const float xl = pf.t - pf.w, xh = pf.t + pf.w;
             for (int sec = s_lo; sec <= s_hi; ++sec) {
                 int a, b;
                 slice_range(c, tab, 3, sec, lo3, hi3, a, b);
-                for (int j = a; j < b; ++j) {
-                    if (!(fabsf(H.x0[j] - pf.t) <= pf.w)) continue;
+                for (int j = lower_bound_x0(H.x0, a, b, xl); j < b && H.x0[j] <= xh; ++j) {
                     const double d = fabs(((double)H.x0[j] + off3) - s2.xc3);
                     if ((d <= s2.w0) & y_compatible(c, H, j, s2.y3)) {
                         if (nF < max_first) my_slot[nF] = (Idx)j;
@@ -460,13 +493,12 @@ __device__ __forceinline__ void track_chunk(const DevConst &c, WarpShared<Idx> &
             if (on) {
                 const int sl = sh.fs[f], o = sl / kMaxFirst;
                 const int j3 = (int)sh.slot[sl];
-                const S2 t2 = extrapolate_seed(c, sh.sx[o], sh.sy[o], sh.stx[o], sh.sty[o], sh.sqop[o]);
+                const SeedRec &t2 = sh.rec[o];
                 // trajectory through (first hit, magnet point), refined window in layer l
-                const double x3 = (double)H.x0[j3] + c.dxdy[3] * t2.y3;
+                const double x3 = (double)H.x0[j3] + c.dxdy[3] * t2.y[3];
                 const double txc = (x3 - t2.xm) / ((double)sh.zw3[f].x - t2.zm);
                 const double xp = t2.xm + txc * (c.z_layer[l] - t2.zm);
-                const double y = l == 0 ? t2.y0 : (l == 1 ? t2.y1 : t2.y2);
-                r = search_layer(c, H, tab, l, xp, y, t2.w1);
+                r = search_layer(c, H, tab, l, xp, t2.y[l], t2.w1, (int)t2.sec[l][0], (int)t2.sec[l][1]);
                 if (l == 0) r.y = -1;   // UTaX keeps the closest hit only
                 sh.near[3 * f + l][0] = (Idx)r.x;
                 sh.near[3 * f + l][1] = (Idx)r.y;
@@ -498,9 +530,8 @@ __device__ __forceinline__ void track_chunk(const DevConst &c, WarpShared<Idx> &
         if (lane < n_fit) {
             const int tk = sh.task[lane], f = tk & 511, i1 = (tk >> 9) & 1, i2 = (tk >> 10) & 1;
             const int sl = sh.fs[f], o = sl / kMaxFirst;
-            const S2 t2 = extrapolate_seed(c, sh.sx[o], sh.sy[o], sh.stx[o], sh.sty[o], sh.sqop[o]);
             const float2 zw = sh.zw3[f];
-            sh.res[lane] = fit_combo(c, H, t2, idx_get(sh.near[3 * f][0]), idx_get(sh.near[3 * f + 1][i1]),
+            sh.res[lane] = fit_combo(c, H, sh.rec[o], idx_get(sh.near[3 * f][0]), idx_get(sh.near[3 * f + 1][i1]),
                                      idx_get(sh.near[3 * f + 2][i2]), (int)sh.slot[sl], (double)zw.x, (double)zw.y);
         }
         __syncwarp();
@@ -542,7 +573,7 @@ __device__ __forceinline__ void track_chunk(const DevConst &c, WarpShared<Idx> &
             if (best.score == kNoScore) {
                 write_not_found(out, s);
             } else {
-                const double ys = (double)sh.sy[lane], txs = (double)sh.stx[lane], tys = (double)sh.sty[lane];
+                const double ys = (double)fy, txs = (double)ftx, tys = (double)fty;
                 out.x[s] = (float)best.a;
                 out.y[s] = (float)(ys + tys * (c.z_ref - c.z_seed));
                 out.tx[s] = (float)best.b;
@@ -598,7 +629,6 @@ k_track(const __grid_constant__ DevConst c, const LayoutPtrs L, const ds_seeds s
     const int h0a = h0 & ~3, cnt = ((h1 + 3) & ~3) - h0a;
     const bool staged = cnt <= cap;   // cap < 65535 (see launch_track)
     unsigned long long *bar = reinterpret_cast<unsigned long long *>(smem_raw);   // first member of both layouts
-    int *tab = staged ? reinterpret_cast<Staged *>(smem_raw)->tab : reinterpret_cast<Direct *>(smem_raw)->tab;
     if (tid == 0 && staged) {
         mbar_init(bar, 1);
         const uint32_t bytes = 4u * (uint32_t)cnt;
@@ -611,7 +641,13 @@ k_track(const __grid_constant__ DevConst c, const LayoutPtrs L, const ds_seeds s
     }
     const int nb = c.n_bins;
     const int32_t *gtab = L.bin_offsets + (size_t)e * (nb + 1);
-    for (int b = tid; b <= nb; b += kTrackThreads) tab[b] = gtab[b];
+    if (staged) {
+        uint16_t *tab = reinterpret_cast<Staged *>(smem_raw)->tab;
+        for (int b = tid; b <= nb; b += kTrackThreads) tab[b] = (uint16_t)gtab[b];
+    } else {
+        int *tab = reinterpret_cast<Direct *>(smem_raw)->tab;
+        for (int b = tid; b <= nb; b += kTrackThreads) tab[b] = gtab[b];
+    }
     __syncthreads();
 
     EventHits H;

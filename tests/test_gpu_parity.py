@@ -111,6 +111,30 @@ def test_layout_equals_lexsort(ds, cfg, n_events, hint):
         assert ((xs >= lo - 1e-3) | (xb == 0)).all() and ((xs <= hi + 1e-3) | (xb == 15)).all()
 
 
+def test_layout_inputs_not_16_byte_aligned(ds, torch):
+    """Input arrays that start 4 bytes off a 16-byte boundary: k_layout stages them with ordinary loads instead of bulk
+    copies and must give the same permutation; ds_reconstruct on the same views must equal the aligned run."""
+    d = gen.generate(1, n_events=16)
+    n = len(d["hits"]["id"])
+    dev = ds.device
+    hits_al = ds.to_device(d["hits"])
+    hits_un = {}
+    for k, v in d["hits"].items():
+        buf = torch.empty(n + 1, dtype=hits_al[k].dtype, device=dev)
+        buf[1:].copy_(hits_al[k])
+        hits_un[k] = buf[1:]
+        assert hits_un[k].data_ptr() % 16 == 4
+    ho = ds.to_device(dict(h=d["hit_offsets"]))["h"]
+    a, b = to_host(ds.layout(hits_al, ho)), to_host(ds.layout(hits_un, ho))
+    for k in ("perm", "x0", "z", "ymin", "ymax", "w", "id", "bin_offsets"):
+        assert np.array_equal(a[k], b[k]), k
+    seeds = ds.to_device(d["seeds"])
+    so = ds.to_device(dict(s=d["seed_offsets"]))["s"]
+    ta, tb = to_host(ds.reconstruct(hits_al, seeds, ho, so)), to_host(ds.reconstruct(hits_un, seeds, ho, so))
+    for k in ta:
+        assert np.array_equal(ta[k], tb[k]), k
+
+
 # ---- S2 extrapolation ----------------------------------------------------------------------------------------------
 def test_extrapolate_equals_oracle(ds):
     d = gen.generate(1, n_events=4)
