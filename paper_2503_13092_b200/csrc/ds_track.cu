@@ -125,6 +125,9 @@ struct WarpShared {
     unsigned short fs[kFirstCap];         // first-hit list: index into slot[]
     unsigned short ffit[kFirstCap];       // first fit task of the first hit (| combinations << 12), kFitNone or kFitInline
     unsigned short task[kFitCap];         // fit task: first hit | i1 << 9 | i2 << 10
+    unsigned long long best_bits[32];     // per seed: smallest score among its fits (bits of the non-negative double)
+    int best_fit[32];                     // per seed: first fit task with that score
+    int n_best[32];                       // per seed: fits with that score (+ 2 for every first hit left to the seed's thread)
 };
 
 // Block-shared state of k_track (carved from dynamic shared memory, followed by the staged hit arrays).
@@ -399,6 +402,9 @@ __device__ __forceinline__ void track_chunk(const DevConst &c, WarpShared<Idx> &
         int nF = 0;
         float fy = 0.f, ftx = 0.f, fty = 0.f;   // kept for the track record (phase C)
         if (lane == 0) { sh.n_fit = 0; sh.fit_end = kFitCap; }
+        sh.best_bits[lane] = (unsigned long long)__double_as_longlong(kNoScore);
+        sh.best_fit[lane] = INT32_MAX;
+        sh.n_best[lane] = 0;
         if (act) {
             const float fx = seeds.x[s], fq = seeds.qop[s];
             fy = seeds.y[s]; ftx = seeds.tx[s]; fty = seeds.ty[s];
@@ -477,10 +483,20 @@ __device__ __forceinline__ void track_chunk(const DevConst &c, WarpShared<Idx> &
         if (take) {
             const int pos = incl - nFc;
             sh.foff[lane] = (unsigned short)pos;
-            for (int k = 0; k < nFc; ++k) {
-                const int j = (int)my_slot[k];
-                sh.fs[pos + k] = (unsigned short)(lane * kMaxFirst + k);
-                sh.zw3[pos + k] = make_float2(H.z[j], H.w[j]);
+            for (int k0 = 0; k0 < nFc; k0 += 5) {   // (z, w) of the first hits: five loads in flight at a time
+                float2 v[5];
+#pragma unroll
+                for (int u = 0; u < 5; ++u) {
+                    const int j = (int)my_slot[min(k0 + u, nFc - 1)];
+                    v[u] = make_float2(H.z[j], H.w[j]);
+                }
+#pragma unroll
+                for (int u = 0; u < 5; ++u) {
+                    if (k0 + u < nFc) {
+                        sh.fs[pos + k0 + u] = (unsigned short)(lane * kMaxFirst + k0 + u);
+                        sh.zw3[pos + k0 + u] = v[u];
+                    }
+                }
             }
         }
         __syncwarp();
@@ -519,50 +535,53 @@ __device__ __forceinline__ void track_chunk(const DevConst &c, WarpShared<Idx> &
                     } else {
                         ff = kFitInline;
                         atomicMin(&sh.fit_end, base);
+                        atomicAdd(&sh.n_best[sh.fs[f] / kMaxFirst], 2);
                     }
                 }
                 sh.ffit[f] = ff;
             }
         }
         __syncwarp();
-        // ---- fit phase: lane per queued combination -- S5 ----------------------------------------------------------------
+        // ---- fit phase: lane per queued combination -- S5; per seed the smallest score, its first fit and how many share it
         const int n_fit = min(sh.n_fit, sh.fit_end);
-        if (lane < n_fit) {
-            const int tk = sh.task[lane], f = tk & 511, i1 = (tk >> 9) & 1, i2 = (tk >> 10) & 1;
-            const int sl = sh.fs[f], o = sl / kMaxFirst;
-            const float2 zw = sh.zw3[f];
-            sh.res[lane] = fit_combo(c, H, sh.rec[o], idx_get(sh.near[3 * f][0]), idx_get(sh.near[3 * f + 1][i1]),
-                                     idx_get(sh.near[3 * f + 2][i2]), (int)sh.slot[sl], (double)zw.x, (double)zw.y);
+        {
+            unsigned long long bits = (unsigned long long)__double_as_longlong(kNoScore);
+            int o = 0;
+            if (lane < n_fit) {
+                const int tk = sh.task[lane], f = tk & 511, i1 = (tk >> 9) & 1, i2 = (tk >> 10) & 1;
+                const int sl = sh.fs[f];
+                o = sl / kMaxFirst;
+                const float2 zw = sh.zw3[f];
+                const FitRes r = fit_combo(c, H, sh.rec[o], idx_get(sh.near[3 * f][0]), idx_get(sh.near[3 * f + 1][i1]),
+                                           idx_get(sh.near[3 * f + 2][i2]), (int)sh.slot[sl], (double)zw.x, (double)zw.y);
+                sh.res[lane] = r;
+                if (r.score != kNoScore) {
+                    bits = (unsigned long long)__double_as_longlong(r.score);   // scores are >= +0: bit order = value order
+                    atomicMin(&sh.best_bits[o], bits);
+                }
+            }
+            __syncwarp();
+            if (lane < n_fit && bits != (unsigned long long)__double_as_longlong(kNoScore) && bits == sh.best_bits[o]) {
+                atomicMin(&sh.best_fit[o], lane);
+                atomicAdd(&sh.n_best[o], 1);
+            }
         }
         __syncwarp();
         // ---- phase C: lane per seed -- S6 and the track record -----------------------------------------------------------
         if (take) {
             const int f0 = sh.foff[lane];
-            // best score over the fit results of the seed's first hits; exact ties and fits that were not queued go
-            // through the general comparison
-            double bscore = kNoScore;
-            int bf = -1, bq = 0;
-            bool general = false;
-            for (int k = 0; k < nFc; ++k) {
-                const unsigned short ff = sh.ffit[f0 + k];
-                if (ff == kFitNone) continue;
-                if (ff == kFitInline) { general = true; continue; }
-                const int base = ff & 0xfff, m = ff >> 12;
-                for (int q = 0; q < m; ++q) {
-                    const double sc = sh.res[base + q].score;
-                    if (sc < bscore) { bscore = sc; bf = f0 + k; bq = q; }
-                    else if (sc == bscore && sc != kNoScore) general = true;
-                }
-            }
+            // one fit with the smallest score: that is the track; exact ties and fits that were not queued go through the
+            // general comparison
+            const int nb = sh.n_best[lane];
+            const bool general = nb >= 2;
+            const int bt = nb == 1 ? sh.best_fit[lane] : -1;
             Candidate best;
             best.score = kNoScore;
             if (general) {
                 best = choose_general<Idx>(c, sh, H, f0, nFc, lane);
-            } else if (bf >= 0) {
-                const int base = sh.ffit[bf] & 0xfff;
-                const FitRes r = sh.res[base + bq];
-                const int m2 = sh.near[3 * bf + 2][1] != (Idx)-1 ? 2 : 1;
-                const int i1 = bq / m2, i2 = bq - i1 * m2;
+            } else if (bt >= 0) {
+                const FitRes r = sh.res[bt];
+                const int tk = sh.task[bt], bf = tk & 511, i1 = (tk >> 9) & 1, i2 = (tk >> 10) & 1;
                 best.score = r.score; best.a = r.a; best.b = r.b; best.chi2 = r.chi2;
                 best.j0 = idx_get(sh.near[3 * bf][0]);
                 best.j1 = idx_get(sh.near[3 * bf + 1][i1]);
@@ -643,7 +662,13 @@ k_track(const __grid_constant__ DevConst c, const LayoutPtrs L, const ds_seeds s
     const int32_t *gtab = L.bin_offsets + (size_t)e * (nb + 1);
     if (staged) {
         uint16_t *tab = reinterpret_cast<Staged *>(smem_raw)->tab;
-        for (int b = tid; b <= nb; b += kTrackThreads) tab[b] = (uint16_t)gtab[b];
+        constexpr int kPer = (kMaxBins + kTrackThreads) / kTrackThreads;
+        int v[kPer];
+#pragma unroll
+        for (int u = 0; u < kPer; ++u) v[u] = gtab[min(tid + u * kTrackThreads, nb)];
+#pragma unroll
+        for (int u = 0; u < kPer; ++u)
+            if (tid + u * kTrackThreads <= nb) tab[tid + u * kTrackThreads] = (uint16_t)v[u];
     } else {
         int *tab = reinterpret_cast<Direct *>(smem_raw)->tab;
         for (int b = tid; b <= nb; b += kTrackThreads) tab[b] = gtab[b];
