@@ -20,11 +20,16 @@ namespace ds {
 
 constexpr int kLayoutThreads = 512;
 constexpr int kMaxBins = 4 * DS_MAX_SECTORS * kXBins;
+constexpr int kSub = 4;   // the sort cuts every x0 slice of the bin table into kSub sub-slices (a power of two)
 
+// Sort bin of a hit: (layer, sector, x0 sub-slice).  t = (x0 + off) * scale is the same fp32 value xbin() floors, and
+// 4t is exact, so floor(floor(kSub * t) / kSub) = floor(t): sub-slice s lies in table slice s / kSub, clamps included.
 __device__ __forceinline__ int fine_bin(const DevConst &c, int id, float x0)
 {
     int sec = min(id_sector(id), c.n_sectors - 1);
-    return (id_layer(id) * c.n_sectors + sec) * kXBins + xbin(x0, c.xb_off, c.xb_scale);
+    float t = floorf((x0 + c.xb_off) * c.xb_scale * (float)kSub);
+    t = fminf(fmaxf(t, 0.0f), (float)(kXBins * kSub - 1));
+    return (id_layer(id) * c.n_sectors + sec) * (kXBins * kSub) + (int)t;
 }
 
 // exclusive scan of v[0..n) in place (n <= a few thousand), v[n] = total.  All threads of the block call it.
@@ -95,14 +100,14 @@ k_layout(const __grid_constant__ DevConst c, const LayoutPtrs p, const int32_t *
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ int warp_sums[33];
     __shared__ __align__(8) unsigned long long bars[3];
-    const int nb = c.n_bins;
+    const int nb = c.n_bins, nfine = nb * kSub;
     // cap is a multiple of 4, so every array starts on a 16-byte boundary
     float *s_x0 = reinterpret_cast<float *>(smem_raw);                 // [cap] x0, later ymin
     int32_t *s_id = reinterpret_cast<int32_t *>(s_x0 + cap);           // [cap] id, later ymax
     uint32_t *s_pk = reinterpret_cast<uint32_t *>(s_id + cap);         // [cap] bin << 20 | slot, later q
     uint32_t *s_buf = s_pk + cap;                                      // [cap] keys in bin order, later z, later w
     uint16_t *s_src = reinterpret_cast<uint16_t *>(s_buf + cap);       // [cap] hits in bin order, later src[q]
-    int *hist = reinterpret_cast<int *>(s_src + cap);                  // [nb + 1]
+    int *hist = reinterpret_cast<int *>(s_src + cap);                  // [nfine + 1]
     unsigned long long *bar_x = &bars[0], *bar_i = &bars[1], *bar_b = &bars[2];
 
     const int e = blockIdx.x;
@@ -117,7 +122,7 @@ k_layout(const __grid_constant__ DevConst c, const LayoutPtrs p, const int32_t *
         mbar_init(bar_i, 1);
         mbar_init(bar_b, 1);
     }
-    for (int b = tid; b <= nb; b += blockDim.x) hist[b] = 0;
+    for (int b = tid; b <= nfine; b += blockDim.x) hist[b] = 0;
     __syncthreads();
 
     if (fast) {
@@ -138,9 +143,9 @@ k_layout(const __grid_constant__ DevConst c, const LayoutPtrs p, const int32_t *
         __syncthreads();
     }
     // B
-    block_exclusive_scan(hist, nb, warp_sums);
+    block_exclusive_scan(hist, nfine, warp_sums);
     int32_t *tab = p.bin_offsets + (size_t)e * (nb + 1);
-    for (int b = tid; b <= nb; b += blockDim.x) tab[b] = hist[b];
+    for (int b = tid; b <= nb; b += blockDim.x) tab[b] = hist[b * kSub];
 
     if (fast) {
         // C
@@ -234,7 +239,7 @@ k_layout(const __grid_constant__ DevConst c, const LayoutPtrs p, const int32_t *
 }
 
 
-static size_t layout_smem_bytes(int cap) { return (size_t)cap * 18 + sizeof(int) * (kMaxBins + 1) + 16; }
+static size_t layout_smem_bytes(int cap, int n_bins) { return (size_t)cap * 18 + sizeof(int) * ((size_t)n_bins * kSub + 1) + 16; }
 
 static int g_layout_smem_set = -1;
 
@@ -246,10 +251,10 @@ cudaError_t launch_layout(const DevConst &c, const LayoutPtrs &p, const int32_t 
     // event are kept as uint16_t
     const int hint = max_event_hits_hint > 0 ? max_event_hits_hint : 4096;
     int cap = ((hint + 3) & ~3) + 8;
-    int cap_max = (int)((227 * 1024 - sizeof(int) * (kMaxBins + 1) - 512) / 18) & ~3;   // 227 KB per CTA
+    int cap_max = (int)((227 * 1024 - sizeof(int) * ((size_t)c.n_bins * kSub + 1) - 512) / 18) & ~3;   // 227 KB per CTA
     if (cap_max > 65532) cap_max = 65532;
     if (cap > cap_max) cap = cap_max;
-    const size_t smem = layout_smem_bytes(cap);
+    const size_t smem = layout_smem_bytes(cap, c.n_bins);
     if ((int)smem > g_layout_smem_set) {
         cudaError_t err = cudaFuncSetAttribute(k_layout, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (err != cudaSuccess) return err;
