@@ -162,10 +162,16 @@ k_layout(const __grid_constant__ DevConst c, const LayoutPtrs p, const int32_t *
             const uint32_t ki = float_key(s_x0[d + i]);
             const int jb = hist[b], je = hist[b + 1];
             int rank = 0, eq = 0;
-            for (int j = jb; j < je; ++j) {
-                const uint32_t km = s_buf[j];
-                rank += km < ki ? 1 : 0;
-                eq += km == ki ? 1 : 0;
+            for (int j = jb; j < je; j += 4) {   // four keys at a time (a sub-slice holds about one)
+                uint32_t km[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) km[u] = s_buf[min(j + u, je - 1)];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const bool in = j + u < je;
+                    rank += (in & (km[u] < ki)) ? 1 : 0;
+                    eq += (in & (km[u] == ki)) ? 1 : 0;
+                }
             }
             if (eq > 1) {   // equal x0 inside the bin: order by (id, original index)
                 const int ii = s_id[d + i];

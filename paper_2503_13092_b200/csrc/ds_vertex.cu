@@ -19,6 +19,7 @@ namespace ds {
 constexpr int kVtxThreads = 128;
 constexpr int kVtxWarps = kVtxThreads / 32;
 constexpr int kVtxCap = 512;   // seeds of an event whose kept tracks are staged in shared memory
+constexpr int kSmallEventSeeds = 256;   // batches with at most this many seeds per event on average: warp per event
 
 struct VtxOut {
     double x, y, z, doca, m_pipi, m_ppi;
@@ -299,42 +300,298 @@ k_vertex_write(const __grid_constant__ DevConst c, const ds_tracks trk, const in
     }
 }
 
+
+// ---- warp-per-event variant (batches of small events: a block per event would leave most of its threads idle) -------
+// k_vertex_count_w  warp per event: charge split by ballots into the event's list, kept tracks with their mass terms
+//                   into the warp's shared memory, lanes over pairs; every lane keeps a bit mask of its passing pairs
+//                   (pair k = 32 * iteration + lane -> bit `iteration`), stored for the write kernel; per-event count
+//                   and the sum of the counts of every group of kGroup events (atomicAdd)
+// k_vertex_write_w  warp per event: offset = counts of the earlier groups + counts of the earlier events of the group;
+//                   only the pairs whose mask bit is set are computed again and written, in pair order
+constexpr int kWThreads = 128;
+constexpr int kWWarps = kWThreads / 32;
+constexpr int kWCap = 96;       // kept tracks of an event staged per warp
+constexpr int kGroup = 256;     // events per group sum
+constexpr int kMaskIters = 64;  // pair iterations covered by the 64-bit lane mask (events above: all pairs again)
+
+struct WarpTracks {
+    float x[kWCap], y[kWCap], tx[kWCap], ty[kWCap];
+    double p[kWCap], k[kWCap], e_pi[kWCap], e_p[kWCap];
+    __device__ __forceinline__ void put(int pos, const VtxTrack &r)
+    {
+        x[pos] = (float)r.x; y[pos] = (float)r.y; tx[pos] = (float)r.tx; ty[pos] = (float)r.ty;   // exact: they were fp32
+        p[pos] = r.p; k[pos] = r.k; e_pi[pos] = r.e_pi; e_p[pos] = r.e_p;
+    }
+    __device__ __forceinline__ VtxTrack get(int pos) const
+    {
+        VtxTrack r;
+        r.x = x[pos]; r.y = y[pos]; r.tx = tx[pos]; r.ty = ty[pos];
+        r.p = p[pos]; r.k = k[pos]; r.e_pi = e_pi[pos]; r.e_p = e_p[pos];
+        return r;
+    }
+};
+
+struct WarpWork {
+    unsigned long long *masks;   // [n_events][32]
+    int32_t *group_sums;         // [ceil(n_events / kGroup)], zeroed before k_vertex_count_w
+};
+
+// pair k of the event -> (a, b) with 32-bit division when it fits
+__device__ __forceinline__ void pair_index(int64_t k, int nneg, int &a, int &b)
+{
+    if (k <= 0xffffffffLL) {
+        const unsigned ua = (unsigned)k / (unsigned)nneg;
+        a = (int)ua;
+        b = (int)((unsigned)k - ua * (unsigned)nneg);
+    } else {
+        const int64_t la = k / nneg;
+        a = (int)la;
+        b = (int)(k - la * nneg);
+    }
+}
+
+__global__ void __launch_bounds__(kWThreads)
+k_vertex_count_w(const __grid_constant__ DevConst c, const ds_tracks trk, const int32_t *__restrict__ seed_offsets,
+                 int n_events, PairLists pl, WarpWork ww, int32_t *__restrict__ n_per_event)
+{
+    __shared__ WarpTracks tracks[kWWarps];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const int e = blockIdx.x * kWWarps + wid;
+    if (e >= n_events) return;
+    const unsigned FULL = 0xffffffffu;
+    WarpTracks &sh = tracks[wid];
+    const int s0 = seed_offsets[e], s1 = seed_offsets[e + 1];
+    const int n_seeds = s1 - s0;
+    int32_t *list = pl.list + s0;
+    // S8: kept tracks, positive to the front and negative to the back of the event's list slice, both in seed order
+    int npos = 0, nneg = 0;
+    for (int chunk0 = s0; chunk0 < s1; chunk0 += 8 * 32) {   // eight chunks of 32 seeds with their loads in flight together
+        int kp[8];
+        float qp[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+            const int s = chunk0 + u * 32 + lane;
+            kp[u] = s < s1 ? trk.keep[s] : 0;
+            qp[u] = s < s1 ? trk.qop[s] : 0.f;
+        }
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+            if (chunk0 + u * 32 >= s1) break;
+            const int s = chunk0 + u * 32 + lane;
+            const bool fp = kp[u] != 0 && qp[u] > 0.f, fn = kp[u] != 0 && qp[u] < 0.f;
+            const unsigned mp = __ballot_sync(FULL, fp), mn = __ballot_sync(FULL, fn);
+            if (fp) list[npos + __popc(mp & lanemask_lt())] = s;
+            if (fn) list[n_seeds - 1 - (nneg + __popc(mn & lanemask_lt()))] = s;
+            npos += __popc(mp);
+            nneg += __popc(mn);
+        }
+    }
+    if (lane == 0) { pl.npos[e] = npos; pl.nneg[e] = nneg; }
+    __syncwarp();   // the list written by this warp is read by this warp
+    const bool staged = npos + nneg <= kWCap;
+    if (staged) {   // positive tracks at [0, npos), negative tracks at [npos, npos + nneg)
+        for (int t = lane; t < npos + nneg; t += 32) sh.put(t, make_track(c, trk, t < npos ? list[t] : list[n_seeds - 1 - (t - npos)]));
+        __syncwarp();
+    }
+    // S9: all (positive, negative) pairs, lanes over pairs
+    const int64_t npairs = (int64_t)npos * nneg;
+    unsigned long long mask = 0ull;
+    int mine = 0, it = 0;
+    for (int64_t k = lane; k < npairs; k += 32, ++it) {
+        int a, b;
+        pair_index(k, nneg, a, b);
+        VtxTrack ta, tb;
+        if (staged) {
+            ta = sh.get(a);
+            tb = sh.get(npos + b);
+        } else {
+            ta = make_track(c, trk, list[a]);
+            tb = make_track(c, trk, list[n_seeds - 1 - b]);
+        }
+        VtxOut o;
+        if (vertex_pair(c, ta, tb, o)) {
+            ++mine;
+            if (it < kMaskIters) mask |= 1ull << it;
+        }
+    }
+    ww.masks[(size_t)e * 32 + lane] = mask;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) mine += __shfl_xor_sync(FULL, mine, o);
+    if (lane == 0) {
+        n_per_event[e] = mine;
+        if (mine) atomicAdd(&ww.group_sums[e / kGroup], mine);
+    }
+}
+
+constexpr int kW2Threads = 256;
+constexpr int kW2Warps = kW2Threads / 32;
+static_assert(kGroup % kW2Warps == 0, "a block of k_vertex_write_w stays inside one group");
+
+__global__ void __launch_bounds__(kW2Threads)
+k_vertex_write_w(const __grid_constant__ DevConst c, const ds_tracks trk, const int32_t *__restrict__ seed_offsets,
+                 int n_events, PairLists pl, WarpWork ww, const ds_vertices out)
+{
+    __shared__ long long warp_part[kW2Warps];
+    __shared__ int cnt[kW2Warps];
+    __shared__ int pairbuf[kW2Warps][32];
+    const unsigned FULL = 0xffffffffu;
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    const int e0 = blockIdx.x * kW2Warps, e = e0 + wid;
+    // S10: vertices of all earlier events = sums of the earlier groups + counts of the earlier events of this group
+    const int g0 = e0 / kGroup;
+    long long part = 0;
+    for (int g = tid; g < g0; g += kW2Threads) part += ww.group_sums[g];
+    for (int i = g0 * kGroup + tid; i < e0; i += kW2Threads) part += out.n_per_event[i];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) part += __shfl_xor_sync(FULL, part, o);
+    if (lane == 0) {
+        warp_part[wid] = part;
+        cnt[wid] = e < n_events ? out.n_per_event[e] : 0;
+    }
+    __syncthreads();
+    if (e >= n_events) return;
+    long long o0 = 0;
+#pragma unroll
+    for (int w = 0; w < kW2Warps; ++w) o0 += warp_part[w] + (w < wid ? cnt[w] : 0);
+    const int mine = cnt[wid];
+    if (lane == 0) {
+        out.offsets[e] = o0;
+        if (e == n_events - 1) {
+            const long long total = o0 + mine;
+            out.offsets[n_events] = total;
+            const long long over = total > out.capacity ? total - out.capacity : 0;
+            out.overflow[0] = (int32_t)(over > 2147483647LL ? 2147483647LL : over);
+        }
+    }
+    if (mine == 0) return;
+    const int s0 = seed_offsets[e], n_seeds = seed_offsets[e + 1] - s0;
+    const int npos = pl.npos[e], nneg = pl.nneg[e];
+    const int32_t *list = pl.list + s0;
+    const unsigned long long mask = ww.masks[(size_t)e * 32 + lane];
+    const int64_t npairs = (int64_t)npos * nneg;
+    const int64_t iters = (npairs + 31) / 32;
+    // S9 again for the pairs that passed, a lane per passing pair: the pair indices are compacted from the masks (32 at a
+    // time, in pair order) so that their tracks are fetched and their vertices computed side by side
+    int *buf = pairbuf[wid];
+    int64_t written = 0;
+    int nbuf = 0;
+    auto flush = [&]() {
+        __syncwarp();
+        if (lane < nbuf) {
+            int a, b;
+            pair_index(buf[lane], nneg, a, b);
+            const int ia = list[a], ib = list[n_seeds - 1 - b];
+            VtxOut o;
+            vertex_pair(c, make_track(c, trk, ia), make_track(c, trk, ib), o);   // passes again: same arithmetic
+            const int64_t pos = o0 + written + lane;
+            if (pos < out.capacity) {
+                out.evt[pos] = e; out.ia[pos] = ia; out.ib[pos] = ib; out.flags[pos] = o.flags;
+                out.x[pos] = (float)o.x; out.y[pos] = (float)o.y; out.z[pos] = (float)o.z; out.doca[pos] = (float)o.doca;
+                out.m_pipi[pos] = (float)o.m_pipi; out.m_ppi[pos] = (float)o.m_ppi;
+            }
+        }
+        written += nbuf;
+        nbuf = 0;
+        __syncwarp();
+    };
+    const int mask_iters = (int)(iters < kMaskIters ? iters : kMaskIters);
+    for (int it = 0; it < mask_iters; ++it) {
+        const bool bit = ((mask >> it) & 1ull) != 0;
+        const unsigned m = __ballot_sync(FULL, bit);
+        if (m == 0) continue;
+        if (nbuf + __popc(m) > 32) flush();
+        if (bit) buf[nbuf + __popc(m & lanemask_lt())] = it * 32 + lane;
+        nbuf += __popc(m);
+    }
+    flush();
+    // pairs beyond the reach of the mask: every one is tried again
+    for (int64_t it = kMaskIters; it < iters; ++it) {
+        const int64_t k = it * 32 + lane;
+        bool pass = false;
+        VtxOut o;
+        int ia = 0, ib = 0;
+        if (k < npairs) {
+            int a, b;
+            pair_index(k, nneg, a, b);
+            ia = list[a];
+            ib = list[n_seeds - 1 - b];
+            pass = vertex_pair(c, make_track(c, trk, ia), make_track(c, trk, ib), o);
+        }
+        const unsigned m = __ballot_sync(FULL, pass);
+        const int64_t pos = o0 + written + __popc(m & lanemask_lt());
+        if (pass && pos < out.capacity) {
+            out.evt[pos] = e; out.ia[pos] = ia; out.ib[pos] = ib; out.flags[pos] = o.flags;
+            out.x[pos] = (float)o.x; out.y[pos] = (float)o.y; out.z[pos] = (float)o.z; out.doca[pos] = (float)o.doca;
+            out.m_pipi[pos] = (float)o.m_pipi; out.m_ppi[pos] = (float)o.m_ppi;
+        }
+        written += __popc(m);
+    }
+}
+
+// Workspace: list [n_seeds], npos [E], nneg [E] (both variants); masks [E][32] and group sums (warp-per-event variant)
+static size_t up256v(size_t v) { return (v + 255) & ~(size_t)255; }
+
 size_t vertex_workspace_bytes(int n_events, int64_t n_seeds)
 {
-    auto up = [](size_t v) { return (v + 255) & ~(size_t)255; };
-    return up(sizeof(int32_t) * (size_t)(n_seeds > 0 ? n_seeds : 1)) + 2 * up(sizeof(int32_t) * (size_t)(n_events > 0 ? n_events : 1));
+    const size_t ne = (size_t)(n_events > 0 ? n_events : 1), ns = (size_t)(n_seeds > 0 ? n_seeds : 1);
+    return up256v(sizeof(int32_t) * ns) + 2 * up256v(sizeof(int32_t) * ne) + up256v(sizeof(unsigned long long) * 32 * ne) +
+           up256v(sizeof(int32_t) * ((ne + kGroup - 1) / kGroup));
 }
 
 cudaError_t launch_vertex(const DevConst &c, const ds_tracks &trk, const int32_t *seed_offsets, int n_events,
                           const ds_vertices &out, void *workspace, cudaStream_t st, Prof &prof)
 {
-    auto up = [](size_t v) { return (v + 255) & ~(size_t)255; };
+    const size_t ne = (size_t)(n_events > 0 ? n_events : 1), ns = (size_t)(trk.n > 0 ? trk.n : 1);
     PairLists pl;
+    WarpWork ww;
     unsigned char *w = static_cast<unsigned char *>(workspace);
     pl.list = reinterpret_cast<int32_t *>(w);
-    w += up(sizeof(int32_t) * (size_t)(trk.n > 0 ? trk.n : 1));
+    w += up256v(sizeof(int32_t) * ns);
     pl.npos = reinterpret_cast<int32_t *>(w);
-    w += up(sizeof(int32_t) * (size_t)(n_events > 0 ? n_events : 1));
+    w += up256v(sizeof(int32_t) * ne);
     pl.nneg = reinterpret_cast<int32_t *>(w);
-    if (n_events > 0) {
-        prof.begin(DS_K_VTX_COUNT, st);
-        k_vertex_count<<<n_events, kVtxThreads, 0, st>>>(c, trk, seed_offsets, pl, out.n_per_event);
+    w += up256v(sizeof(int32_t) * ne);
+    ww.masks = reinterpret_cast<unsigned long long *>(w);
+    w += up256v(sizeof(unsigned long long) * 32 * ne);
+    ww.group_sums = reinterpret_cast<int32_t *>(w);
+    const size_t n_groups = (ne + kGroup - 1) / kGroup;
+    cudaError_t err = cudaSuccess;
+    // batches of small events (the Run-3-like configurations): a warp per event; large events: a block per event
+    const bool small_events = n_events > 0 && trk.n / n_events <= kSmallEventSeeds;
+    if (n_events <= 0) {
+        prof.begin(DS_K_VTX_SCAN, st);
+        k_vertex_scan<<<1, kScanThreads, 0, st>>>(out.n_per_event, n_events, out.offsets, out.capacity, out.overflow);
         prof.end(st);
-        cudaError_t err = cudaGetLastError();
-        if (err != cudaSuccess) return err;
+        return cudaGetLastError();
     }
+    if (small_events) {
+        err = cudaMemsetAsync(ww.group_sums, 0, sizeof(int32_t) * n_groups, st);
+        if (err != cudaSuccess) return err;
+        prof.begin(DS_K_VTX_COUNT, st);
+        k_vertex_count_w<<<(n_events + kWWarps - 1) / kWWarps, kWThreads, 0, st>>>(c, trk, seed_offsets, n_events, pl, ww,
+                                                                                   out.n_per_event);
+        prof.end(st);
+        err = cudaGetLastError();
+        if (err != cudaSuccess) return err;
+        prof.begin(DS_K_VTX_WRITE, st);
+        k_vertex_write_w<<<(n_events + kW2Warps - 1) / kW2Warps, kW2Threads, 0, st>>>(c, trk, seed_offsets, n_events, pl, ww, out);
+        prof.end(st);
+        return cudaGetLastError();
+    }
+    prof.begin(DS_K_VTX_COUNT, st);
+    k_vertex_count<<<n_events, kVtxThreads, 0, st>>>(c, trk, seed_offsets, pl, out.n_per_event);
+    prof.end(st);
+    err = cudaGetLastError();
+    if (err != cudaSuccess) return err;
     prof.begin(DS_K_VTX_SCAN, st);
     k_vertex_scan<<<1, kScanThreads, 0, st>>>(out.n_per_event, n_events, out.offsets, out.capacity, out.overflow);
     prof.end(st);
-    cudaError_t err = cudaGetLastError();
+    err = cudaGetLastError();
     if (err != cudaSuccess) return err;
-    if (n_events > 0) {
-        prof.begin(DS_K_VTX_WRITE, st);
-        k_vertex_write<<<n_events, kVtxThreads, 0, st>>>(c, trk, seed_offsets, pl, out);
-        prof.end(st);
-        err = cudaGetLastError();
-    }
-    return err;
+    prof.begin(DS_K_VTX_WRITE, st);
+    k_vertex_write<<<n_events, kVtxThreads, 0, st>>>(c, trk, seed_offsets, pl, out);
+    prof.end(st);
+    return cudaGetLastError();
 }
 
 }  // namespace ds

@@ -373,6 +373,24 @@ def test_empty_and_ragged_inputs(ds, orc_mlp):
     assert not t0["found"].any() and v0["n"] == 0
 
 
+def test_vertexing_large_events_in_a_small_event_batch(ds, orc_mlp):
+    """A few cfg3 events (~500 seeds, thousands of pairs) among many empty ones: the batch averages few seeds per event
+    and takes the warp-per-event vertex kernels, whose staging capacity and pair mask these events exceed.  The same
+    events alone take the block-per-event kernels; both must give the oracle's list."""
+    d = gen.generate(3, n_events=5)
+    pad = 40
+    ho = np.concatenate([d["hit_offsets"], np.full(pad, d["hit_offsets"][-1], np.int32)])
+    so = np.concatenate([d["seed_offsets"], np.full(pad, d["seed_offsets"][-1], np.int32)])
+    d2 = dict(d, n_events=5 + pad, hit_offsets=ho, seed_offsets=so)
+    assert len(d["seeds"]["x"]) / d2["n_events"] <= 256 < len(d["seeds"]["x"]) / d["n_events"]
+    st2, sv2, t2, v2 = check_both(ds, d2, orc_mlp)
+    st1, sv1, t1, v1 = check_both(ds, d, orc_mlp)
+    assert v1["n"] == v2["n"] and v1["n"] > 0
+    for k in ("evt", "ia", "ib", "flags", "x", "y", "z", "doca", "m_pipi", "m_ppi"):
+        assert np.array_equal(v1[k], v2[k]), k
+    assert np.array_equal(v1["offsets"], v2["offsets"][:6]) and (v2["offsets"][5:] == v2["offsets"][5]).all()
+
+
 def test_duplicate_hits_and_ties(ds, orc_mlp):
     """Every hit duplicated with a different id: equal distances and equal scores everywhere -> id tie-breaks decide."""
     d = gen.generate(1, n_events=20)
