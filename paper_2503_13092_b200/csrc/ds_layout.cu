@@ -247,8 +247,6 @@ k_layout(const __grid_constant__ DevConst c, const LayoutPtrs p, const int32_t *
 
 static size_t layout_smem_bytes(int cap, int n_bins) { return (size_t)cap * 18 + sizeof(int) * ((size_t)n_bins * kSub + 1) + 16; }
 
-static int g_layout_smem_set = -1;
-
 cudaError_t launch_layout(const DevConst &c, const LayoutPtrs &p, const int32_t *hit_offsets, int n_events,
                           int max_event_hits_hint, cudaStream_t st, Prof &prof)
 {
@@ -261,11 +259,10 @@ cudaError_t launch_layout(const DevConst &c, const LayoutPtrs &p, const int32_t 
     if (cap_max > 65532) cap_max = 65532;
     if (cap > cap_max) cap = cap_max;
     const size_t smem = layout_smem_bytes(cap, c.n_bins);
-    if ((int)smem > g_layout_smem_set) {
-        cudaError_t err = cudaFuncSetAttribute(k_layout, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (err != cudaSuccess) return err;
-        g_layout_smem_set = (int)smem;
-    }
+    // opt in to the full 227 KB of dynamic shared memory; per device, cheap and the same value for every caller, so it is
+    // simply set at every launch (handles on several devices and host threads share this code)
+    cudaError_t aerr = cudaFuncSetAttribute(k_layout, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    if (aerr != cudaSuccess) return aerr;
     // the bulk copies need 16-byte aligned sources (offsets inside the arrays are handled by the kernel)
     const uintptr_t bits = reinterpret_cast<uintptr_t>(p.x0) | reinterpret_cast<uintptr_t>(p.z) |
                            reinterpret_cast<uintptr_t>(p.ymin) | reinterpret_cast<uintptr_t>(p.ymax) |

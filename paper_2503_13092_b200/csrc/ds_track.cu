@@ -688,8 +688,6 @@ k_track(const __grid_constant__ DevConst c, const LayoutPtrs L, const ds_seeds s
     }
 }
 
-static int g_track_smem_set = -1;
-
 cudaError_t launch_track(const DevConst &c, const LayoutPtrs &lay, const ds_seeds &seeds, const int32_t *hit_offsets,
                          const int32_t *seed_offsets, int n_events, int max_event_hits_hint, const ds_tracks &out,
                          cudaStream_t st, Prof &prof)
@@ -705,11 +703,10 @@ cudaError_t launch_track(const DevConst &c, const LayoutPtrs &lay, const ds_seed
     if (cap > cap_max) cap = cap_max;
     size_t smem = fixed + (size_t)cap * 12;
     if (smem < sizeof(TrackShared<int>)) smem = sizeof(TrackShared<int>);   // the layout of an event that is not staged
-    if ((int)smem > g_track_smem_set) {
-        cudaError_t err = cudaFuncSetAttribute(k_track, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (err != cudaSuccess) return err;
-        g_track_smem_set = (int)smem;
-    }
+    // opt in to the full 227 KB of dynamic shared memory; per device, cheap and the same value for every caller, so it is
+    // simply set at every launch (handles on several devices and host threads share this code)
+    cudaError_t aerr = cudaFuncSetAttribute(k_track, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    if (aerr != cudaSuccess) return aerr;
     prof.begin(DS_K_TRACK, st);
     k_track<<<n_events, kTrackThreads, smem, st>>>(c, lay, seeds, hit_offsets, seed_offsets, out, cap);
     prof.end(st);
