@@ -35,6 +35,9 @@ PARAMS = dict(
     m_pi=139.57, m_p=938.27, m_ks=497.6, m_lambda=1115.68,
     dm_ks=50.0, dm_lambda=20.0,
     n2_min=1e-12,                            # A-14
+    # curved-track vertexing (P:255-P:269): gamma = -MP (c0 + c1 q/p[1/MeV]) (Eq. 3); the synthetic
+    # configurations have no field upstream of the UT, so MP = 0 (straight tracks, A-20) is the default
+    magnet_polarity=0.0, gamma_c0=-1.5e-8, gamma_c1=9.3e-3, vtx_newton_iters=3,
 )
 
 # A-10: fixed input normalisation (mu, sigma) for [x, y, tx, ty, qop, chi2, qop_seed, chi2_seed]

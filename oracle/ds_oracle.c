@@ -57,6 +57,10 @@ typedef struct {
     double doca_max, zv_min, zv_max;
     double m_pi, m_p, m_ks, m_lambda, dm_ks, dm_lambda;
     double n2_min;               /* |d_a x d_b|^2 floor                                 (A-14)       */
+    double magnet_polarity;      /* MP of Eq. 3: +1 / -1; 0 = straight tracks (gamma = 0, A-20)      */
+    double gamma_c0, gamma_c1;   /* gamma = -MP (c0 + c1 q/p[1/MeV]); paper: -1.5e-8, 9.3e-3 (Eq. 3, A-27)   */
+    int32_t vtx_newton_iters;    /* Newton-Raphson iterations ("three")           (A-28)              */
+    int32_t pad2_;
     double edge_rel;             /* relative margin below which a decision is "edge" (1e-5)          */
 } orc_params;
 
@@ -184,6 +188,55 @@ int orc_poca(double xa, double ya, double txa, double tya, double xb, double yb,
     out[3] = sqrt(dq[0] * dq[0] + dq[1] * dq[1] + dq[2] * dq[2]);
     out[5] = sa; out[6] = sb; out[7] = 0.0;
     return 1;
+}
+
+/* ------------------------------------------------------------------------------------------------------------
+ * O-S9c  closest approach of two curved trajectories
+ *     Traj_i(z) = ( x_i + tx_i (z - z0) + gamma_i (z - z0)^2,  y_i + ty_i (z - z0),  z )          (Eq. 4)
+ * by Newton-Raphson on F(u, v) = |Traj_a(z0 + u) - Traj_b(z0 + v)|^2: start at the straight-line solution
+ * (orc_poca), then n_iter times (u, v) -= H^-1 grad F with the exact gradient and 2x2 Hessian (A-28).
+ * out[10] = { vx, vy, vz, doca, |n|^2, u, v, |last step|, tx_a at vz, tx_b at vz }.  Returns 0 if the straight
+ * lines are parallel (|n|^2 < n2_min, A-14), else 1.
+ * ------------------------------------------------------------------------------------------------------------ */
+int orc_poca_curved(double xa, double ya, double txa, double tya, double ga, double xb, double yb, double txb,
+                    double tyb, double gb, double z_ref, double n2_min, int n_iter, double *out)
+{
+    double po[8], u, v, step = 0.0, qa[3], qb[3], dq[3];
+    int it, k;
+    if (!orc_poca(xa, ya, txa, tya, xb, yb, txb, tyb, z_ref, n2_min, po)) { out[4] = po[4]; return 0; }
+    u = po[5]; v = po[6];
+    for (it = 0; it < n_iter; ++it) {
+        /* D = Traj_a - Traj_b; dD/du = Da, dD/dv = -Db */
+        double D[3] = { xa + txa * u + ga * u * u - (xb + txb * v + gb * v * v), ya + tya * u - (yb + tyb * v), u - v };
+        double Da[3] = { txa + 2.0 * ga * u, tya, 1.0 }, Db[3] = { txb + 2.0 * gb * v, tyb, 1.0 };
+        /* F/2: gradient and Hessian */
+        double gu = D[0] * Da[0] + D[1] * Da[1] + D[2] * Da[2];
+        double gv = -(D[0] * Db[0] + D[1] * Db[1] + D[2] * Db[2]);
+        double Huu = Da[0] * Da[0] + Da[1] * Da[1] + Da[2] * Da[2] + D[0] * 2.0 * ga;
+        double Hvv = Db[0] * Db[0] + Db[1] * Db[1] + Db[2] * Db[2] - D[0] * 2.0 * gb;
+        double Huv = -(Da[0] * Db[0] + Da[1] * Db[1] + Da[2] * Db[2]);
+        double det = Huu * Hvv - Huv * Huv, du, dv;
+        if (det == 0.0) break;
+        du = -(Hvv * gu - Huv * gv) / det;
+        dv = -(Huu * gv - Huv * gu) / det;
+        u += du; v += dv;
+        step = sqrt(du * du + dv * dv);
+    }
+    qa[0] = xa + txa * u + ga * u * u; qa[1] = ya + tya * u; qa[2] = z_ref + u;
+    qb[0] = xb + txb * v + gb * v * v; qb[1] = yb + tyb * v; qb[2] = z_ref + v;
+    for (k = 0; k < 3; ++k) { out[k] = 0.5 * (qa[k] + qb[k]); dq[k] = qa[k] - qb[k]; }
+    out[3] = sqrt(dq[0] * dq[0] + dq[1] * dq[1] + dq[2] * dq[2]);
+    out[4] = po[4]; out[5] = u; out[6] = v; out[7] = step;
+    /* slope dx/dz of each track at the vertex z (Eq. 2: the slope the masses are computed with) */
+    out[8] = txa + 2.0 * ga * (out[2] - z_ref);
+    out[9] = txb + 2.0 * gb * (out[2] - z_ref);
+    return 1;
+}
+
+/* gamma of Eq. 3; q/p given in 1/GeV, the parametrisation wants 1/MeV (A-27) */
+double orc_gamma(const orc_params *p, double qop_gev)
+{
+    return -p->magnet_polarity * (p->gamma_c0 + p->gamma_c1 * (qop_gev / 1000.0));
 }
 
 /* invariant mass of two tracks with slopes (tx, ty), momenta p [MeV] and mass hypotheses m1, m2 [MeV] */
@@ -430,20 +483,27 @@ static int vertex_pair(const orc_geom *g, const orc_params *p, const double *x, 
                        int *flags, int *edge)
 {
     const double eps = p->edge_rel;
-    double po[8], pa, pb, mpipi, mppi, m_doca, m_z1, m_z2, m_ks, m_l, m_prot, m_n2;
+    double po[10], pa, pb, mpipi, mppi, m_doca, m_z1, m_z2, m_ks, m_l, m_prot, m_n2, txa, txb;
     int a, b, ok, c_doca, c_z1, c_z2, f0, f1, robust_fail, marginal;
     *edge = 0;
     if (!(qop[i] * qop[j] < 0.0)) return 0;                       /* P:279 opposite charges */
     a = qop[i] > 0.0 ? i : j; b = qop[i] > 0.0 ? j : i;
     *ia = a; *ib = b;
-    ok = orc_poca(x[a], y[a], tx[a], ty[a], x[b], y[b], tx[b], ty[b], g->z_ref, p->n2_min, po);
+    txa = tx[a]; txb = tx[b];
+    if (p->magnet_polarity != 0.0) {   /* curved trajectories, Newton-Raphson (N1); slopes at the vertex for the masses */
+        ok = orc_poca_curved(x[a], y[a], tx[a], ty[a], orc_gamma(p, qop[a]), x[b], y[b], tx[b], ty[b],
+                             orc_gamma(p, qop[b]), g->z_ref, p->n2_min, p->vtx_newton_iters, po);
+        if (ok) { txa = po[8]; txb = po[9]; }
+    } else {
+        ok = orc_poca(x[a], y[a], tx[a], ty[a], x[b], y[b], tx[b], ty[b], g->z_ref, p->n2_min, po);
+    }
     m_n2 = relm(po[4], p->n2_min);
     if (!ok) { if (m_n2 < eps) *edge = 1; return 0; }
     pa = 1000.0 / fabs(qop[a]); pb = 1000.0 / fabs(qop[b]);       /* MeV; qop in 1/GeV */
-    mpipi = orc_inv_mass(tx[a], ty[a], pa, p->m_pi, tx[b], ty[b], pb, p->m_pi);
+    mpipi = orc_inv_mass(txa, ty[a], pa, p->m_pi, txb, ty[b], pb, p->m_pi);
     /* proton hypothesis for the track of larger momentum, tie -> the positive one (A-15) */
-    if (pa >= pb) mppi = orc_inv_mass(tx[a], ty[a], pa, p->m_p, tx[b], ty[b], pb, p->m_pi);
-    else          mppi = orc_inv_mass(tx[a], ty[a], pa, p->m_pi, tx[b], ty[b], pb, p->m_p);
+    if (pa >= pb) mppi = orc_inv_mass(txa, ty[a], pa, p->m_p, txb, ty[b], pb, p->m_pi);
+    else          mppi = orc_inv_mass(txa, ty[a], pa, p->m_pi, txb, ty[b], pb, p->m_p);
     m_prot = relm(pa, pb);
     vtx[0] = po[0]; vtx[1] = po[1]; vtx[2] = po[2]; vtx[3] = po[3]; vtx[4] = mpipi; vtx[5] = mppi;
     c_doca = po[3] < p->doca_max;               m_doca = relm(po[3], p->doca_max);

@@ -32,7 +32,8 @@ class OrcParams(ct.Structure):
                 ("pad_", ct.c_int32), ("doca_max", ct.c_double), ("zv_min", ct.c_double), ("zv_max", ct.c_double),
                 ("m_pi", ct.c_double), ("m_p", ct.c_double), ("m_ks", ct.c_double), ("m_lambda", ct.c_double),
                 ("dm_ks", ct.c_double), ("dm_lambda", ct.c_double), ("n2_min", ct.c_double),
-                ("edge_rel", ct.c_double)]
+                ("magnet_polarity", ct.c_double), ("gamma_c0", ct.c_double), ("gamma_c1", ct.c_double),
+                ("vtx_newton_iters", ct.c_int32), ("pad2_", ct.c_int32), ("edge_rel", ct.c_double)]
 
 
 class OrcMlp(ct.Structure):
@@ -50,6 +51,9 @@ def lib():
         _lib.orc_inv_mass.restype = ct.c_double
         _lib.orc_inv_mass.argtypes = [ct.c_double] * 8
         _lib.orc_poca.argtypes = [ct.c_double] * 10 + [c_dp]
+        _lib.orc_poca_curved.argtypes = [ct.c_double] * 12 + [ct.c_int, c_dp]
+        _lib.orc_gamma.restype = ct.c_double
+        _lib.orc_gamma.argtypes = [ct.c_void_p, ct.c_double]
         _lib.orc_extrapolate.argtypes = [ct.c_void_p, ct.c_void_p] + [ct.c_double] * 5 + [c_dp]
         _lib.orc_fit_line.argtypes = [ct.c_int, c_dp, c_dp, c_dp, ct.c_double, c_dp, c_dp, c_dp]
     return _lib
@@ -129,6 +133,20 @@ def poca(xa, ya, txa, tya, xb, yb, txb, tyb, z_ref, n2_min=1e-12):
     out = np.zeros(8)
     ok = lib().orc_poca(xa, ya, txa, tya, xb, yb, txb, tyb, z_ref, n2_min, _p(out))
     return bool(ok), dict(vertex=out[0:3].copy(), doca=out[3], n2=out[4], s_a=out[5], s_b=out[6])
+
+
+def poca_curved(xa, ya, txa, tya, ga, xb, yb, txb, tyb, gb, z_ref, n_iter=3, n2_min=1e-12):
+    """O-S9c: Newton-Raphson closest approach of two parabolic trajectories (Eq. 4)."""
+    out = np.zeros(10)
+    ok = lib().orc_poca_curved(xa, ya, txa, tya, ga, xb, yb, txb, tyb, gb, z_ref, n2_min, n_iter, _p(out))
+    return bool(ok), dict(vertex=out[0:3].copy(), doca=out[3], n2=out[4], u=out[5], v=out[6], last_step=out[7],
+                          tx_a=out[8], tx_b=out[9])
+
+
+def gamma(params: dict, qop_gev: float) -> float:
+    """Eq. 3 with q/p converted from 1/GeV to 1/MeV."""
+    p = make_params(params)
+    return lib().orc_gamma(ct.byref(p), qop_gev)
 
 
 def inv_mass(tx1, ty1, p1, m1, tx2, ty2, p2, m2) -> float:

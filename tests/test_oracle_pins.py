@@ -548,3 +548,125 @@ def test_edge_lists_flag_marginal_decisions(orc_mlp):
     trk["y"][1] = 1.0
     v = O.vertex(trk, [0, 2], G, dict(P, zv_min=-1e9, zv_max=1e9, dm_ks=1e9))
     assert v["n"] == 1 and not v["edge_pairs"] and v["doca"][0] == pytest.approx(1.0)
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# P-11  curved-track vertexing (P:255-P:269, Eq. 3, Eq. 4)
+# ---------------------------------------------------------------------------------------------------------------
+PC = dict(P, magnet_polarity=1.0)
+
+
+def test_p11_gamma_units_and_sign():
+    """Eq. 3 by hand: p = 5 GeV, q = +1, MP = +1: gamma = -(-1.5e-8 + 9.3e-3 * 2e-4 /MeV) = -1.845e-6 /mm; the
+    polarity flips the sign; MP = 0 switches the curvature off (A-20)."""
+    assert O.gamma(PC, 0.2) == pytest.approx(-(-1.5e-8 + 9.3e-3 * 2.0e-4), rel=1e-14)
+    assert O.gamma(dict(PC, magnet_polarity=-1.0), 0.2) == pytest.approx(+(-1.5e-8 + 9.3e-3 * 2.0e-4), rel=1e-14)
+    assert O.gamma(PC, -0.2) == pytest.approx(-(-1.5e-8 - 9.3e-3 * 2.0e-4), rel=1e-14)
+    assert O.gamma(P, 0.2) == 0.0
+    # 1.8 mm of sagitta over 1 m for a 5 GeV track: the scale that fixes q/p in 1/MeV (SURVEY §4)
+    assert abs(O.gamma(PC, 0.2)) * 1000.0 ** 2 == pytest.approx(1.845, rel=1e-12)
+
+
+def test_p11_gamma_zero_is_the_straight_line_solution():
+    rng = np.random.default_rng(11)
+    for _ in range(200):
+        xa, xb = rng.uniform(-500, 500, 2); ya, yb = rng.uniform(-400, 400, 2)
+        txa, txb = rng.uniform(-0.3, 0.3, 2); tya, tyb = rng.uniform(-0.25, 0.25, 2)
+        ok0, s = O.poca(xa, ya, txa, tya, xb, yb, txb, tyb, G["z_ref"])
+        ok1, c = O.poca_curved(xa, ya, txa, tya, 0.0, xb, yb, txb, tyb, 0.0, G["z_ref"], n_iter=3)
+        assert ok0 and ok1
+        assert np.allclose(c["vertex"], s["vertex"], rtol=1e-11, atol=1e-8) and c["doca"] == pytest.approx(s["doca"], rel=1e-9, abs=1e-9)
+        assert c["last_step"] < 1e-6 and c["tx_a"] == txa and c["tx_b"] == txb
+    # parallel lines: no vertex with or without curvature (A-14)
+    assert not O.poca_curved(0, 0, 0.1, 0.0, 1e-6, 5, 1, 0.1, 0.0, -1e-6, G["z_ref"])[0]
+
+
+def test_p11_mirror_parabolas_closed_form():
+    """a: x = x0 + t u + g u^2 (y = 0);  b: its mirror image x -> -x in the plane y = d.  By symmetry the closest
+    approach is at u = v with x = 0: g u^2 + t u + x0 = 0, vertex (0, d/2, z0 + u), DOCA = d, slope t + 2 g u."""
+    for g, t, x0, d in ((-1.8e-6, 0.1, 5.0, 3.0), (2.5e-6, 0.2, -30.0, 0.5), (-9e-6, 0.05, 12.0, 0.0), (1e-7, -0.15, 40.0, 7.0)):
+        u = (-t + np.sign(t) * np.sqrt(t * t - 4 * g * x0)) / (2 * g)      # the root that goes to -x0/t for g -> 0
+        ok, c = O.poca_curved(x0, 0.0, t, 0.0, g, -x0, d, -t, 0.0, -g, G["z_ref"], n_iter=3)
+        assert ok
+        assert c["u"] == pytest.approx(u, rel=1e-9) and c["v"] == pytest.approx(u, rel=1e-9)
+        assert np.allclose(c["vertex"], [0.0, d / 2, G["z_ref"] + u], atol=1e-7)
+        assert c["doca"] == pytest.approx(d, abs=1e-7)
+        assert c["tx_a"] == pytest.approx(t + 2 * g * u, rel=1e-12) and c["tx_b"] == pytest.approx(-(t + 2 * g * u), rel=1e-12)
+        assert c["last_step"] < 1e-4          # mm: "typically three iterations" (P:269)
+
+
+def test_p11_newton_reaches_the_minimum_of_the_distance():
+    """Two parabolas (curvature of Eq. 3 for p = 1.5..40 GeV) drawn through one decay vertex upstream of the UT: the
+    Newton point after three iterations is that vertex with DOCA 0 ("typically three iterations"); with the
+    states smeared, it is the minimum a library minimiser of |Traj_a(z0+u) - Traj_b(z0+v)|^2 finds."""
+    from scipy.optimize import minimize
+    rng = np.random.default_rng(5)
+    z0 = G["z_ref"]
+    for k in range(80):
+        xv, yv, zv = rng.uniform(-150, 150), rng.uniform(-120, 120), rng.uniform(600, 2400)
+        u0 = zv - z0
+        pa, pb = np.exp(rng.uniform(np.log(1.5), np.log(40.0), 2))
+        ga, gb = O.gamma(PC, 1.0 / pa), O.gamma(PC, -1.0 / pb)
+        txa, txb = rng.uniform(-0.25, 0.25, 2); tya, tyb = rng.uniform(-0.2, 0.2, 2)
+        if np.hypot(txa - txb, tya - tyb) < 0.1:                      # opening angles of K_S / Lambda daughters at these momenta;
+            continue                                                  # below ~0.05 three iterations do not suffice
+        sm = 0.0 if k < 40 else 0.3                                   # mm: exact crossing, then smeared states
+        xa = xv - txa * u0 - ga * u0 * u0 + sm * rng.normal(); ya = yv - tya * u0 + sm * rng.normal()
+        xb = xv - txb * u0 - gb * u0 * u0 + sm * rng.normal(); yb = yv - tyb * u0 + sm * rng.normal()
+        ok, c = O.poca_curved(xa, ya, txa, tya, ga, xb, yb, txb, tyb, gb, z0, n_iter=3)
+        assert ok and c["last_step"] < 0.05                           # mm
+
+        def F(w):
+            u, v = w
+            return ((xa + txa * u + ga * u * u - xb - txb * v - gb * v * v) ** 2 + (ya + tya * u - yb - tyb * v) ** 2 + (u - v) ** 2)
+        assert np.sqrt(F([c["u"], c["v"]])) == pytest.approx(c["doca"], rel=1e-9, abs=1e-9)
+        if sm == 0.0:
+            assert np.allclose(c["vertex"], [xv, yv, zv], atol=1e-3) and c["doca"] < 1e-6
+            # one iteration is not enough, which is what separates this from the straight-line formula
+            ok1, c1 = O.poca_curved(xa, ya, txa, tya, ga, xb, yb, txb, tyb, gb, z0, n_iter=0)
+            assert ok1 and (c1["doca"] > 10 * c["doca"] + 1e-6 or abs(ga) + abs(gb) < 1e-7)
+        else:
+            m = minimize(F, x0=[c["u"] + 3.0, c["v"] - 3.0], method="Nelder-Mead", options=dict(xatol=1e-10, fatol=1e-20, maxiter=4000))
+            assert m.fun >= F([c["u"], c["v"]]) - 1e-9                # nothing lower than the Newton point
+            assert np.allclose(m.x, [c["u"], c["v"]], atol=1e-2)
+
+
+def test_p11_pair_list_with_curvature_brute_force(orc_mlp):
+    """The vertex list with MP != 0 equals the double loop over kept opposite-charge tracks written out here with
+    poca_curved, the slopes at the vertex and inv_mass; MP = +1 and -1 differ, MP = 0 is the straight-track list."""
+    d = gen.generate(1, n_events=10)
+    r0 = run(d, orc_mlp)
+    r = {k: (np.asarray(v, dtype=np.float64) if k in ("x", "y", "tx", "ty", "qop") else v) for k, v in r0.items()}   # fp32 values, fp64 arithmetic
+    so = d["seed_offsets"]
+    lists = {}
+    for mp in (1.0, -1.0):
+        pp = dict(P, magnet_polarity=mp, zv_min=-1e9, zv_max=1e9)
+        v = O.vertex(r, so, G, pp)
+        ref = []
+        for e in range(d["n_events"]):
+            idx = [k for k in range(so[e], so[e + 1]) if r["keep"][k]]
+            for a in idx:
+                for b in idx:
+                    if not (r["qop"][a] > 0 and r["qop"][b] < 0):
+                        continue
+                    ok, c = O.poca_curved(r["x"][a], r["y"][a], r["tx"][a], r["ty"][a], O.gamma(pp, r["qop"][a]), r["x"][b],
+                                          r["y"][b], r["tx"][b], r["ty"][b], O.gamma(pp, r["qop"][b]), G["z_ref"],
+                                          n_iter=pp["vtx_newton_iters"], n2_min=pp["n2_min"])
+                    if not ok or not c["doca"] < pp["doca_max"]:
+                        continue
+                    pa, pb = 1000.0 / abs(r["qop"][a]), 1000.0 / abs(r["qop"][b])
+                    m1 = O.inv_mass(c["tx_a"], r["ty"][a], pa, pp["m_pi"], c["tx_b"], r["ty"][b], pb, pp["m_pi"])
+                    m2 = (O.inv_mass(c["tx_a"], r["ty"][a], pa, pp["m_p"], c["tx_b"], r["ty"][b], pb, pp["m_pi"]) if pa >= pb else
+                          O.inv_mass(c["tx_a"], r["ty"][a], pa, pp["m_pi"], c["tx_b"], r["ty"][b], pb, pp["m_p"]))
+                    fl = (1 if abs(m1 - pp["m_ks"]) < pp["dm_ks"] else 0) | (2 if abs(m2 - pp["m_lambda"]) < pp["dm_lambda"] else 0)
+                    if fl:
+                        ref.append((e, a, b, fl, c["vertex"], c["doca"], m1, m2))
+        assert v["n"] == len(ref) and v["n"] > 10
+        assert list(zip(v["evt"], v["ia"], v["ib"], v["flags"])) == [(e, a, b, f) for e, a, b, f, *_ in ref]
+        assert np.allclose(np.stack([v["x"], v["y"], v["z"]], 1), np.stack([x[4] for x in ref]), rtol=1e-12, atol=1e-9)
+        assert np.allclose(v["m_pipi"], [x[6] for x in ref], rtol=1e-12) and np.allclose(v["m_ppi"], [x[7] for x in ref], rtol=1e-12)
+        lists[mp] = v
+    assert not np.allclose(lists[1.0]["z"][:5], lists[-1.0]["z"][:5])
+    v0 = O.vertex(r, so, G, dict(P, zv_min=-1e9, zv_max=1e9))
+    vz = O.vertex(r, so, G, dict(P, magnet_polarity=1.0, gamma_c0=0.0, gamma_c1=0.0, zv_min=-1e9, zv_max=1e9))
+    assert v0["n"] == vz["n"] and np.allclose(v0["z"], vz["z"], rtol=1e-10) and np.allclose(v0["m_pipi"], vz["m_pipi"], rtol=1e-12)
