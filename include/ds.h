@@ -90,6 +90,13 @@ typedef struct {
     double doca_max, zv_min, zv_max;  /* vertex cuts (BASELINE cfg3)                                             */
     double m_pi, m_p, m_ks, m_lambda, dm_ks, dm_lambda; /* MeV                                                   */
     double n2_min;                    /* pairs with |d_a x d_b|^2 below this have no vertex       (A-14)        */
+    /* Curved-track vertexing (P:255-P:269): x_i(z) = x_i + tx_i (z - z_ref) + gamma_i (z - z_ref)^2 (Eq. 4) with
+     * gamma_i = -magnet_polarity * (gamma_c0 + gamma_c1 * qop_i / 1000) (Eq. 3; qop in 1/GeV, the parametrisation in
+     * 1/MeV, A-27); closest approach by vtx_newton_iters Newton-Raphson steps from the straight-line solution (P:269:
+     * three, A-28); the masses use the slopes at the vertex z.  magnet_polarity = 0: straight tracks, closed form. */
+    double magnet_polarity, gamma_c0, gamma_c1;
+    int32_t vtx_newton_iters;         /* 0..16                                                                  */
+    int32_t pad_;
 } ds_params;
 #define DS_MAX_FIRST_HITS 10
 
@@ -199,7 +206,8 @@ int ds_ghost_killer(ds_handle *h, const ds_seeds *seeds, const ds_params *p, ds_
 size_t ds_vertex_workspace_bytes(const ds_handle *h, int n_events, int64_t n_seeds);
 
 /* Per event: all (positive, negative) pairs of tracks with keep = 1; closed-form closest approach of the two
- * straight lines, midpoint vertex, DOCA, m_pipi, m_ppi (proton = larger momentum, A-15), cuts; passing pairs are
+ * straight lines (or, with magnet_polarity != 0, Newton-Raphson on the two parabolas of Eq. 4), midpoint vertex, DOCA,
+ * m_pipi, m_ppi (proton = larger momentum, A-15), cuts; passing pairs are
  * written in (ia, ib) order: count -> exclusive scan over events -> write.  Only x, y, tx, ty, qop, keep of `trk`
  * are read.  Deciding arithmetic in fp64. */
 int ds_vertex(ds_handle *h, const ds_tracks *trk, const int32_t *seed_offsets, int n_events, const ds_params *p,

@@ -42,6 +42,7 @@ bool make_const(const ds_geometry &g, const ds_params *p, DevConst &c)
 {
     if (!p || p->struct_size != sizeof(ds_params)) return false;
     if (p->max_first_hits < 1 || p->max_first_hits > DS_MAX_FIRST_HITS) return false;
+    if (p->vtx_newton_iters < 0 || p->vtx_newton_iters > 16) return false;
     double dmax = 0.0;
     for (int l = 0; l < 4; ++l) {
         c.z_layer[l] = g.z_layer[l];
@@ -68,6 +69,8 @@ bool make_const(const ds_geometry &g, const ds_params *p, DevConst &c)
     c.doca_max = p->doca_max; c.zv_min = p->zv_min; c.zv_max = p->zv_max;
     c.m_pi = p->m_pi; c.m_p = p->m_p; c.m_ks = p->m_ks; c.m_lambda = p->m_lambda;
     c.dm_ks = p->dm_ks; c.dm_lambda = p->dm_lambda; c.n2_min = p->n2_min;
+    c.vtx_mp = p->magnet_polarity; c.gamma_c0 = p->gamma_c0; c.gamma_c1 = p->gamma_c1;
+    c.vtx_iters = p->vtx_newton_iters; c.pad2_ = 0;
     return true;
 }
 

@@ -261,7 +261,10 @@ cudaError_t launch_layout(const DevConst &c, const LayoutPtrs &p, const int32_t 
     const size_t smem = layout_smem_bytes(cap, c.n_bins);
     // opt in to the full 227 KB of dynamic shared memory; per device, cheap and the same value for every caller, so it is
     // simply set at every launch (handles on several devices and host threads share this code)
-    cudaError_t aerr = cudaFuncSetAttribute(k_layout, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    cudaFuncAttributes fa;
+    cudaError_t aerr = cudaFuncGetAttributes(&fa, k_layout);
+    if (aerr != cudaSuccess) return aerr;
+    aerr = cudaFuncSetAttribute(k_layout, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - (int)fa.sharedSizeBytes);
     if (aerr != cudaSuccess) return aerr;
     // the bulk copies need 16-byte aligned sources (offsets inside the arrays are handled by the kernel)
     const uintptr_t bits = reinterpret_cast<uintptr_t>(p.x0) | reinterpret_cast<uintptr_t>(p.z) |

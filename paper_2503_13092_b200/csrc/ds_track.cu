@@ -705,7 +705,10 @@ cudaError_t launch_track(const DevConst &c, const LayoutPtrs &lay, const ds_seed
     if (smem < sizeof(TrackShared<int>)) smem = sizeof(TrackShared<int>);   // the layout of an event that is not staged
     // opt in to the full 227 KB of dynamic shared memory; per device, cheap and the same value for every caller, so it is
     // simply set at every launch (handles on several devices and host threads share this code)
-    cudaError_t aerr = cudaFuncSetAttribute(k_track, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    cudaFuncAttributes fa;
+    cudaError_t aerr = cudaFuncGetAttributes(&fa, k_track);
+    if (aerr != cudaSuccess) return aerr;
+    aerr = cudaFuncSetAttribute(k_track, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - (int)fa.sharedSizeBytes);
     if (aerr != cudaSuccess) return aerr;
     prof.begin(DS_K_TRACK, st);
     k_track<<<n_events, kTrackThreads, smem, st>>>(c, lay, seeds, hit_offsets, seed_offsets, out, cap);

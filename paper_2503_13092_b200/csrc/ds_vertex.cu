@@ -30,6 +30,7 @@ struct VtxOut {
 // (|d| = sqrt(tx^2 + ty^2 + 1), p in MeV, k = p / |d|, E under the pion and the proton hypothesis).
 struct VtxTrack {
     double x, y, tx, ty, p, k, e_pi, e_p;
+    double g;   // gamma of Eq. 3: curvature of x(z) upstream of the UT; 0 with magnet_polarity = 0
 };
 
 __device__ __forceinline__ VtxTrack make_track(const DevConst &c, const ds_tracks &t, int i)
@@ -41,28 +42,30 @@ __device__ __forceinline__ VtxTrack make_track(const DevConst &c, const ds_track
     r.k = r.p / sqrt(r.tx * r.tx + r.ty * r.ty + 1.0);
     r.e_pi = sqrt(r.p * r.p + c.m_pi * c.m_pi);
     r.e_p = sqrt(r.p * r.p + c.m_p * c.m_p);
+    r.g = -c.vtx_mp * (c.gamma_c0 + c.gamma_c1 * (q / 1000.0));   // q/p in 1/GeV, the parametrisation in 1/MeV (A-27)
     return r;
 }
 
 // Kept tracks of one event in shared memory (positive tracks from the front, negative tracks from the back).
 struct VtxShared {
     float x[kVtxCap], y[kVtxCap], tx[kVtxCap], ty[kVtxCap];
-    double p[kVtxCap], k[kVtxCap], e_pi[kVtxCap], e_p[kVtxCap];
+    double p[kVtxCap], k[kVtxCap], e_pi[kVtxCap], e_p[kVtxCap], g[kVtxCap];
     __device__ __forceinline__ void put(int pos, const VtxTrack &r)
     {
         x[pos] = (float)r.x; y[pos] = (float)r.y; tx[pos] = (float)r.tx; ty[pos] = (float)r.ty;   // exact: they were fp32
-        p[pos] = r.p; k[pos] = r.k; e_pi[pos] = r.e_pi; e_p[pos] = r.e_p;
+        p[pos] = r.p; k[pos] = r.k; e_pi[pos] = r.e_pi; e_p[pos] = r.e_p; g[pos] = r.g;
     }
     __device__ __forceinline__ VtxTrack get(int pos) const
     {
         VtxTrack r;
         r.x = x[pos]; r.y = y[pos]; r.tx = tx[pos]; r.ty = ty[pos];
-        r.p = p[pos]; r.k = k[pos]; r.e_pi = e_pi[pos]; r.e_p = e_p[pos];
+        r.p = p[pos]; r.k = k[pos]; r.e_pi = e_pi[pos]; r.e_p = e_p[pos]; r.g = g[pos];
         return r;
     }
 };
 
 // a = positive track, b = negative track.  Returns true iff the pair passes every cut; o is complete only then.
+template <bool kCurved>
 __device__ __forceinline__ bool vertex_pair(const DevConst &c, const VtxTrack &a, const VtxTrack &b, VtxOut &o)
 {
     // n = d_a x d_b with d = (tx, ty, 1): built from slope differences; |n|^2 = A*C - B^2 (Lagrange) without cancellation
@@ -72,9 +75,27 @@ __device__ __forceinline__ bool vertex_pair(const DevConst &c, const VtxTrack &a
     const double A = a.tx * a.tx + a.ty * a.ty + 1.0, B = a.tx * b.tx + a.ty * b.ty + 1.0, C = b.tx * b.tx + b.ty * b.ty + 1.0;
     const double rx = a.x - b.x, ry = a.y - b.y;
     const double Dd = a.tx * rx + a.ty * ry, Ee = b.tx * rx + b.ty * ry;
-    const double sa = (B * Ee - C * Dd) / n2, sb = (A * Ee - B * Dd) / n2;
-    const double qax = a.x + sa * a.tx, qay = a.y + sa * a.ty, qaz = c.z_ref + sa;
-    const double qbx = b.x + sb * b.tx, qby = b.y + sb * b.ty, qbz = c.z_ref + sb;
+    double sa = (B * Ee - C * Dd) / n2, sb = (A * Ee - B * Dd) / n2;
+    constexpr bool curved = kCurved;   // the launcher instantiates the straight-track kernels for magnet_polarity = 0
+    if (curved) {
+        // Newton-Raphson on F(u, v) = |Traj_a(z_ref + u) - Traj_b(z_ref + v)|^2 with the parabolas of Eq. 4, from the
+        // straight-line solution (A-28); gradient and Hessian of F / 2
+        for (int it = 0; it < c.vtx_iters; ++it) {
+            const double Dx = a.x + a.tx * sa + a.g * sa * sa - (b.x + b.tx * sb + b.g * sb * sb);
+            const double Dy = a.y + a.ty * sa - (b.y + b.ty * sb), Dz = sa - sb;
+            const double dax = a.tx + 2.0 * a.g * sa, dbx = b.tx + 2.0 * b.g * sb;
+            const double gu = Dx * dax + Dy * a.ty + Dz, gv = -(Dx * dbx + Dy * b.ty + Dz);
+            const double Huu = dax * dax + a.ty * a.ty + 1.0 + Dx * 2.0 * a.g;
+            const double Hvv = dbx * dbx + b.ty * b.ty + 1.0 - Dx * 2.0 * b.g;
+            const double Huv = -(dax * dbx + a.ty * b.ty + 1.0);
+            const double det = Huu * Hvv - Huv * Huv;
+            if (det == 0.0) break;
+            sa += -(Hvv * gu - Huv * gv) / det;
+            sb += -(Huu * gv - Huv * gu) / det;
+        }
+    }
+    const double qax = a.x + sa * a.tx + a.g * sa * sa, qay = a.y + sa * a.ty, qaz = c.z_ref + sa;
+    const double qbx = b.x + sb * b.tx + b.g * sb * sb, qby = b.y + sb * b.ty, qbz = c.z_ref + sb;
     const double dx = qax - qbx, dy = qay - qby, dz = qaz - qbz;
     o.x = 0.5 * (qax + qbx);
     o.y = 0.5 * (qay + qby);
@@ -82,7 +103,14 @@ __device__ __forceinline__ bool vertex_pair(const DevConst &c, const VtxTrack &a
     o.doca = sqrt(dx * dx + dy * dy + dz * dz);
     if (!(o.doca < c.doca_max && c.zv_min <= o.z && o.z <= c.zv_max)) return false;
     // invariant masses: same momentum sum under both hypotheses; proton = larger momentum (A-15)
-    const double px = a.k * a.tx + b.k * b.tx, py = a.k * a.ty + b.k * b.ty, pz = a.k + b.k;
+    double atx = a.tx, btx = b.tx, ak = a.k, bk = b.k;
+    if (curved) {   // slopes dx/dz at the vertex z (Eq. 2) and with them the direction normalisation
+        atx = a.tx + 2.0 * a.g * (o.z - c.z_ref);
+        btx = b.tx + 2.0 * b.g * (o.z - c.z_ref);
+        ak = a.p / sqrt(atx * atx + a.ty * a.ty + 1.0);
+        bk = b.p / sqrt(btx * btx + b.ty * b.ty + 1.0);
+    }
+    const double px = ak * atx + bk * btx, py = ak * a.ty + bk * b.ty, pz = ak + bk;
     const double p2 = px * px + py * py + pz * pz;
     const double e1 = a.e_pi + b.e_pi, e2 = a.p >= b.p ? a.e_p + b.e_pi : a.e_pi + b.e_p;
     const double m1 = e1 * e1 - p2, m2 = e2 * e2 - p2;
@@ -151,6 +179,7 @@ __device__ __forceinline__ void block_ordered_offsets(bool f0, bool f1, int (*wa
     off1 = b1 + __popc(m1 & lanemask_lt());
 }
 
+template <bool kCurved>
 __global__ void __launch_bounds__(kVtxThreads)
 k_vertex_count(const __grid_constant__ DevConst c, const ds_tracks trk, const int32_t *__restrict__ seed_offsets,
                PairLists pl, int32_t *__restrict__ n_per_event)
@@ -195,7 +224,7 @@ k_vertex_count(const __grid_constant__ DevConst c, const ds_tracks trk, const in
         int ia, ib;
         pair_tracks(c, trk, ps, k, ta, tb, ia, ib);
         VtxOut o;
-        mine += vertex_pair(c, ta, tb, o) ? 1 : 0;
+        mine += vertex_pair<kCurved>(c, ta, tb, o) ? 1 : 0;
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) mine += __shfl_xor_sync(0xffffffffu, mine, o);
@@ -253,6 +282,7 @@ k_vertex_scan(const int32_t *__restrict__ n_per_event, int n_events, int64_t *__
     }
 }
 
+template <bool kCurved>
 __global__ void __launch_bounds__(kVtxThreads)
 k_vertex_write(const __grid_constant__ DevConst c, const ds_tracks trk, const int32_t *__restrict__ seed_offsets,
                PairLists pl, const ds_vertices out)
@@ -286,7 +316,7 @@ k_vertex_write(const __grid_constant__ DevConst c, const ds_tracks trk, const in
         if (k < npairs) {
             VtxTrack ta, tb;
             pair_tracks(c, trk, ps, k, ta, tb, ia, ib);
-            pass = vertex_pair(c, ta, tb, o);
+            pass = vertex_pair<kCurved>(c, ta, tb, o);
         }
         int off, off1, tot, tot1;
         block_ordered_offsets(pass, false, warp_cnt, off, off1, tot, tot1);
@@ -316,17 +346,17 @@ constexpr int kMaskIters = 64;  // pair iterations covered by the 64-bit lane ma
 
 struct WarpTracks {
     float x[kWCap], y[kWCap], tx[kWCap], ty[kWCap];
-    double p[kWCap], k[kWCap], e_pi[kWCap], e_p[kWCap];
+    double p[kWCap], k[kWCap], e_pi[kWCap], e_p[kWCap], g[kWCap];
     __device__ __forceinline__ void put(int pos, const VtxTrack &r)
     {
         x[pos] = (float)r.x; y[pos] = (float)r.y; tx[pos] = (float)r.tx; ty[pos] = (float)r.ty;   // exact: they were fp32
-        p[pos] = r.p; k[pos] = r.k; e_pi[pos] = r.e_pi; e_p[pos] = r.e_p;
+        p[pos] = r.p; k[pos] = r.k; e_pi[pos] = r.e_pi; e_p[pos] = r.e_p; g[pos] = r.g;
     }
     __device__ __forceinline__ VtxTrack get(int pos) const
     {
         VtxTrack r;
         r.x = x[pos]; r.y = y[pos]; r.tx = tx[pos]; r.ty = ty[pos];
-        r.p = p[pos]; r.k = k[pos]; r.e_pi = e_pi[pos]; r.e_p = e_p[pos];
+        r.p = p[pos]; r.k = k[pos]; r.e_pi = e_pi[pos]; r.e_p = e_p[pos]; r.g = g[pos];
         return r;
     }
 };
@@ -350,6 +380,7 @@ __device__ __forceinline__ void pair_index(int64_t k, int nneg, int &a, int &b)
     }
 }
 
+template <bool kCurved>
 __global__ void __launch_bounds__(kWThreads)
 k_vertex_count_w(const __grid_constant__ DevConst c, const ds_tracks trk, const int32_t *__restrict__ seed_offsets,
                  int n_events, PairLists pl, WarpWork ww, int32_t *__restrict__ n_per_event)
@@ -409,7 +440,7 @@ k_vertex_count_w(const __grid_constant__ DevConst c, const ds_tracks trk, const 
             tb = make_track(c, trk, list[n_seeds - 1 - b]);
         }
         VtxOut o;
-        if (vertex_pair(c, ta, tb, o)) {
+        if (vertex_pair<kCurved>(c, ta, tb, o)) {
             ++mine;
             if (it < kMaskIters) mask |= 1ull << it;
         }
@@ -427,6 +458,7 @@ constexpr int kW2Threads = 256;
 constexpr int kW2Warps = kW2Threads / 32;
 static_assert(kGroup % kW2Warps == 0, "a block of k_vertex_write_w stays inside one group");
 
+template <bool kCurved>
 __global__ void __launch_bounds__(kW2Threads)
 k_vertex_write_w(const __grid_constant__ DevConst c, const ds_tracks trk, const int32_t *__restrict__ seed_offsets,
                  int n_events, PairLists pl, WarpWork ww, const ds_vertices out)
@@ -482,7 +514,7 @@ k_vertex_write_w(const __grid_constant__ DevConst c, const ds_tracks trk, const 
             pair_index(buf[lane], nneg, a, b);
             const int ia = list[a], ib = list[n_seeds - 1 - b];
             VtxOut o;
-            vertex_pair(c, make_track(c, trk, ia), make_track(c, trk, ib), o);   // passes again: same arithmetic
+            vertex_pair<kCurved>(c, make_track(c, trk, ia), make_track(c, trk, ib), o);   // passes again: same arithmetic
             const int64_t pos = o0 + written + lane;
             if (pos < out.capacity) {
                 out.evt[pos] = e; out.ia[pos] = ia; out.ib[pos] = ib; out.flags[pos] = o.flags;
@@ -515,7 +547,7 @@ k_vertex_write_w(const __grid_constant__ DevConst c, const ds_tracks trk, const 
             pair_index(k, nneg, a, b);
             ia = list[a];
             ib = list[n_seeds - 1 - b];
-            pass = vertex_pair(c, make_track(c, trk, ia), make_track(c, trk, ib), o);
+            pass = vertex_pair<kCurved>(c, make_track(c, trk, ia), make_track(c, trk, ib), o);
         }
         const unsigned m = __ballot_sync(FULL, pass);
         const int64_t pos = o0 + written + __popc(m & lanemask_lt());
@@ -558,6 +590,7 @@ cudaError_t launch_vertex(const DevConst &c, const ds_tracks &trk, const int32_t
     cudaError_t err = cudaSuccess;
     // batches of small events (the Run-3-like configurations): a warp per event; large events: a block per event
     const bool small_events = n_events > 0 && trk.n / n_events <= kSmallEventSeeds;
+    const bool curved = c.vtx_mp != 0.0;   // parabolic trajectories + Newton-Raphson (P:255-P:269); else straight tracks
     if (n_events <= 0) {
         prof.begin(DS_K_VTX_SCAN, st);
         k_vertex_scan<<<1, kScanThreads, 0, st>>>(out.n_per_event, n_events, out.offsets, out.capacity, out.overflow);
@@ -568,18 +601,28 @@ cudaError_t launch_vertex(const DevConst &c, const ds_tracks &trk, const int32_t
         err = cudaMemsetAsync(ww.group_sums, 0, sizeof(int32_t) * n_groups, st);
         if (err != cudaSuccess) return err;
         prof.begin(DS_K_VTX_COUNT, st);
-        k_vertex_count_w<<<(n_events + kWWarps - 1) / kWWarps, kWThreads, 0, st>>>(c, trk, seed_offsets, n_events, pl, ww,
-                                                                                   out.n_per_event);
+        if (curved)
+            k_vertex_count_w<true><<<(n_events + kWWarps - 1) / kWWarps, kWThreads, 0, st>>>(c, trk, seed_offsets, n_events, pl, ww,
+                                                                                             out.n_per_event);
+        else
+            k_vertex_count_w<false><<<(n_events + kWWarps - 1) / kWWarps, kWThreads, 0, st>>>(c, trk, seed_offsets, n_events, pl,
+                                                                                              ww, out.n_per_event);
         prof.end(st);
         err = cudaGetLastError();
         if (err != cudaSuccess) return err;
         prof.begin(DS_K_VTX_WRITE, st);
-        k_vertex_write_w<<<(n_events + kW2Warps - 1) / kW2Warps, kW2Threads, 0, st>>>(c, trk, seed_offsets, n_events, pl, ww, out);
+        if (curved)
+            k_vertex_write_w<true><<<(n_events + kW2Warps - 1) / kW2Warps, kW2Threads, 0, st>>>(c, trk, seed_offsets, n_events, pl, ww, out);
+        else
+            k_vertex_write_w<false><<<(n_events + kW2Warps - 1) / kW2Warps, kW2Threads, 0, st>>>(c, trk, seed_offsets, n_events, pl, ww, out);
         prof.end(st);
         return cudaGetLastError();
     }
     prof.begin(DS_K_VTX_COUNT, st);
-    k_vertex_count<<<n_events, kVtxThreads, 0, st>>>(c, trk, seed_offsets, pl, out.n_per_event);
+    if (curved)
+        k_vertex_count<true><<<n_events, kVtxThreads, 0, st>>>(c, trk, seed_offsets, pl, out.n_per_event);
+    else
+        k_vertex_count<false><<<n_events, kVtxThreads, 0, st>>>(c, trk, seed_offsets, pl, out.n_per_event);
     prof.end(st);
     err = cudaGetLastError();
     if (err != cudaSuccess) return err;
@@ -589,7 +632,10 @@ cudaError_t launch_vertex(const DevConst &c, const ds_tracks &trk, const int32_t
     err = cudaGetLastError();
     if (err != cudaSuccess) return err;
     prof.begin(DS_K_VTX_WRITE, st);
-    k_vertex_write<<<n_events, kVtxThreads, 0, st>>>(c, trk, seed_offsets, pl, out);
+    if (curved)
+        k_vertex_write<true><<<n_events, kVtxThreads, 0, st>>>(c, trk, seed_offsets, pl, out);
+    else
+        k_vertex_write<false><<<n_events, kVtxThreads, 0, st>>>(c, trk, seed_offsets, pl, out);
     prof.end(st);
     return cudaGetLastError();
 }

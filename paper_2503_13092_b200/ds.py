@@ -47,7 +47,9 @@ class DsParams(ct.Structure):
                 ("max_first_hits", ct.c_int32), ("mlp_thr", ct.c_double), ("mlp_keep_above", ct.c_int32),
                 ("max_event_hits_hint", ct.c_int32), ("doca_max", ct.c_double), ("zv_min", ct.c_double),
                 ("zv_max", ct.c_double), ("m_pi", ct.c_double), ("m_p", ct.c_double), ("m_ks", ct.c_double),
-                ("m_lambda", ct.c_double), ("dm_ks", ct.c_double), ("dm_lambda", ct.c_double), ("n2_min", ct.c_double)]
+                ("m_lambda", ct.c_double), ("dm_ks", ct.c_double), ("dm_lambda", ct.c_double), ("n2_min", ct.c_double),
+                ("magnet_polarity", ct.c_double), ("gamma_c0", ct.c_double), ("gamma_c1", ct.c_double),
+                ("vtx_newton_iters", ct.c_int32), ("pad_", ct.c_int32)]
 
 
 class DsHits(ct.Structure):

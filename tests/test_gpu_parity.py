@@ -373,6 +373,22 @@ def test_empty_and_ragged_inputs(ds, orc_mlp):
     assert not t0["found"].any() and v0["n"] == 0
 
 
+@pytest.mark.parametrize("cfg,n_events,mp", [(1, 300, 1.0), (1, 300, -1.0), (3, 40, 1.0)])
+def test_curved_track_vertexing(ds, orc_mlp, cfg, n_events, mp):
+    """parabolic trajectories upstream of the UT (Eq. 3 / Eq. 4) and Newton-Raphson closest approach
+     in both vertex kernel variants (cfg1: warp per event, cfg3: block per event) against the oracle."""
+    d = gen.generate(cfg, n_events=n_events)
+    pc = dict(P, magnet_polarity=mp)
+    st, sv, t, v = check_both(ds, d, orc_mlp, params=pc)
+    t0, v0 = gpu_run(ds, d)
+    assert v["n"] > 50 and v0["n"] > 50
+    both = min(len(v["z"]), len(v0["z"]), 50)
+    assert not np.allclose(v["z"][:both], v0["z"][:both], rtol=1e-6)      # the curvature moves the vertices
+    # no curvature left: the straight-track list again
+    t1, v1 = gpu_run(ds, d, params=dict(pc, gamma_c0=0.0, gamma_c1=0.0))
+    assert v1["n"] == v0["n"] and np.array_equal(v1["ia"], v0["ia"]) and np.allclose(v1["z"], v0["z"], rtol=1e-6)
+
+
 def test_vertexing_large_events_in_a_small_event_batch(ds, orc_mlp):
     """A few cfg3 events (~500 seeds, thousands of pairs) among many empty ones: the batch averages few seeds per event
     and takes the warp-per-event vertex kernels, whose staging capacity and pair mask these events exceed.  The same
