@@ -155,6 +155,8 @@ def run_reference(args, rank):
         return
     import gen
     from gen import constants as C
+    if args.magnet_polarity != 0.0:
+        C.PARAMS = dict(C.PARAMS, magnet_polarity=args.magnet_polarity)
     d = gen.generate(CFG, n_events=args.subbatch, workers=min(8, os.cpu_count() or 1))
     per_step = min(10.0, 150.0 / max(1, args.steps + args.warmup))
     n = sized_sample(d, per_step, args.subbatch)
@@ -191,6 +193,8 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--magnet-polarity", type=float, default=0.0,
+                    help="+1 / -1: curved-track vertexing (SURVEY 8f N1, P:255-P:269) in both arms; 0 = BASELINE configs")
     args = ap.parse_args()
     rank, world = int(os.environ.get("RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
     local = int(os.environ.get("LOCAL_RANK", 0))
@@ -201,6 +205,8 @@ def main():
 
     from gen import constants as C
     import gen
+    if args.magnet_polarity != 0.0:   # both arms (the oracle legs read C.PARAMS) vertex with the parabolas of Eq. 4
+        C.PARAMS = dict(C.PARAMS, magnet_polarity=args.magnet_polarity)
     n_sub = max(1, args.events // args.subbatch)
     workers = max(1, min(32, (os.cpu_count() or 1) // max(1, world)))
     t0 = time.time()
@@ -389,6 +395,7 @@ def main():
                        "subbatches": n_sub, "events_per_subbatch": args.subbatch, "cuda_streams": n_streams,
                        "hits": sum(n_hits), "seeds": sum(n_seeds), "tracks_found": n_found, "tracks_kept": n_keep, "vertices": n_vtx,
                        "l2": "inputs larger than L2 (each sub-batch reads ~0.76 GB; 7.6 GB per step)",
+                       "magnet_polarity": args.magnet_polarity,
                        "parallelism": f"dp{world} (events sharded, no data-path collective)"},
             "roofline": roofline, "whole_path_gbs": whole_gbs, "whole_path_frac": whole_gbs / peak, "kernels": kernels,
             "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,

@@ -90,8 +90,9 @@ __device__ __forceinline__ bool vertex_pair(const DevConst &c, const VtxTrack &a
             const double Huv = -(dax * dbx + a.ty * b.ty + 1.0);
             const double det = Huu * Hvv - Huv * Huv;
             if (det == 0.0) break;
-            sa += -(Hvv * gu - Huv * gv) / det;
-            sb += -(Huu * gv - Huv * gu) / det;
+            const double inv = 1.0 / det;   // one division for both components
+            sa -= (Hvv * gu - Huv * gv) * inv;
+            sb -= (Huu * gv - Huv * gu) * inv;
         }
     }
     const double qax = a.x + sa * a.tx + a.g * sa * sa, qay = a.y + sa * a.ty, qaz = c.z_ref + sa;
