@@ -360,3 +360,25 @@ def generate(cfg_index: int, n_events: int | None = None, first_block: int = 0, 
     else:
         blocks = [_gen_one(j) for j in jobs]
     return take_events(concat(blocks), n_events)
+
+
+def with_clone_seeds(d: dict, every: int = 3, seed: int = 7) -> dict:
+    """Every `every`-th seed of an event once more at the end of the event, slightly displaced: a second SciFi segment of
+    the same particle, which finds the same UT hits -- the case clone killing exists for.  Input recipe only."""
+    rng = np.random.default_rng(seed)
+    so = d["seed_offsets"]
+    parts, new_so = {k: [] for k in d["seeds"]}, [0]
+    for e in range(d["n_events"]):
+        a, b = int(so[e]), int(so[e + 1])
+        dup = np.arange(a, b)[::every]
+        dx = rng.normal(0, 0.05, len(dup))
+        dq = rng.normal(0, 0.002, len(dup))
+        for k, v in d["seeds"].items():
+            c = v[dup].copy()
+            if k == "x":
+                c = (c + dx).astype(v.dtype)
+            if k == "qop":
+                c = (c * (1 + dq)).astype(v.dtype)
+            parts[k] += [v[a:b], c]
+        new_so.append(new_so[-1] + (b - a) + len(dup))
+    return dict(d, seeds={k: np.concatenate(v) for k, v in parts.items()}, seed_offsets=np.array(new_so, dtype=np.int32))

@@ -581,6 +581,43 @@ int64_t orc_vertex(const orc_geom *g, const orc_params *p, int n_events, const i
     return total;
 }
 
+/* ============================================================================================================
+ *  O-S6b  clone killing across seeds: "Iterating over all possible track pairs that have
+ *  more than two shared UT hits ..., the candidates with lower scores are killed."
+ *  Reading A-31: two found tracks of one event share a hit when they hold the same hit index in the same layer;
+ *  a pair with at least min_shared (3) shared hits is a clone pair; its worse member is killed, worse = larger
+ *  chi2 + miss_penalty * (4 - nhits) (the S6 score, A-9), ties -> larger seed index.  Every pair is judged on the
+ *  tracks as they came out of S6 (a killed track still kills), so the result does not depend on an iteration order.
+ *  chi2 / nhits / hit / found are the per-seed track records; killed[s] = 1 for the tracks removed.  Returns their
+ *  number.
+ * ============================================================================================================ */
+int64_t orc_clone_kill(const orc_params *p, int min_shared, int n_events, const int32_t *seed_off, const double *chi2,
+                       const int32_t *nhits, const int32_t *hit, const int32_t *found, int32_t *killed)
+{
+    int e;
+    int64_t n_killed = 0;
+    for (e = 0; e < n_events; ++e) {
+        int i, j, l;
+        for (i = seed_off[e]; i < seed_off[e + 1]; ++i) {
+            double si = chi2[i] + p->miss_penalty * (double)(4 - nhits[i]);
+            killed[i] = 0;
+            if (!found[i]) continue;
+            for (j = seed_off[e]; j < seed_off[e + 1]; ++j) {
+                double sj;
+                int shared = 0;
+                if (j == i || !found[j]) continue;
+                for (l = 0; l < 4; ++l)
+                    if (hit[4 * i + l] >= 0 && hit[4 * i + l] == hit[4 * j + l]) ++shared;
+                if (shared < min_shared) continue;
+                sj = chi2[j] + p->miss_penalty * (double)(4 - nhits[j]);
+                if (sj < si || (sj == si && j < i)) killed[i] = 1;      /* j is the better one of the pair */
+            }
+            n_killed += killed[i];
+        }
+    }
+    return n_killed;
+}
+
 int orc_max_threads(void)
 {
 #ifdef _OPENMP

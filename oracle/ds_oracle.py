@@ -183,6 +183,20 @@ def reconstruct(hits: dict, hit_offsets, seeds: dict, seed_offsets, geom: dict, 
     return out
 
 
+def clone_kill(tracks: dict, seed_offsets, params: dict, min_shared: int = 3) -> np.ndarray:
+    """O-S6b (N3): killed[s] = 1 for found tracks that share >= min_shared UT hits with a better track."""
+    so = _i(seed_offsets)
+    chi2 = _d(tracks["chi2"])
+    nhits, hit, found = _i(tracks["nhits"]), _i(np.asarray(tracks["hit"]).reshape(-1)), _i(tracks["found"])
+    killed = np.zeros(len(chi2), dtype=np.int32)
+    p = make_params(params)
+    lib().orc_clone_kill.restype = ct.c_int64
+    n = lib().orc_clone_kill(ct.byref(p), int(min_shared), len(so) - 1, _p(so, c_ip), _p(chi2), _p(nhits, c_ip), _p(hit, c_ip),
+                             _p(found, c_ip), _p(killed, c_ip))
+    assert n == int(killed.sum())
+    return killed
+
+
 def vertex(tracks: dict, seed_offsets, geom: dict, params: dict, edge_rel: float = 1e-5, n_threads: int = 0,
            capacity: int | None = None) -> dict:
     """O-S8/O-S9 for all events on the given per-seed track arrays (x, y, tx, ty, qop, keep)."""

@@ -670,3 +670,67 @@ def test_p11_pair_list_with_curvature_brute_force(orc_mlp):
     v0 = O.vertex(r, so, G, dict(P, zv_min=-1e9, zv_max=1e9))
     vz = O.vertex(r, so, G, dict(P, magnet_polarity=1.0, gamma_c0=0.0, gamma_c1=0.0, zv_min=-1e9, zv_max=1e9))
     assert v0["n"] == vz["n"] and np.allclose(v0["z"], vz["z"], rtol=1e-10) and np.allclose(v0["m_pipi"], vz["m_pipi"], rtol=1e-12)
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# P-12  clone killing across seeds, reading A-31
+# ---------------------------------------------------------------------------------------------------------------
+def _trk(chi2, nhits, hits, found=None):
+    n = len(chi2)
+    return dict(chi2=np.array(chi2, dtype=np.float64), nhits=np.array(nhits, dtype=np.int32),
+                found=np.array(found if found is not None else [1] * n, dtype=np.int32), hit=np.array(hits, dtype=np.int32))
+
+
+def test_p12_clone_kill_hand_cases():
+    # "more than two shared UT hits": three shared -> the worse one goes; two shared -> nobody
+    t = _trk([1.0, 2.0], [4, 4], [[1, 2, 3, 4], [1, 2, 3, 9]])
+    assert O.clone_kill(t, [0, 2], P).tolist() == [0, 1]
+    t = _trk([1.0, 2.0], [4, 4], [[1, 2, 3, 4], [1, 2, 7, 9]])
+    assert O.clone_kill(t, [0, 2], P).tolist() == [0, 0]
+    # same hit index in ANOTHER layer is not a shared hit; missing layers (-1) never count
+    t = _trk([1.0, 2.0], [4, 4], [[1, 2, 3, 4], [2, 1, 4, 3]])
+    assert O.clone_kill(t, [0, 2], P).tolist() == [0, 0]
+    t = _trk([1.0, 2.0], [2, 2], [[1, -1, -1, 4], [1, -1, -1, 4]])
+    assert O.clone_kill(t, [0, 2], P).tolist() == [0, 0]
+    # score = chi2 + miss_penalty * (4 - nhits): a 3-hit track with the smaller chi2 loses against a 4-hit one (A-9)
+    t = _trk([0.5, 3.0], [3, 4], [[1, 2, -1, 4], [1, 2, 3, 4]])
+    assert O.clone_kill(t, [0, 2], P).tolist() == [1, 0]
+    assert O.clone_kill(t, [0, 2], dict(P, miss_penalty=0.0)).tolist() == [0, 1]
+    # equal scores: the later seed goes
+    t = _trk([2.0, 2.0], [4, 4], [[1, 2, 3, 4], [1, 2, 3, 4]])
+    assert O.clone_kill(t, [0, 2], P).tolist() == [0, 1]
+    # judged on the S6 output: B is killed by A and still kills C (no dependence on an iteration order)
+    t = _trk([1.0, 2.0, 3.0], [4, 4, 4], [[1, 2, 3, 4], [1, 2, 3, 9], [8, 2, 3, 9]])
+    assert O.clone_kill(t, [0, 3], P).tolist() == [0, 1, 1]
+    # tracks that were not found neither kill nor are killed; events do not mix
+    t = _trk([1.0, 2.0, 3.0], [4, 4, 4], [[1, 2, 3, 4], [1, 2, 3, 4], [1, 2, 3, 4]], found=[0, 1, 1])
+    assert O.clone_kill(t, [0, 3], P).tolist() == [0, 0, 1]
+    assert O.clone_kill(t, [0, 2, 3], P).tolist() == [0, 0, 0]
+    # thresholds: 5 shared hits cannot happen, 1 is enough for every overlapping pair
+    t = _trk([1.0, 2.0], [4, 4], [[1, 2, 3, 4], [1, 7, 8, 9]])
+    assert O.clone_kill(t, [0, 2], P, min_shared=5).tolist() == [0, 0] and O.clone_kill(t, [0, 2], P, min_shared=1).tolist() == [0, 1]
+
+
+def test_p12_clone_kill_equals_set_arithmetic(orc_mlp):
+    """On reconstructed cfg1 events with a third of the seeds doubled (gen.with_clone_seeds): the same list from a
+    restatement with Python sets of (layer, hit) pairs; without doubled seeds the synthetic events hold no clones."""
+    d0 = gen.generate(1, n_events=40)
+    r0 = run(d0, orc_mlp)
+    assert O.clone_kill(r0, d0["seed_offsets"], P).sum() == 0
+    d = gen.with_clone_seeds(d0)
+    r = run(d, orc_mlp)
+    so = d["seed_offsets"]
+    k = O.clone_kill(r, so, P)
+    ref = np.zeros_like(k)
+    score = r["chi2"].astype(np.float64) + P["miss_penalty"] * (4 - r["nhits"])
+    for e in range(d["n_events"]):
+        idx = [i for i in range(so[e], so[e + 1]) if r["found"][i]]
+        sets = {i: {(l, int(h)) for l, h in enumerate(r["hit"][i]) if h >= 0} for i in idx}
+        for i in idx:
+            for j in idx:
+                if i != j and len(sets[i] & sets[j]) > 2 and (score[j], j) < (score[i], i):
+                    ref[i] = 1
+    assert np.array_equal(k, ref)
+    # a doubled true seed makes a clone pair of which one member goes: the found tracks return to the original count
+    n0 = int(r0["found"].sum())
+    assert k.sum() > 50 and abs(int(r["found"].sum()) - int(k.sum()) - n0) <= 0.05 * n0
