@@ -126,6 +126,7 @@ def algorithmic_bytes(n_events, n_hits, n_seeds, n_found, n_keep, n_vtx):
         "k_vertex_count": 28 * n_keep + 8 * n_seeds + 4 * n_events,
         "k_vertex_scan": 16 * n_events,
         "k_vertex_write": 28 * n_keep + 40 * n_vtx,
+        "k_clone": 28 * n_seeds,                                           # hit[4], chi2, nhits, found of every slot
     }
 
 
@@ -193,6 +194,8 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--clone-min-shared", type=int, default=0,
+                    help="3: clone killing across seeds between S6 and S7 (SURVEY 8f N3, P:115); 0 = BASELINE configs")
     ap.add_argument("--magnet-polarity", type=float, default=0.0,
                     help="+1 / -1: curved-track vertexing (SURVEY 8f N1, P:255-P:269) in both arms; 0 = BASELINE configs")
     args = ap.parse_args()
@@ -207,6 +210,8 @@ def main():
     import gen
     if args.magnet_polarity != 0.0:   # both arms (the oracle legs read C.PARAMS) vertex with the parabolas of Eq. 4
         C.PARAMS = dict(C.PARAMS, magnet_polarity=args.magnet_polarity)
+    if args.clone_min_shared:         # our arm only: the timed oracle legs have no clone-killing step
+        C.PARAMS = dict(C.PARAMS, clone_min_shared=args.clone_min_shared)
     n_sub = max(1, args.events // args.subbatch)
     workers = max(1, min(32, (os.cpu_count() or 1) // max(1, world)))
     t0 = time.time()
@@ -395,7 +400,7 @@ def main():
                        "subbatches": n_sub, "events_per_subbatch": args.subbatch, "cuda_streams": n_streams,
                        "hits": sum(n_hits), "seeds": sum(n_seeds), "tracks_found": n_found, "tracks_kept": n_keep, "vertices": n_vtx,
                        "l2": "inputs larger than L2 (each sub-batch reads ~0.76 GB; 7.6 GB per step)",
-                       "magnet_polarity": args.magnet_polarity,
+                       "magnet_polarity": args.magnet_polarity, "clone_min_shared": args.clone_min_shared,
                        "parallelism": f"dp{world} (events sharded, no data-path collective)"},
             "roofline": roofline, "whole_path_gbs": whole_gbs, "whole_path_frac": whole_gbs / peak, "kernels": kernels,
             "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,

@@ -38,6 +38,8 @@ PARAMS = dict(
     # curved-track vertexing (P:255-P:269): gamma = -MP (c0 + c1 q/p[1/MeV]) (Eq. 3); the synthetic
     # configurations have no field upstream of the UT, so MP = 0 (straight tracks, A-20) is the default
     magnet_polarity=0.0, gamma_c0=-1.5e-8, gamma_c1=9.3e-3, vtx_newton_iters=3,
+    # clone killing across seeds: shared hits that make a clone pair; 0 = off (BASELINE configs)
+    clone_min_shared=0,
 )
 
 # A-10: fixed input normalisation (mu, sigma) for [x, y, tx, ty, qop, chi2, qop_seed, chi2_seed]

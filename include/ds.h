@@ -96,7 +96,10 @@ typedef struct {
      * three, A-28); the masses use the slopes at the vertex z.  magnet_polarity = 0: straight tracks, closed form. */
     double magnet_polarity, gamma_c0, gamma_c1;
     int32_t vtx_newton_iters;         /* 0..16                                                                  */
-    int32_t pad_;
+    int32_t clone_min_shared;         /* clone killing across seeds (A-31): found tracks of an event that share at
+                                         least this many UT hits (same index, same layer) with a better track (smaller
+                                         chi2 + miss_penalty*(4 - nhits), ties: earlier seed) are removed after S6;
+                                         paper: 3 ("more than two"); 0 = off (the BASELINE configurations)              */
 } ds_params;
 #define DS_MAX_FIRST_HITS 10
 
@@ -198,6 +201,12 @@ int ds_reconstruct(ds_handle *h, const ds_hits *hits, const ds_seeds *seeds, con
                    const int32_t *seed_offsets, int n_events, const ds_params *p, ds_tracks *out, void *workspace,
                    size_t workspace_bytes, void *cuda_stream);
 
+/* Clone killing alone (A-31; needs params->clone_min_shared > 0): removes from `trk` (x..chi2, nhits, hit, found
+ * are read) every found track that shares enough hits with a better one; its slot becomes the "not found" record
+ * (zeros, hit = -1, found = score = keep = 0).  ds_reconstruct does the same between S6 and S7. */
+int ds_clone_kill(ds_handle *h, const int32_t *seed_offsets, int n_events, const ds_params *p, ds_tracks *trk,
+                  void *cuda_stream);
+
 /* S7 alone: re-score tracks already in `trk` (reads x..chi2, found and the seeds' qop / chi2; writes score, keep). */
 int ds_ghost_killer(ds_handle *h, const ds_seeds *seeds, const ds_params *p, ds_tracks *trk, void *cuda_stream);
 
@@ -226,7 +235,7 @@ int ds_process_host(ds_handle *h, const ds_hits *hits, const ds_seeds *seeds, co
 /* ---- per-kernel device timing (measurement aid; no effect on results) ------------------------------------------ */
 
 /* Kernels of the path, in launch order. */
-enum { DS_K_LAYOUT = 0, DS_K_TRACK, DS_K_MLP, DS_K_VTX_COUNT, DS_K_VTX_SCAN, DS_K_VTX_WRITE, DS_K_COUNT };
+enum { DS_K_LAYOUT = 0, DS_K_TRACK, DS_K_MLP, DS_K_VTX_COUNT, DS_K_VTX_SCAN, DS_K_VTX_WRITE, DS_K_CLONE, DS_K_COUNT };
 
 typedef struct {
     size_t struct_size;

@@ -43,6 +43,7 @@ bool make_const(const ds_geometry &g, const ds_params *p, DevConst &c)
     if (!p || p->struct_size != sizeof(ds_params)) return false;
     if (p->max_first_hits < 1 || p->max_first_hits > DS_MAX_FIRST_HITS) return false;
     if (p->vtx_newton_iters < 0 || p->vtx_newton_iters > 16) return false;
+    if (p->clone_min_shared < 0) return false;
     double dmax = 0.0;
     for (int l = 0; l < 4; ++l) {
         c.z_layer[l] = g.z_layer[l];
@@ -70,7 +71,7 @@ bool make_const(const ds_geometry &g, const ds_params *p, DevConst &c)
     c.m_pi = p->m_pi; c.m_p = p->m_p; c.m_ks = p->m_ks; c.m_lambda = p->m_lambda;
     c.dm_ks = p->dm_ks; c.dm_lambda = p->dm_lambda; c.n2_min = p->n2_min;
     c.vtx_mp = p->magnet_polarity; c.gamma_c0 = p->gamma_c0; c.gamma_c1 = p->gamma_c1;
-    c.vtx_iters = p->vtx_newton_iters; c.pad2_ = 0;
+    c.vtx_iters = p->vtx_newton_iters; c.clone_min_shared = p->clone_min_shared;
     return true;
 }
 
@@ -271,6 +272,22 @@ int ds_ghost_killer(ds_handle *h, const ds_seeds *seeds, const ds_params *p, ds_
     return DS_OK;
 }
 
+int ds_clone_kill(ds_handle *h, const int32_t *seed_offsets, int n_events, const ds_params *p, ds_tracks *trk,
+                  void *cuda_stream)
+{
+    if (!h || !seed_offsets || n_events < 0 || !trk || !tracks_ok(trk, trk->n)) return DS_E_ARG;
+    if (!h->has_geom) return DS_E_NOGEOM;
+    DevConst c;
+    if (!make_const(h->geom, p, c) || c.clone_min_shared <= 0) return DS_E_ARG;
+    DeviceGuard guard(h->device);
+    if (!guard.ok) return DS_E_CUDA;
+    if (launch_clone(c, seed_offsets, n_events, *trk, (cudaStream_t)cuda_stream, h->prof) != cudaSuccess) {
+        cudaGetLastError();
+        return DS_E_CUDA;
+    }
+    return DS_OK;
+}
+
 int ds_reconstruct(ds_handle *h, const ds_hits *hits, const ds_seeds *seeds, const int32_t *hit_offsets,
                    const int32_t *seed_offsets, int n_events, const ds_params *p, ds_tracks *out, void *workspace,
                    size_t workspace_bytes, void *cuda_stream)
@@ -291,6 +308,7 @@ int ds_reconstruct(ds_handle *h, const ds_hits *hits, const ds_seeds *seeds, con
     carve_layout(workspace, c.n_bins, n_events, hits->n, L);
     cudaError_t err = launch_layout(c, L, hit_offsets, n_events, p->max_event_hits_hint, st, h->prof);
     if (err == cudaSuccess) err = launch_track(c, L, *seeds, hit_offsets, seed_offsets, n_events, p->max_event_hits_hint, *out, st, h->prof);
+    if (err == cudaSuccess) err = launch_clone(c, seed_offsets, n_events, *out, st, h->prof);
     if (err == cudaSuccess) err = launch_mlp(c, h->d_mlp, *seeds, *out, st, h->prof);
     if (err != cudaSuccess) {
         cudaGetLastError();
@@ -400,6 +418,7 @@ int ds_process_host(ds_handle *h, const ds_hits *hits, const ds_seeds *seeds, co
     carve_layout(wrec, c.n_bins, n_events, hits->n, L);
     err = launch_layout(c, L, d_hoff, n_events, p->max_event_hits_hint, st, h->prof);
     if (err == cudaSuccess) err = launch_track(c, L, dsd, d_hoff, d_soff, n_events, p->max_event_hits_hint, dt, st, h->prof);
+    if (err == cudaSuccess) err = launch_clone(c, d_soff, n_events, dt, st, h->prof);
     if (err == cudaSuccess) err = launch_mlp(c, h->d_mlp, dsd, dt, st, h->prof);
     if (err == cudaSuccess) err = launch_vertex(c, dt, d_soff, n_events, dv, wvtx, st, h->prof);
     auto d2h = [&](void *dst, const void *src, size_t bytes) {
@@ -456,7 +475,8 @@ int ds_profile_read(ds_handle *h, ds_profile *out)
 
 const char *ds_kernel_name(int k)
 {
-    static const char *names[DS_K_COUNT] = {"k_layout", "k_track", "k_mlp", "k_vertex_count", "k_vertex_scan", "k_vertex_write"};
+    static const char *names[DS_K_COUNT] = {"k_layout", "k_track", "k_mlp", "k_vertex_count", "k_vertex_scan", "k_vertex_write",
+                                               "k_clone"};
     return (k >= 0 && k < DS_K_COUNT) ? names[k] : nullptr;
 }
 

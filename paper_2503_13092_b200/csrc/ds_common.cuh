@@ -33,7 +33,7 @@ struct DevConst {
     int mlp_keep_above, pad_;
     double doca_max, zv_min, zv_max, m_pi, m_p, m_ks, m_lambda, dm_ks, dm_lambda, n2_min;
     double vtx_mp, gamma_c0, gamma_c1;   // curved-track vertexing: gamma = -vtx_mp * (gamma_c0 + gamma_c1 * qop / 1000)
-    int vtx_iters, pad2_;
+    int vtx_iters, clone_min_shared;
 };
 
 // Device copy of the ghost-killer weights (global memory, staged to shared memory by the kernel).
@@ -165,6 +165,9 @@ cudaError_t launch_extrapolate(const DevConst &c, const ds_seeds &seeds, double 
 cudaError_t launch_track(const DevConst &c, const LayoutPtrs &lay, const ds_seeds &seeds, const int32_t *hit_offsets,
                          const int32_t *seed_offsets, int n_events, int max_event_hits_hint, const ds_tracks &out,
                          cudaStream_t st, Prof &prof);
+
+cudaError_t launch_clone(const DevConst &c, const int32_t *seed_offsets, int n_events, const ds_tracks &trk, cudaStream_t st,
+                         Prof &prof);
 
 cudaError_t launch_mlp(const DevConst &c, const DevMlp *mlp, const ds_seeds &seeds, const ds_tracks &trk,
                        cudaStream_t st, Prof &prof);

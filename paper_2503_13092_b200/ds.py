@@ -49,7 +49,7 @@ class DsParams(ct.Structure):
                 ("zv_max", ct.c_double), ("m_pi", ct.c_double), ("m_p", ct.c_double), ("m_ks", ct.c_double),
                 ("m_lambda", ct.c_double), ("dm_ks", ct.c_double), ("dm_lambda", ct.c_double), ("n2_min", ct.c_double),
                 ("magnet_polarity", ct.c_double), ("gamma_c0", ct.c_double), ("gamma_c1", ct.c_double),
-                ("vtx_newton_iters", ct.c_int32), ("pad_", ct.c_int32)]
+                ("vtx_newton_iters", ct.c_int32), ("clone_min_shared", ct.c_int32)]
 
 
 class DsHits(ct.Structure):
@@ -75,7 +75,7 @@ class DsVertices(ct.Structure):
                 ("offsets", ct.c_void_p), ("overflow", ct.c_void_p), ("capacity", ct.c_int64)]
 
 
-DS_K_COUNT = 6
+DS_K_COUNT = 7
 
 
 class DsProfile(ct.Structure):
@@ -124,6 +124,7 @@ def lib() -> ct.CDLL:
         L.ds_reconstruct.argtypes = [vp, ct.POINTER(DsHits), ct.POINTER(DsSeeds), vp, vp, ct.c_int,
                                      ct.POINTER(DsParams), ct.POINTER(DsTracks), vp, ct.c_size_t, vp]
         L.ds_ghost_killer.argtypes = [vp, ct.POINTER(DsSeeds), ct.POINTER(DsParams), ct.POINTER(DsTracks), vp]
+        L.ds_clone_kill.argtypes = [vp, vp, ct.c_int, ct.POINTER(DsParams), ct.POINTER(DsTracks), vp]
         L.ds_vertex_workspace_bytes.argtypes = [vp, ct.c_int, ct.c_int64]
         L.ds_vertex_workspace_bytes.restype = ct.c_size_t
         L.ds_vertex.argtypes = [vp, ct.POINTER(DsTracks), vp, ct.c_int, ct.POINTER(DsParams), ct.POINTER(DsVertices),
@@ -278,6 +279,12 @@ def ds_reconstruct(h, hits, seeds, hit_offsets, seed_offsets, n_events, params: 
                                 _stream_ptr(stream)), "ds_reconstruct")
 
 
+def ds_clone_kill(h, seed_offsets, n_events: int, params: DsParams, tracks, stream=None) -> None:
+    ts = _tracks(tracks)
+    _check(lib().ds_clone_kill(h, _ptr(seed_offsets), n_events, ct.byref(params), ct.byref(ts), _stream_ptr(stream)),
+           "ds_clone_kill")
+
+
 def ds_ghost_killer(h, seeds, params: DsParams, tracks, stream=None) -> None:
     ss, ts = _seeds(seeds), _tracks(tracks)
     _check(lib().ds_ghost_killer(h, ct.byref(ss), ct.byref(params), ct.byref(ts), _stream_ptr(stream)),
@@ -428,6 +435,10 @@ class Downstream:
             workspace = self.workspace(ne, hits["id"].numel(), seeds["x"].numel())
         ds_reconstruct(self.h, hits, seeds, hit_offsets, seed_offsets, ne, self.params, out, workspace, stream)
         return out
+
+    def clone_kill(self, tracks: dict, seed_offsets, stream=None):
+        ds_clone_kill(self.h, seed_offsets, seed_offsets.numel() - 1, self.params, tracks, stream)
+        return tracks
 
     def ghost_killer(self, seeds: dict, tracks: dict, stream=None):
         ds_ghost_killer(self.h, seeds, self.params, tracks, stream)

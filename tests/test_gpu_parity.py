@@ -389,6 +389,40 @@ def test_curved_track_vertexing(ds, orc_mlp, cfg, n_events, mp):
     assert v1["n"] == v0["n"] and np.array_equal(v1["ia"], v0["ia"]) and np.allclose(v1["z"], v0["z"], rtol=1e-6)
 
 
+@pytest.mark.parametrize("cfg,n_events", [(1, 200), (3, 30)])
+def test_clone_killing(ds, orc_mlp, cfg, n_events):
+    """on events with doubled seeds, ds_reconstruct with clone_min_shared = 3 equals its own
+    S6 output with the oracle's clone list removed, slot by slot and bit for bit; ds_clone_kill alone does the same."""
+    d = gen.with_clone_seeds(gen.generate(cfg, n_events=n_events))
+    t0, _ = gpu_run(ds, d)                                          # clone killing off: the S6 / S7 records
+    killed = O.clone_kill(t0, d["seed_offsets"], P).astype(bool)
+    assert killed.sum() > 20 and not killed[t0["found"] == 0].any()
+    pk = dict(P, clone_min_shared=3)
+    t1, v1 = gpu_run(ds, d, params=pk)
+    exp = {k: v.copy() for k, v in t0.items()}
+    for k in ("x", "y", "tx", "ty", "qop", "chi2", "score"):
+        exp[k][killed] = 0.0
+    for k in ("nhits", "found", "keep"):
+        exp[k][killed] = 0
+    exp["hit"][killed] = -1
+    for k in exp:
+        assert np.array_equal(t1[k], exp[k]), k
+    # the vertices are those of the surviving tracks
+    ov = O.vertex(t1, d["seed_offsets"], G, pk)
+    assert v1["n"] == ov["n"] or ov["edge_pairs"]
+    parity.compare_vertices(v1, ov)
+    # standalone entry point on device-resident S6 / S7 records
+    ds.set_params(pk)
+    try:
+        dev = ds.to_device(t0)
+        so = ds.to_device(dict(s=d["seed_offsets"]))["s"]
+        t2 = to_host(ds.clone_kill(dev, so))
+    finally:
+        ds.set_params(P)
+    for k in exp:
+        assert np.array_equal(t2[k], exp[k]), k
+
+
 def test_vertexing_large_events_in_a_small_event_batch(ds, orc_mlp):
     """A few cfg3 events (~500 seeds, thousands of pairs) among many empty ones: the batch averages few seeds per event
     and takes the warp-per-event vertex kernels, whose staging capacity and pair mask these events exceed.  The same
