@@ -5,72 +5,91 @@
 // is a clone pair and its worse member -- larger chi2 + miss_penalty * (4 - nhits), ties: the later seed -- is removed;
 // every pair is judged on the tracks as S6 left them, so the result does not depend on an iteration order.
 //
-// One thread block per event: the (hit[4], score, found) records of the event's seeds are staged in shared memory, a
-// thread per track counts shared hits against every other found track (integer compares; the scores in fp64 from the
-// fp32 chi2 of the record), then the removed tracks are reset to the "not found" record (score and keep included).
+// One thread block per event: the (hit[4], score, seed index) records of the event's FOUND tracks are compacted into
+// shared memory (a handful out of ~150 seed slots), a thread per found track counts shared hits against every other one
+// (integer compares; the scores in fp64 from the fp32 chi2 of the record), then the removed tracks are reset to the "not
+// found" record (score and keep included).  Events with more found tracks than the staging holds are judged straight
+// from the records in two passes.
 #include "ds_common.cuh"
 
 namespace ds {
 
 constexpr int kCloneThreads = 128;
-constexpr int kCloneCap = 1024;   // seeds of an event staged in shared memory (24 B each)
+constexpr int kCloneCap = 1024;   // found tracks of an event staged in shared memory (28 B each)
+
+__device__ __forceinline__ int shared_hits(const int4 &a, const int4 &b)
+{
+    return (a.x >= 0 && a.x == b.x) + (a.y >= 0 && a.y == b.y) + (a.z >= 0 && a.z == b.z) + (a.w >= 0 && a.w == b.w);
+}
 
 __global__ void __launch_bounds__(kCloneThreads)
 k_clone(const __grid_constant__ DevConst c, const int32_t *__restrict__ seed_offsets, const ds_tracks trk)
 {
     __shared__ int4 s_hit[kCloneCap];
-    __shared__ double s_score[kCloneCap];   // < 0: no track in this slot
+    __shared__ double s_score[kCloneCap];
+    __shared__ int s_idx[kCloneCap];
+    __shared__ int n_found;
     const int e = blockIdx.x, tid = threadIdx.x;
     const int s0 = seed_offsets[e], n = seed_offsets[e + 1] - s0;
     if (n < 2) return;
-    const bool staged = n <= kCloneCap;
     const int4 *ghit = reinterpret_cast<const int4 *>(trk.hit) + s0;
-    auto score_of = [&](int i) {   // S6 score (A-9) of seed slot i, -1 if it holds no track
-        return trk.found[s0 + i] ? (double)trk.chi2[s0 + i] + c.miss_penalty * (double)(4 - trk.nhits[s0 + i]) : -1.0;
-    };
-    if (staged) {
-        for (int i = tid; i < n; i += kCloneThreads) {
-            s_hit[i] = ghit[i];
-            s_score[i] = score_of(i);
-        }
-        __syncthreads();
-    }
     const int min_shared = c.clone_min_shared;
-    constexpr unsigned kMark = 0x7fc0c10eu;   // a NaN payload no sigmoid produces: "removed", parked in score between the passes
+    auto score_of = [&](int i) {   // S6 score (A-9) of seed slot i
+        return (double)trk.chi2[s0 + i] + c.miss_penalty * (double)(4 - trk.nhits[s0 + i]);
+    };
     auto reset = [&](int64_t s) {
         trk.x[s] = 0.f; trk.y[s] = 0.f; trk.tx[s] = 0.f; trk.ty[s] = 0.f; trk.qop[s] = 0.f; trk.chi2[s] = 0.f;
         trk.score[s] = 0.f; trk.nhits[s] = 0; trk.found[s] = 0; trk.keep[s] = 0;
         reinterpret_cast<int4 *>(trk.hit)[s] = make_int4(-1, -1, -1, -1);
     };
-    for (int i0 = 0; i0 < n; i0 += kCloneThreads) {
-        const int i = i0 + tid;
-        bool killed = false;
-        if (i < n) {
-            const double si = staged ? s_score[i] : score_of(i);
-            if (si >= 0.0) {
-                const int4 hi = staged ? s_hit[i] : ghit[i];
-                for (int j = 0; j < n; ++j) {
-                    const double sj = staged ? s_score[j] : score_of(j);
-                    if (j == i || sj < 0.0) continue;
-                    const int4 hj = staged ? s_hit[j] : ghit[j];
-                    const int shared = (hi.x >= 0 && hi.x == hj.x) + (hi.y >= 0 && hi.y == hj.y) + (hi.z >= 0 && hi.z == hj.z) +
-                                       (hi.w >= 0 && hi.w == hj.w);
-                    if (shared >= min_shared && (sj < si || (sj == si && j < i))) killed = true;
-                }
+    if (tid == 0) n_found = 0;
+    __syncthreads();
+    for (int i = tid; i < n; i += kCloneThreads) {
+        if (trk.found[s0 + i]) {
+            const int pos = atomicAdd(&n_found, 1);   // any order: the tie-break uses the seed index kept in s_idx
+            if (pos < kCloneCap) {
+                s_idx[pos] = i;
+                s_hit[pos] = ghit[i];
+                s_score[pos] = score_of(i);
             }
         }
-        if (killed) {
-            // staged: the judgement reads the shared-memory copy, the record can go at once; else the records are what
-            // the other threads still read, so the track is only marked (in a field the judgement does not read)
-            if (staged) reset(s0 + i);
-            else trk.score[s0 + i] = __uint_as_float(kMark);
+    }
+    __syncthreads();
+    const int nf = n_found;
+    if (nf < 2) return;
+    if (nf <= kCloneCap) {
+        for (int a = tid; a < nf; a += kCloneThreads) {
+            const int4 ha = s_hit[a];
+            const double sa = s_score[a];
+            const int ia = s_idx[a];
+            bool killed = false;
+            for (int b = 0; b < nf; ++b) {
+                if (b == a || shared_hits(ha, s_hit[b]) < min_shared) continue;
+                const double sb = s_score[b];
+                if (sb < sa || (sb == sa && s_idx[b] < ia)) killed = true;
+            }
+            if (killed) reset(s0 + ia);   // the judgement reads the shared-memory copy: the record can go at once
         }
+        return;
     }
-    if (!staged) {
-        __syncthreads();
-        for (int i = tid; i < n; i += kCloneThreads)
-            if (__float_as_uint(trk.score[s0 + i]) == kMark) reset(s0 + i);
+    // more found tracks than the staging holds: judge from the records; a removed track is first only marked (in a field
+    // the judgement does not read), the records change after every thread has read them
+    constexpr unsigned kMark = 0x7fc0c10eu;   // a NaN payload no sigmoid produces
+    for (int i = tid; i < n; i += kCloneThreads) {
+        if (!trk.found[s0 + i]) continue;
+        const int4 hi = ghit[i];
+        const double si = score_of(i);
+        bool killed = false;
+        for (int j = 0; j < n; ++j) {
+            if (j == i || !trk.found[s0 + j] || shared_hits(hi, ghit[j]) < min_shared) continue;
+            const double sj = score_of(j);
+            if (sj < si || (sj == si && j < i)) killed = true;
+        }
+        if (killed) trk.score[s0 + i] = __uint_as_float(kMark);
     }
+    __syncthreads();
+    for (int i = tid; i < n; i += kCloneThreads)
+        if (__float_as_uint(trk.score[s0 + i]) == kMark) reset(s0 + i);
 }
 
 cudaError_t launch_clone(const DevConst &c, const int32_t *seed_offsets, int n_events, const ds_tracks &trk, cudaStream_t st,
