@@ -40,6 +40,9 @@ PARAMS = dict(
     magnet_polarity=0.0, gamma_c0=-1.5e-8, gamma_c1=9.3e-3, vtx_newton_iters=3,
     # clone killing across seeds: shared hits that make a clone pair; 0 = off (BASELINE configs)
     clone_min_shared=0,
+    # Dv1 triplet search (P:107-P:111): 1 = every UTbX hit of the y-compatible sectors starts a candidate
+    # and the UTaX hit is mandatory; 0 = Dv0 (first window, <= 10 closest), the BASELINE configurations
+    dv1=0,
 )
 
 # A-10: fixed input normalisation (mu, sigma) for [x, y, tx, ty, qop, chi2, qop_seed, chi2_seed]

@@ -60,7 +60,7 @@ typedef struct {
     double magnet_polarity;      /* MP of Eq. 3: +1 / -1; 0 = straight tracks (gamma = 0, A-20)      */
     double gamma_c0, gamma_c1;   /* gamma = -MP (c0 + c1 q/p[1/MeV]); paper: -1.5e-8, 9.3e-3 (Eq. 3, A-27)   */
     int32_t vtx_newton_iters;    /* Newton-Raphson iterations ("three")           (A-28)              */
-    int32_t pad2_;
+    int32_t dv1;                 /* 1: Dv1 triplet search (P:107-P:111); 0: Dv0         */
     double edge_rel;             /* relative margin below which a decision is "edge" (1e-5)          */
 } orc_params;
 
@@ -333,7 +333,7 @@ static void reconstruct_seed(const orc_geom *g, const orc_params *p, const orc_m
                              int32_t *found_out, int32_t *keep_out, int32_t *edge_out, double *margin_out)
 {
     double ex[12], zm, xm, txp, xc3, w0, w1, yl[4];
-    cand_hit F[64], C0[4], C1[4], C2[4];
+    cand_hit F64[64], *F = F64, C0[4], C1[4], C2[4];
     int nF, f, l, edge = 0, maxF = p->max_first_hits;
     double min_margin = 1e300, second_score = 1e300;
     const double eps = p->edge_rel;
@@ -347,8 +347,15 @@ static void reconstruct_seed(const orc_geom *g, const orc_params *p, const orc_m
     for (l = 0; l < 4; ++l) yl[l] = ex[3 + l];
     (void)txp;
 
-    /* O-S3: first window in UTbX (layer 3), up to 10 closest */
-    nF = window_search(g, p, nh, x0, ymin, ymax, id, 3, yl[3], xc3, w0, maxF, F, scratch, &edge, &min_margin);
+    if (!p->dv1) {
+        /* O-S3: first window in UTbX (layer 3), up to 10 closest */
+        nF = window_search(g, p, nh, x0, ymin, ymax, id, 3, yl[3], xc3, w0, maxF, F, scratch, &edge, &min_margin);
+    } else {
+        /* Dv1 (P:107-P:111; A-32): no first window that assumes a track from the origin -- every UTbX hit of the
+         * y-compatible sectors starts a triplet (UTbX hit, UTaX hit, magnet point) */
+        F = (cand_hit *)malloc(sizeof(cand_hit) * (size_t)(nh > 0 ? nh : 1));
+        nF = window_search(g, p, nh, x0, ymin, ymax, id, 3, yl[3], 0.0, 1e300, nh > 0 ? nh : 1, F, scratch, &edge, &min_margin);
+    }
 
     for (f = 0; f < nF; ++f) {
         /* O-S4: new trajectory from the hit position and the magnet point (Fig. 7) */
@@ -359,6 +366,7 @@ static void reconstruct_seed(const orc_geom *g, const orc_params *p, const orc_m
         double xp1 = xm + txc * (g->z_layer[1] - zm);
         double xp2 = xm + txc * (g->z_layer[2] - zm);
         n0 = window_search(g, p, nh, x0, ymin, ymax, id, 0, yl[0], xp0, w1, 1, C0, scratch, &edge, &min_margin);
+        if (p->dv1 && n0 == 0) continue;   /* Dv1: the triplet needs its UTaX hit collinear with UTbX hit and magnet point */
         n1 = window_search(g, p, nh, x0, ymin, ymax, id, 1, yl[1], xp1, w1, 2, C1, scratch, &edge, &min_margin);
         n2 = window_search(g, p, nh, x0, ymin, ymax, id, 2, yl[2], xp2, w1, 2, C2, scratch, &edge, &min_margin);
 
@@ -437,6 +445,7 @@ static void reconstruct_seed(const orc_geom *g, const orc_params *p, const orc_m
     }
     *edge_out = edge;
     *margin_out = min_margin;
+    if (F != F64) free(F);
 }
 
 /* ------------------------------------------------------------------------------------------------------------

@@ -33,7 +33,7 @@ class OrcParams(ct.Structure):
                 ("m_pi", ct.c_double), ("m_p", ct.c_double), ("m_ks", ct.c_double), ("m_lambda", ct.c_double),
                 ("dm_ks", ct.c_double), ("dm_lambda", ct.c_double), ("n2_min", ct.c_double),
                 ("magnet_polarity", ct.c_double), ("gamma_c0", ct.c_double), ("gamma_c1", ct.c_double),
-                ("vtx_newton_iters", ct.c_int32), ("pad2_", ct.c_int32), ("edge_rel", ct.c_double)]
+                ("vtx_newton_iters", ct.c_int32), ("dv1", ct.c_int32), ("edge_rel", ct.c_double)]
 
 
 class OrcMlp(ct.Structure):

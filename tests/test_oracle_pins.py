@@ -734,3 +734,76 @@ def test_p12_clone_kill_equals_set_arithmetic(orc_mlp):
     # a doubled true seed makes a clone pair of which one member goes: the found tracks return to the original count
     n0 = int(r0["found"].sum())
     assert k.sum() > 50 and abs(int(r["found"].sum()) - int(k.sum()) - n0) <= 0.05 * n0
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# P-13  Dv1 triplet search (P:107-P:111), reading A-32
+# ---------------------------------------------------------------------------------------------------------------
+PD = dict(P, dv1=1)
+
+
+def test_p13_dv1_noise_free_recovery(orc_mlp):
+    """cfg0 (no noise, no smearing): Dv1 finds the generated hits of every seed, as Dv0 does (P-1)."""
+    d = gen.generate(0)
+    r0, r1 = run(d, orc_mlp), O.reconstruct(d["hits"], d["hit_offsets"], d["seeds"], d["seed_offsets"], G, PD, orc_mlp)
+    assert r1["found"].all() and (r1["nhits"] == 4).all()
+    assert np.array_equal(r0["hit"], r1["hit"]) and np.allclose(r0["chi2"], r1["chi2"], atol=1e-6)
+
+
+def test_p13_dv1_finds_tracks_outside_the_first_window(orc_mlp):
+    """The point of Dv1: a track through the magnet point whose UT slope is not the one the first window assumes
+    (large opening angle).  Its UTbX hit lies 3 w0 off the window centre: Dv0 skips the seed, Dv1 builds the triplet
+    (UTbX hit, UTaX hit, magnet point) and the full track; without the UTaX hit there is no triplet and no track."""
+    seed = _one_seed()
+    ex, xs = _line_hits(seed)
+    x3 = xs[3] + 3.0 * ex["w0"]
+    rows = [(3, x3, ex["y_l"][3], 1)] + _partners(ex, x3)
+    h = _mk_hits(rows)
+    assert not O.reconstruct(h, [0, 4], seed, [0, 1], G, P, orc_mlp)["found"][0]
+    r = O.reconstruct(h, [0, 4], seed, [0, 1], G, PD, orc_mlp)
+    assert r["found"][0] and r["nhits"][0] == 4 and sorted(r["hit"][0].tolist()) == [0, 1, 2, 3] and r["chi2"][0] < 1e-6
+    tx_c = (x3 - ex["x_m"]) / (G["z_layer"][3] - ex["z_m"])
+    assert r["tx"][0] == pytest.approx(tx_c, rel=1e-5)
+    # no UTaX hit: Dv0 logic would accept UTbX + UTaU + UTbV (3 hits), the triplet search does not
+    no_ax = _mk_hits([rows[0], rows[2], rows[3]])
+    assert not O.reconstruct(no_ax, [0, 3], seed, [0, 1], G, PD, orc_mlp)["found"][0]
+    in_window = _mk_hits([(3, xs[3], ex["y_l"][3], 1)] + _partners(ex, xs[3])[1:])
+    assert O.reconstruct(in_window, [0, 3], seed, [0, 1], G, P, orc_mlp)["found"][0]
+    assert not O.reconstruct(in_window, [0, 3], seed, [0, 1], G, PD, orc_mlp)["found"][0]
+    # the UTaX hit must be collinear within w1
+    for f, ok in ((0.9, True), (1.1, False)):
+        rr = list(rows)
+        rr[1] = (0, rows[1][1] + f * ex["w1"], rows[1][2], rows[1][3])
+        assert bool(O.reconstruct(_mk_hits(rr), [0, 4], seed, [0, 1], G, dict(PD, chi2ndf_max=1e30), orc_mlp)["found"][0]) == ok
+
+
+def test_p13_dv1_only_y_compatible_sectors_and_no_cap(orc_mlp):
+    """"Each SciFi track searches only for hits within compatible Y sectors" (P:109-P:111); and there is no "10 closest"
+    cap: with 25 UTbX hits in the sector, the one that completes a triplet is found wherever it ranks in distance."""
+    seed = _one_seed()
+    ex, xs = _line_hits(seed)
+    x3 = xs[3] + 200.0
+    good = [(3, x3, ex["y_l"][3], 1)] + _partners(ex, x3)
+    noise = [(3, xs[3] + 4.0 * k, ex["y_l"][3], 200 + k) for k in range(-12, 13)]      # 25 hits nearer to the window centre
+    r = O.reconstruct(_mk_hits(good + noise), [0, len(good) + len(noise)], seed, [0, 1], G, PD, orc_mlp)
+    assert r["found"][0] and r["hit"][0, 3] == 0 and r["nhits"][0] == 4
+    # the same UTbX hit two sectors away in y is not looked at
+    far = [(3, x3, ex["y_l"][3] + 200.0, 1)] + _partners(ex, x3)
+    hf = _mk_hits(far)
+    hf["x0"][0] = x3
+    assert not O.reconstruct(hf, [0, 4], seed, [0, 1], G, PD, orc_mlp)["found"][0]
+
+
+def test_p13_dv1_superset_on_cfg1(orc_mlp):
+    """On cfg1 events: every Dv0 track with a UTaX hit is a Dv1 candidate, so Dv1 finds a track for that seed with a score
+    at least as good; Dv1 never returns a track without its UTaX and UTbX hits."""
+    d = gen.generate(1, n_events=8)
+    r0 = run(d, orc_mlp)
+    r1 = O.reconstruct(d["hits"], d["hit_offsets"], d["seeds"], d["seed_offsets"], G, PD, orc_mlp)
+    f1 = r1["found"] == 1
+    assert (r1["hit"][f1][:, 0] >= 0).all() and (r1["hit"][f1][:, 3] >= 0).all()
+    with_ax = (r0["found"] == 1) & (r0["hit"][:, 0] >= 0)
+    assert with_ax.sum() > 50 and f1[with_ax].all()
+    s0 = r0["chi2"].astype(np.float64) + P["miss_penalty"] * (4 - r0["nhits"])
+    s1 = r1["chi2"].astype(np.float64) + P["miss_penalty"] * (4 - r1["nhits"])
+    assert (s1[with_ax] <= s0[with_ax] + 1e-4).all()
