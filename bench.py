@@ -158,6 +158,8 @@ def run_reference(args, rank):
     from gen import constants as C
     if args.magnet_polarity != 0.0:
         C.PARAMS = dict(C.PARAMS, magnet_polarity=args.magnet_polarity)
+    if args.dv1:
+        C.PARAMS = dict(C.PARAMS, dv1=1)
     d = gen.generate(CFG, n_events=args.subbatch, workers=min(8, os.cpu_count() or 1))
     per_step = min(10.0, 150.0 / max(1, args.steps + args.warmup))
     n = sized_sample(d, per_step, args.subbatch)
@@ -194,6 +196,8 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--dv1", action="store_true",
+                    help="Dv1 triplet search instead of the Dv0 first window (SURVEY 8f N2, P:107-P:111) in both arms")
     ap.add_argument("--clone-min-shared", type=int, default=0,
                     help="3: clone killing across seeds between S6 and S7 (SURVEY 8f N3, P:115); 0 = BASELINE configs")
     ap.add_argument("--magnet-polarity", type=float, default=0.0,
@@ -210,6 +214,8 @@ def main():
     import gen
     if args.magnet_polarity != 0.0:   # both arms (the oracle legs read C.PARAMS) vertex with the parabolas of Eq. 4
         C.PARAMS = dict(C.PARAMS, magnet_polarity=args.magnet_polarity)
+    if args.dv1:
+        C.PARAMS = dict(C.PARAMS, dv1=1)
     if args.clone_min_shared:         # our arm only: the timed oracle legs have no clone-killing step
         C.PARAMS = dict(C.PARAMS, clone_min_shared=args.clone_min_shared)
     n_sub = max(1, args.events // args.subbatch)
@@ -400,7 +406,7 @@ def main():
                        "subbatches": n_sub, "events_per_subbatch": args.subbatch, "cuda_streams": n_streams,
                        "hits": sum(n_hits), "seeds": sum(n_seeds), "tracks_found": n_found, "tracks_kept": n_keep, "vertices": n_vtx,
                        "l2": "inputs larger than L2 (each sub-batch reads ~0.76 GB; 7.6 GB per step)",
-                       "magnet_polarity": args.magnet_polarity, "clone_min_shared": args.clone_min_shared,
+                       "magnet_polarity": args.magnet_polarity, "clone_min_shared": args.clone_min_shared, "dv1": bool(args.dv1),
                        "parallelism": f"dp{world} (events sharded, no data-path collective)"},
             "roofline": roofline, "whole_path_gbs": whole_gbs, "whole_path_frac": whole_gbs / peak, "kernels": kernels,
             "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,

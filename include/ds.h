@@ -100,6 +100,11 @@ typedef struct {
                                          least this many UT hits (same index, same layer) with a better track (smaller
                                          chi2 + miss_penalty*(4 - nhits), ties: earlier seed) are removed after S6;
                                          paper: 3 ("more than two"); 0 = off (the BASELINE configurations)              */
+    int32_t dv1;                      /* 1: Dv1 triplet search (P:107-P:111, A-32): no first window -- every UTbX hit of
+                                         the seed's y-compatible sectors starts a candidate, which needs a UTaX hit within
+                                         the refined window of the line through that hit and the magnet point; stereo
+                                         hits, fit and choice as Dv0.  0: Dv0 (the BASELINE configurations)               */
+    int32_t pad_;
 } ds_params;
 #define DS_MAX_FIRST_HITS 10
 

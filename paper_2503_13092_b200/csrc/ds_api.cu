@@ -72,6 +72,7 @@ bool make_const(const ds_geometry &g, const ds_params *p, DevConst &c)
     c.dm_ks = p->dm_ks; c.dm_lambda = p->dm_lambda; c.n2_min = p->n2_min;
     c.vtx_mp = p->magnet_polarity; c.gamma_c0 = p->gamma_c0; c.gamma_c1 = p->gamma_c1;
     c.vtx_iters = p->vtx_newton_iters; c.clone_min_shared = p->clone_min_shared;
+    c.dv1 = p->dv1 != 0; c.pad3_ = 0;
     return true;
 }
 

@@ -34,6 +34,7 @@ struct DevConst {
     double doca_max, zv_min, zv_max, m_pi, m_p, m_ks, m_lambda, dm_ks, dm_lambda, n2_min;
     double vtx_mp, gamma_c0, gamma_c1;   // curved-track vertexing: gamma = -vtx_mp * (gamma_c0 + gamma_c1 * qop / 1000)
     int vtx_iters, clone_min_shared;
+    int dv1, pad3_;
 };
 
 // Device copy of the ghost-killer weights (global memory, staged to shared memory by the kernel).

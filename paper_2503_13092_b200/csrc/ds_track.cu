@@ -128,7 +128,11 @@ struct WarpShared {
     unsigned long long best_bits[32];     // per seed: smallest score among its fits (bits of the non-negative double)
     int best_fit[32];                     // per seed: first fit task with that score
     int n_best[32];                       // per seed: fits with that score (+ 2 for every first hit left to the seed's thread)
+    int dv_off[32], dv_a[32];             // Dv1: first item and first UTbX candidate of the seed
+    // Dv1 keeps at most kFirstCap triplets in slot[]; the rest of it holds the fit queue (4 per triplet)
+    __device__ __forceinline__ unsigned short *dv_task_ptr() { return reinterpret_cast<unsigned short *>(slot + kFirstCap); }
 };
+static_assert((32 * kMaxFirst - kFirstCap) * 2 >= 4 * kFirstCap * 2, "slot[] holds the Dv1 triplets and their fit queue");
 
 // Block-shared state of k_track (carved from dynamic shared memory, followed by the staged hit arrays).
 template <typename Idx>
@@ -614,20 +618,259 @@ __device__ __forceinline__ void track_chunk(const DevConst &c, WarpShared<Idx> &
     }
 }
 
-// All seeds of one event: every warp of the block takes an equal share (at most 32 at a time).
+// ---- Dv1 (P:107-P:111, reading A-32): triplet search ---------------------------------------------------
+// No first window: every UTbX hit of the seed's y-compatible sectors starts a candidate, and the candidate needs a UTaX
+// hit collinear (within w1) with that hit and the magnet point -- the triplet.  The sectors s_lo..s_hi of UTbX are one
+// contiguous range of the sorted slice, so a seed's candidates are (range start, count); the warp walks the items
+// (seed, UTbX hit) of its <= 32 seeds 32 at a time:
+//   T  lane per item: y-compatibility of the UTbX hit, trajectory through it and the magnet point, UTaX search;
+//      items with a UTaX hit are compacted into the triplet list (the first-hit list of Dv0, filled by ballots)
+//   whenever >= 32 triplets wait (and at the end):
+//   S  two lanes per triplet, UTaU / UTbV searches (closest 2); the lane of UTaU queues the <= 4 fits
+//   F  lane per queued fit, 32 at a time; per seed the best fit of the window (atomicMin on the score bits) is compared
+//      by the seed's lane with the best candidate it holds so far (exact ties: full (hits, ids) comparison)
+// and each seed's lane writes its track record at the end.
 template <typename Idx>
+__device__ __forceinline__ Candidate make_candidate(const WarpShared<Idx> &sh, const FitRes &r, int tk)
+{
+    const int f = tk & 511, i1 = (tk >> 9) & 1, i2 = (tk >> 10) & 1;
+    Candidate cand;
+    cand.score = r.score; cand.a = r.a; cand.b = r.b; cand.chi2 = r.chi2;
+    cand.j0 = idx_get(sh.near[3 * f][0]);
+    cand.j1 = idx_get(sh.near[3 * f + 1][i1]);
+    cand.j2 = idx_get(sh.near[3 * f + 2][i2]);
+    cand.j3 = (int)sh.slot[f];
+    cand.nh = 1 + (cand.j0 >= 0) + (cand.j1 >= 0) + (cand.j2 >= 0);
+    return cand;
+}
+
+template <typename Idx>
+__device__ __forceinline__ FitRes fit_task(const DevConst &c, const WarpShared<Idx> &sh, const EventHits &H, int tk)
+{
+    const int f = tk & 511, i1 = (tk >> 9) & 1, i2 = (tk >> 10) & 1;
+    const float2 zw = sh.zw3[f];
+    return fit_combo(c, H, sh.rec[sh.fs[f]], idx_get(sh.near[3 * f][0]), idx_get(sh.near[3 * f + 1][i1]),
+                     idx_get(sh.near[3 * f + 2][i2]), (int)sh.slot[f], (double)zw.x, (double)zw.y);
+}
+
+// S + F for the triplets [0, n_trip) of the warp's list (fs = owner lane, slot = UTbX hit, near[3f] = UTaX hit, zw3);
+// `best` is the candidate the calling lane's seed holds so far.
+template <typename Idx>
+__device__ __forceinline__ void dv1_flush(const DevConst &c, WarpShared<Idx> &sh, const Idx *tab, const EventHits &H,
+                                          int n_trip, Candidate &best)
+{
+    const unsigned FULL = 0xffffffffu;
+    const int lane = threadIdx.x & 31;
+    if (lane == 0) sh.n_fit = 0;
+    __syncwarp();
+    // ---- S: stereo layers, two lanes per triplet ---------------------------------------------------------------------------
+    for (int fb = 0; fb < n_trip; fb += 16) {
+        const int g = lane >> 1, l = 1 + (lane & 1);
+        const int f = fb + g;
+        const bool on = f < n_trip;
+        int2 r = make_int2(-1, -1);
+        if (on) {
+            const SeedRec &t2 = sh.rec[sh.fs[f]];
+            const int j3 = (int)sh.slot[f];
+            const double x3 = (double)H.x0[j3] + c.dxdy[3] * t2.y[3];
+            const double txc = (x3 - t2.xm) / ((double)sh.zw3[f].x - t2.zm);
+            const double xp = t2.xm + txc * (c.z_layer[l] - t2.zm);
+            r = search_layer(c, H, tab, l, xp, t2.y[l], t2.w1, (int)t2.sec[l][0], (int)t2.sec[l][1]);
+            sh.near[3 * f + l][0] = (Idx)r.x;
+            sh.near[3 * f + l][1] = (Idx)r.y;
+        }
+        const unsigned has1 = __ballot_sync(FULL, r.x >= 0), has2 = __ballot_sync(FULL, r.y >= 0);
+        if (on && l == 1) {
+            const int nh = 2 + ((has1 >> (2 * g)) & 1) + ((has1 >> (2 * g + 1)) & 1);   // UTbX + UTaX + stereo hits
+            if (nh >= c.min_hits) {
+                const int m1 = 1 + ((has2 >> (2 * g)) & 1), m2 = 1 + ((has2 >> (2 * g + 1)) & 1);
+                const int base = atomicAdd(&sh.n_fit, m1 * m2);
+                for (int i1 = 0; i1 < m1; ++i1)
+                    for (int i2 = 0; i2 < m2; ++i2)
+                        sh.dv_task_ptr()[base + i1 * m2 + i2] = (unsigned short)(f | (i1 << 9) | (i2 << 10));
+            }
+        }
+    }
+    __syncwarp();
+    // ---- F: fits, 32 at a time; per seed the best of the window against the seed's best so far ---------------------------------
+    const int n_fit = sh.n_fit;
+    for (int tb = 0; tb < n_fit; tb += 32) {
+        sh.best_bits[lane] = (unsigned long long)__double_as_longlong(kNoScore);
+        sh.best_fit[lane] = INT32_MAX;
+        sh.n_best[lane] = 0;
+        __syncwarp();
+        const int t = tb + lane;
+        unsigned long long bits = (unsigned long long)__double_as_longlong(kNoScore);
+        int o = 0, tk = 0;
+        FitRes r;
+        r.score = kNoScore;
+        if (t < n_fit) {
+            tk = sh.dv_task_ptr()[t];
+            o = sh.fs[tk & 511];
+            r = fit_task<Idx>(c, sh, H, tk);
+            if (r.score != kNoScore) {
+                bits = (unsigned long long)__double_as_longlong(r.score);
+                atomicMin(&sh.best_bits[o], bits);
+            }
+        }
+        __syncwarp();
+        const bool top = t < n_fit && r.score != kNoScore && bits == sh.best_bits[o];
+        if (top) {
+            atomicMin(&sh.best_fit[o], lane);
+            atomicAdd(&sh.n_best[o], 1);
+        }
+        __syncwarp();
+        if (top && sh.best_fit[o] == lane) sh.res[o] = r;   // the window's best fit of seed o (first of equal ones)
+        __syncwarp();
+        const int nb = sh.n_best[lane];
+        if (nb == 1) {
+            const Candidate cand = make_candidate<Idx>(sh, sh.res[lane], sh.dv_task_ptr()[tb + sh.best_fit[lane]]);
+            if (cand.score < best.score || (cand.score == best.score && tie_better(H, cand, best))) best = cand;
+        } else if (nb >= 2) {   // equal scores inside the window: every fit of this seed once more, full comparison
+            for (int q = tb; q < min(tb + 32, n_fit); ++q) {
+                const int tq = sh.dv_task_ptr()[q];
+                if (sh.fs[tq & 511] != lane) continue;
+                const FitRes rq = fit_task<Idx>(c, sh, H, tq);
+                if (rq.score == kNoScore) continue;
+                const Candidate cand = make_candidate<Idx>(sh, rq, tq);
+                if (cand.score < best.score || (cand.score == best.score && tie_better(H, cand, best))) best = cand;
+            }
+        }
+        __syncwarp();
+    }
+}
+
+// Seeds [cb, ce) (at most 32) of one event with the Dv1 triplet search, by one warp on its own.
+template <typename Idx>
+__device__ __forceinline__ void track_chunk_dv1(const DevConst &c, WarpShared<Idx> &sh, const Idx *tab, const EventHits &H,
+                                                const ds_seeds &seeds, int cb, int ce, const ds_tracks &out)
+{
+    const unsigned FULL = 0xffffffffu;
+    const int lane = threadIdx.x & 31;
+    const int s = cb + lane;
+    const bool act = s < ce;
+    // ---- per seed: S2 and the range of its UTbX candidates ----------------------------------------------------------------------
+    float fy = 0.f, ftx = 0.f, fty = 0.f;
+    int a_o = 0, n_o = 0;
+    if (act) {
+        const float fx = seeds.x[s], fq = seeds.qop[s];
+        fy = seeds.y[s]; ftx = seeds.tx[s]; fty = seeds.ty[s];
+        const S2 s2 = extrapolate_seed(c, fx, fy, ftx, fty, fq);
+        SeedRec &r = sh.rec[lane];
+        r.xm = s2.xm; r.zm = s2.zm; r.w1 = s2.w1;
+        r.y[0] = s2.y0; r.y[1] = s2.y1; r.y[2] = s2.y2; r.y[3] = s2.y3;
+#pragma unroll
+        for (int l = 0; l < 3; ++l) {
+            int tl, th;
+            sector_range(c, l == 0 ? s2.y0 : (l == 1 ? s2.y1 : s2.y2), tl, th);
+            r.sec[l][0] = (unsigned char)(th < tl ? 1 : tl);
+            r.sec[l][1] = (unsigned char)(th < tl ? 0 : th);
+        }
+        int s_lo, s_hi;
+        sector_range(c, s2.y3, s_lo, s_hi);
+        if (s_lo <= s_hi) {   // the sectors of a layer follow each other in the sorted slice: one range
+            a_o = (int)tab[(3 * c.n_sectors + s_lo) * kXBins];
+            n_o = (int)tab[(3 * c.n_sectors + s_hi + 1) * kXBins] - a_o;
+        }
+    }
+    int incl = n_o;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const int t = __shfl_up_sync(FULL, incl, d);
+        if (lane >= d) incl += t;
+    }
+    const int total = __shfl_sync(FULL, incl, 31);
+    sh.dv_off[lane] = incl - n_o;
+    sh.dv_a[lane] = a_o;
+    __syncwarp();
+
+    Candidate best;
+    best.score = kNoScore; best.a = 0.0; best.b = 0.0; best.chi2 = 0.0;
+    best.nh = 0; best.j0 = -1; best.j1 = -1; best.j2 = -1; best.j3 = -1;
+    int n_trip = 0;
+    // ---- T: lane per item (seed, UTbX hit) -----------------------------------------------------------------------------------------
+    for (int t0 = 0; t0 < total; t0 += 32) {
+        const int t = t0 + lane;
+        bool has = false;
+        int o = 0, j3 = 0, j0 = -1;
+        float z3 = 0.f;
+        if (t < total) {
+            int lo = 0, hi = 32;   // last seed whose first item is <= t (seeds without items share the offset of the next)
+            while (hi - lo > 1) {
+                const int mid = (lo + hi) >> 1;
+                if (sh.dv_off[mid] <= t) lo = mid; else hi = mid;
+            }
+            o = lo;
+            j3 = sh.dv_a[o] + (t - sh.dv_off[o]);
+            const SeedRec &t2 = sh.rec[o];
+            if (y_compatible(c, H, j3, t2.y[3])) {
+                z3 = H.z[j3];
+                const double x3 = (double)H.x0[j3] + c.dxdy[3] * t2.y[3];
+                const double txc = (x3 - t2.xm) / ((double)z3 - t2.zm);
+                const double xp = t2.xm + txc * (c.z_layer[0] - t2.zm);
+                j0 = search_layer(c, H, tab, 0, xp, t2.y[0], t2.w1, (int)t2.sec[0][0], (int)t2.sec[0][1]).x;
+                has = j0 >= 0;
+            }
+        }
+        const unsigned m = __ballot_sync(FULL, has);
+        if (m == 0) continue;
+        if (has) {
+            const int f = n_trip + __popc(m & lanemask_lt());
+            sh.fs[f] = (unsigned short)o;
+            sh.slot[f] = (Idx)j3;
+            sh.near[3 * f][0] = (Idx)j0;
+            sh.near[3 * f][1] = (Idx)-1;
+            sh.zw3[f] = make_float2(z3, H.w[j3]);
+        }
+        n_trip += __popc(m);
+        if (n_trip >= 32) {   // the list holds 64: room for one more round of items is guaranteed after this
+            dv1_flush<Idx>(c, sh, tab, H, n_trip, best);
+            n_trip = 0;
+        }
+    }
+    if (n_trip > 0) dv1_flush<Idx>(c, sh, tab, H, n_trip, best);
+    // ---- track record ------------------------------------------------------------------------------------------------------------
+    if (act) {
+        if (best.score == kNoScore) {
+            write_not_found(out, s);
+        } else {
+            const double ys = (double)fy, txs = (double)ftx, tys = (double)fty;
+            out.x[s] = (float)best.a;
+            out.y[s] = (float)(ys + tys * (c.z_ref - c.z_seed));
+            out.tx[s] = (float)best.b;
+            out.ty[s] = (float)tys;
+            out.qop[s] = (float)((txs - best.b) / c.kick);
+            out.chi2[s] = (float)best.chi2;
+            out.nhits[s] = best.nh;
+            out.found[s] = 1;
+            int4 hv;
+            hv.x = best.j0 >= 0 ? H.perm[best.j0] : -1;
+            hv.y = best.j1 >= 0 ? H.perm[best.j1] : -1;
+            hv.z = best.j2 >= 0 ? H.perm[best.j2] : -1;
+            hv.w = H.perm[best.j3];
+            reinterpret_cast<int4 *>(out.hit)[s] = hv;
+        }
+    }
+    __syncwarp();   // the lists are rewritten by the warp's next chunk
+}
+
+// All seeds of one event: every warp of the block takes an equal share (at most 32 at a time).
+template <typename Idx, bool kDv1>
 __device__ __forceinline__ void track_event(const DevConst &c, TrackShared<Idx> &sh, const EventHits &H,
                                             const ds_seeds &seeds, int s_begin, int s_end, const ds_tracks &out)
 {
     const int wid = threadIdx.x >> 5;
     const int chunk = min(32, (s_end - s_begin + kTrackWarps - 1) / kTrackWarps);
-    for (int cb = s_begin + wid * chunk; cb < s_end; cb += kTrackWarps * chunk)
-        track_chunk<Idx>(c, sh.warp[wid], sh.tab, H, seeds, cb, min(cb + chunk, s_end), out);
+    for (int cb = s_begin + wid * chunk; cb < s_end; cb += kTrackWarps * chunk) {
+        if (kDv1) track_chunk_dv1<Idx>(c, sh.warp[wid], sh.tab, H, seeds, cb, min(cb + chunk, s_end), out);
+        else track_chunk<Idx>(c, sh.warp[wid], sh.tab, H, seeds, cb, min(cb + chunk, s_end), out);
+    }
 }
 
 #ifndef DS_TRACK_MINBLOCKS
 #define DS_TRACK_MINBLOCKS 3
 #endif
+template <bool kDv1>
 __global__ void __launch_bounds__(kTrackThreads, DS_TRACK_MINBLOCKS)
 k_track(const __grid_constant__ DevConst c, const LayoutPtrs L, const ds_seeds seeds,
         const int32_t *__restrict__ hit_offsets, const int32_t *__restrict__ seed_offsets, const ds_tracks out, int cap)
@@ -681,10 +924,10 @@ k_track(const __grid_constant__ DevConst c, const LayoutPtrs L, const ds_seeds s
         mbar_wait(bar, 0);
         const int d = h0 - h0a;
         H.x0 = st_x0 + d; H.ymin = st_ymin + d; H.ymax = st_ymax + d;
-        track_event<uint16_t>(c, *reinterpret_cast<Staged *>(smem_raw), H, seeds, s_begin, s_end, out);
+        track_event<uint16_t, kDv1>(c, *reinterpret_cast<Staged *>(smem_raw), H, seeds, s_begin, s_end, out);
     } else {
         H.x0 = L.sx0 + h0; H.ymin = L.symin + h0; H.ymax = L.symax + h0;
-        track_event<int>(c, *reinterpret_cast<Direct *>(smem_raw), H, seeds, s_begin, s_end, out);
+        track_event<int, kDv1>(c, *reinterpret_cast<Direct *>(smem_raw), H, seeds, s_begin, s_end, out);
     }
 }
 
@@ -705,15 +948,19 @@ cudaError_t launch_track(const DevConst &c, const LayoutPtrs &lay, const ds_seed
     if (smem < sizeof(TrackShared<int>)) smem = sizeof(TrackShared<int>);   // the layout of an event that is not staged
     // opt in to the full 227 KB of dynamic shared memory; per device, cheap and the same value for every caller, so it is
     // simply set at every launch (handles on several devices and host threads share this code)
-    cudaFuncAttributes fa;
-    cudaError_t aerr = cudaFuncGetAttributes(&fa, k_track);
-    if (aerr != cudaSuccess) return aerr;
-    aerr = cudaFuncSetAttribute(k_track, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - (int)fa.sharedSizeBytes);
-    if (aerr != cudaSuccess) return aerr;
-    prof.begin(DS_K_TRACK, st);
-    k_track<<<n_events, kTrackThreads, smem, st>>>(c, lay, seeds, hit_offsets, seed_offsets, out, cap);
-    prof.end(st);
-    return cudaGetLastError();
+    auto launch = [&](auto kernel) -> cudaError_t {
+        cudaFuncAttributes fa;
+        cudaError_t aerr = cudaFuncGetAttributes(&fa, kernel);
+        if (aerr != cudaSuccess) return aerr;
+        aerr = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - (int)fa.sharedSizeBytes);
+        if (aerr != cudaSuccess) return aerr;
+        prof.begin(DS_K_TRACK, st);
+        kernel<<<n_events, kTrackThreads, smem, st>>>(c, lay, seeds, hit_offsets, seed_offsets, out, cap);
+        prof.end(st);
+        return cudaGetLastError();
+    };
+    // Dv1 (triplet search, P:107-P:111) and Dv0 are separate instantiations: the Dv0 hot path carries none of the other's code
+    return c.dv1 ? launch(k_track<true>) : launch(k_track<false>);
 }
 
 }  // namespace ds

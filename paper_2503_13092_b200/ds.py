@@ -49,7 +49,7 @@ class DsParams(ct.Structure):
                 ("zv_max", ct.c_double), ("m_pi", ct.c_double), ("m_p", ct.c_double), ("m_ks", ct.c_double),
                 ("m_lambda", ct.c_double), ("dm_ks", ct.c_double), ("dm_lambda", ct.c_double), ("n2_min", ct.c_double),
                 ("magnet_polarity", ct.c_double), ("gamma_c0", ct.c_double), ("gamma_c1", ct.c_double),
-                ("vtx_newton_iters", ct.c_int32), ("clone_min_shared", ct.c_int32)]
+                ("vtx_newton_iters", ct.c_int32), ("clone_min_shared", ct.c_int32), ("dv1", ct.c_int32), ("pad_", ct.c_int32)]
 
 
 class DsHits(ct.Structure):

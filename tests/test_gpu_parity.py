@@ -389,6 +389,18 @@ def test_curved_track_vertexing(ds, orc_mlp, cfg, n_events, mp):
     assert v1["n"] == v0["n"] and np.array_equal(v1["ia"], v0["ia"]) and np.allclose(v1["z"], v0["z"], rtol=1e-6)
 
 
+@pytest.mark.parametrize("cfg,n_events,hint", [(0, 10, 0), (1, 80, 0), (3, 12, 0), (2, 8, 0), (2, 8, 12288)])
+def test_dv1_triplet_search(ds, orc_mlp, cfg, n_events, hint):
+    """SURVEY §8f N2 (P:107-P:111, A-32): no first window, every UTbX hit of the y-compatible sectors, mandatory collinear
+    UTaX hit -- staged events, events above the staging capacity (cfg2 with the default hint) and many seeds (cfg3)."""
+    d = gen.generate(cfg, n_events=n_events)
+    pd = dict(P, dv1=1, max_event_hits_hint=hint)
+    st, sv, t, v = check_both(ds, d, orc_mlp, params=pd)
+    assert st["found"] > 0 and (t["hit"][t["found"] == 1][:, [0, 3]] >= 0).all()
+    t0, _ = gpu_run(ds, d, params=dict(P, max_event_hits_hint=hint))
+    print(f"cfg{cfg}: Dv1 finds {int(t['found'].sum())} tracks, Dv0 {int(t0['found'].sum())}; {st}")
+
+
 @pytest.mark.parametrize("cfg,n_events", [(1, 200), (3, 30)])
 def test_clone_killing(ds, orc_mlp, cfg, n_events):
     """on events with doubled seeds, ds_reconstruct with clone_min_shared = 3 equals its own
