@@ -648,9 +648,9 @@ template <typename Idx>
 __device__ __forceinline__ FitRes fit_task(const DevConst &c, const WarpShared<Idx> &sh, const EventHits &H, int tk)
 {
     const int f = tk & 511, i1 = (tk >> 9) & 1, i2 = (tk >> 10) & 1;
-    const float2 zw = sh.zw3[f];
+    const int j3 = (int)sh.slot[f];
     return fit_combo(c, H, sh.rec[sh.fs[f]], idx_get(sh.near[3 * f][0]), idx_get(sh.near[3 * f + 1][i1]),
-                     idx_get(sh.near[3 * f + 2][i2]), (int)sh.slot[f], (double)zw.x, (double)zw.y);
+                     idx_get(sh.near[3 * f + 2][i2]), j3, (double)sh.zw3[f].x, (double)H.w[j3]);
 }
 
 // S + F for the triplets [0, n_trip) of the warp's list (fs = owner lane, slot = UTbX hit, near[3f] = UTaX hit, zw3);
@@ -789,22 +789,26 @@ __device__ __forceinline__ void track_chunk_dv1(const DevConst &c, WarpShared<Id
     best.nh = 0; best.j0 = -1; best.j1 = -1; best.j2 = -1; best.j3 = -1;
     int n_trip = 0;
     // ---- T: lane per item (seed, UTbX hit) -----------------------------------------------------------------------------------------
+    // item t -> (seed, UTbX hit); z of the hit comes from global memory and is fetched one round ahead
+    auto item = [&](int t, int &o, int &j3, float &z3) {
+        // last seed whose first item is <= t (seeds without items share the offset of the next); a lane's items only go up
+        while (o < 31 && sh.dv_off[o + 1] <= t) ++o;
+        j3 = sh.dv_a[o] + (t - sh.dv_off[o]);
+        z3 = H.z[j3];
+    };
+    int o_nx = 0, j3_nx = 0;
+    float z3_nx = 0.f;
+    if (lane < total) item(lane, o_nx, j3_nx, z3_nx);
     for (int t0 = 0; t0 < total; t0 += 32) {
         const int t = t0 + lane;
         bool has = false;
-        int o = 0, j3 = 0, j0 = -1;
-        float z3 = 0.f;
+        const int o = o_nx, j3 = j3_nx;
+        const float z3 = z3_nx;
+        int j0 = -1;
+        if (t + 32 < total) item(t + 32, o_nx, j3_nx, z3_nx);
         if (t < total) {
-            int lo = 0, hi = 32;   // last seed whose first item is <= t (seeds without items share the offset of the next)
-            while (hi - lo > 1) {
-                const int mid = (lo + hi) >> 1;
-                if (sh.dv_off[mid] <= t) lo = mid; else hi = mid;
-            }
-            o = lo;
-            j3 = sh.dv_a[o] + (t - sh.dv_off[o]);
             const SeedRec &t2 = sh.rec[o];
             if (y_compatible(c, H, j3, t2.y[3])) {
-                z3 = H.z[j3];
                 const double x3 = (double)H.x0[j3] + c.dxdy[3] * t2.y[3];
                 const double txc = (x3 - t2.xm) / ((double)z3 - t2.zm);
                 const double xp = t2.xm + txc * (c.z_layer[0] - t2.zm);
@@ -820,7 +824,7 @@ __device__ __forceinline__ void track_chunk_dv1(const DevConst &c, WarpShared<Id
             sh.slot[f] = (Idx)j3;
             sh.near[3 * f][0] = (Idx)j0;
             sh.near[3 * f][1] = (Idx)-1;
-            sh.zw3[f] = make_float2(z3, H.w[j3]);
+            sh.zw3[f] = make_float2(z3, 0.f);   // w of the UTbX hit is read by the fit
         }
         n_trip += __popc(m);
         if (n_trip >= 32) {   // the list holds 64: room for one more round of items is guaranteed after this
