@@ -371,6 +371,11 @@ def test_empty_and_ragged_inputs(ds, orc_mlp):
     z = dict(d2, hits={k: v[:0] for k, v in hits.items()}, hit_offsets=np.zeros(10, np.int32))
     t0, v0 = gpu_run(ds, z)
     assert not t0["found"].any() and v0["n"] == 0
+    # the "next" rows on the same ragged events: Dv1 search, clone killing, curved-track vertexing together
+    check_both(ds, d2, orc_mlp, params=dict(P, dv1=1, magnet_polarity=1.0))
+    t1, _ = gpu_run(ds, d2, params=dict(P, dv1=1, clone_min_shared=3))
+    t2, _ = gpu_run(ds, z, params=dict(P, dv1=1, clone_min_shared=3, magnet_polarity=-1.0))
+    assert not t2["found"].any() and t1["found"].sum() > 0
 
 
 @pytest.mark.parametrize("cfg,n_events,mp", [(1, 300, 1.0), (1, 300, -1.0), (3, 40, 1.0)])
@@ -470,7 +475,10 @@ def test_duplicate_hits_and_ties(ds, orc_mlp):
         for k in hits:
             hits[k][ho[e]:ho[e + 1]] = hits[k][p]
     assert n * 2 == ho[-1]
-    check_both(ds, dict(d, hits=hits, hit_offsets=ho), orc_mlp)
+    d2 = dict(d, hits=hits, hit_offsets=ho)
+    check_both(ds, d2, orc_mlp)
+    # the same in the Dv1 triplet search: equal scores inside a fit window go through its full (hits, ids) comparison
+    check_both(ds, d2, orc_mlp, params=dict(P, dv1=1))
 
 
 def test_dense_window_more_than_ten_first_hits(ds, orc_mlp):
