@@ -504,32 +504,32 @@ __device__ __forceinline__ void track_chunk(const DevConst &c, WarpShared<Idx> &
             }
         }
         __syncwarp();
-        // ---- phase B: three lanes per first hit, one per layer -- S4; lane 0 of the three queues the fits ----------------
-        for (int fb = 0; fb < n_first; fb += 10) {
-            const int g = lane / 3, l = lane - 3 * g;
-            const int f = fb + g;
-            const bool on = lane < 30 && f < n_first;
-            int2 r = make_int2(-1, -1);
-            if (on) {
+        // ---- phase B: lane per first hit -- S4 in UTaX, UTaU, UTbV one after the other; the lane queues the fits --------------
+        for (int fb = 0; fb < n_first; fb += 32) {
+            const int f = fb + lane;
+            if (f < n_first) {
                 const int sl = sh.fs[f], o = sl / kMaxFirst;
                 const int j3 = (int)sh.slot[sl];
                 const SeedRec &t2 = sh.rec[o];
-                // trajectory through (first hit, magnet point), refined window in layer l
+                // trajectory through (first hit, magnet point), refined windows
                 const double x3 = (double)H.x0[j3] + c.dxdy[3] * t2.y[3];
                 const double txc = (x3 - t2.xm) / ((double)sh.zw3[f].x - t2.zm);
-                const double xp = t2.xm + txc * (c.z_layer[l] - t2.zm);
-                r = search_layer(c, H, tab, l, xp, t2.y[l], t2.w1, (int)t2.sec[l][0], (int)t2.sec[l][1]);
-                if (l == 0) r.y = -1;   // UTaX keeps the closest hit only
-                sh.near[3 * f + l][0] = (Idx)r.x;
-                sh.near[3 * f + l][1] = (Idx)r.y;
-            }
-            const int g3 = min(3 * g, 29);
-            const unsigned has1 = __ballot_sync(FULL, r.x >= 0), has2 = __ballot_sync(FULL, r.y >= 0);
-            if (on && l == 0) {
-                const int nh = 1 + ((has1 >> g3) & 1) + ((has1 >> (g3 + 1)) & 1) + ((has1 >> (g3 + 2)) & 1);
+                int2 r[3];
+#pragma unroll
+                for (int l = 0; l < 3; ++l) {
+                    const double xp = t2.xm + txc * (c.z_layer[l] - t2.zm);
+                    r[l] = search_layer(c, H, tab, l, xp, t2.y[l], t2.w1, (int)t2.sec[l][0], (int)t2.sec[l][1]);
+                }
+                r[0].y = -1;   // UTaX keeps the closest hit only
+#pragma unroll
+                for (int l = 0; l < 3; ++l) {
+                    sh.near[3 * f + l][0] = (Idx)r[l].x;
+                    sh.near[3 * f + l][1] = (Idx)r[l].y;
+                }
+                const int nh = 1 + (r[0].x >= 0) + (r[1].x >= 0) + (r[2].x >= 0);
                 unsigned short ff = kFitNone;
                 if (nh >= c.min_hits) {
-                    const int m1 = 1 + ((has2 >> (g3 + 1)) & 1), m2 = 1 + ((has2 >> (g3 + 2)) & 1);
+                    const int m1 = r[1].y >= 0 ? 2 : 1, m2 = r[2].y >= 0 ? 2 : 1;
                     const int base = atomicAdd(&sh.n_fit, m1 * m2);
                     if (base + m1 * m2 <= kFitCap) {
                         ff = (unsigned short)(base | ((m1 * m2) << 12));
@@ -539,7 +539,7 @@ __device__ __forceinline__ void track_chunk(const DevConst &c, WarpShared<Idx> &
                     } else {
                         ff = kFitInline;
                         atomicMin(&sh.fit_end, base);
-                        atomicAdd(&sh.n_best[sh.fs[f] / kMaxFirst], 2);
+                        atomicAdd(&sh.n_best[o], 2);
                     }
                 }
                 sh.ffit[f] = ff;
