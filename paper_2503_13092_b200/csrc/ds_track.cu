@@ -154,6 +154,10 @@ struct EventHits {
 template <typename Idx>
 __device__ __forceinline__ int idx_get(Idx v) { return v == (Idx)-1 ? -1 : (int)v; }
 
+// z, w, id and perm of a hit live in global memory and are read only for hits that passed a window -- a phase later than
+// the window test that picked them.  The test issues an L1 prefetch so that the later read does not wait on DRAM.
+__device__ __forceinline__ void prefetch_l1(const void *p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
+
 // y-compatibility of hit j (O-S3: ymin - y_tol <= y <= ymax + y_tol); no short circuit: both loads are always issued
 __device__ __forceinline__ bool y_compatible(const DevConst &c, const EventHits &H, int j, double y)
 {
@@ -384,6 +388,21 @@ __device__ __noinline__ Candidate choose_general(const DevConst &c, const WarpSh
     return best;
 }
 
+// A lane's seed state, read before the block waits for its table and hits (the loads overlap that wait)
+struct SeedPre {
+    float x, y, tx, ty, qop;
+    int s;   // the seed these values belong to, -1 = none
+};
+
+__device__ __forceinline__ SeedPre load_seed(const ds_seeds &seeds, int s, bool valid)
+{
+    SeedPre p;
+    p.s = valid ? s : -1;
+    p.x = valid ? seeds.x[s] : 0.f; p.y = valid ? seeds.y[s] : 0.f; p.tx = valid ? seeds.tx[s] : 0.f;
+    p.ty = valid ? seeds.ty[s] : 0.f; p.qop = valid ? seeds.qop[s] : 0.f;
+    return p;
+}
+
 // Seeds [cb, ce) (at most 32) of one event, by one warp on its own: rounds of
 //   A  lane per seed:       S2, first window in UTbX (S3) -> the seed's <= max_first first hits; warp scan of the counts
 //   B  three lanes per first hit, one per layer: refined windows (S4); the first lane of the three queues the fits
@@ -392,7 +411,7 @@ __device__ __noinline__ Candidate choose_general(const DevConst &c, const WarpSh
 // A round takes the longest prefix of the remaining seeds whose first hits fit the warp's list.
 template <typename Idx>
 __device__ __forceinline__ void track_chunk(const DevConst &c, WarpShared<Idx> &sh, const Idx *tab, const EventHits &H,
-                                            const ds_seeds &seeds, int cb, int ce, const ds_tracks &out)
+                                            const ds_seeds &seeds, int cb, int ce, const ds_tracks &out, const SeedPre &pre)
 {
     const unsigned FULL = 0xffffffffu;
     const int lane = threadIdx.x & 31;
@@ -410,8 +429,9 @@ __device__ __forceinline__ void track_chunk(const DevConst &c, WarpShared<Idx> &
         sh.best_fit[lane] = INT32_MAX;
         sh.n_best[lane] = 0;
         if (act) {
-            const float fx = seeds.x[s], fq = seeds.qop[s];
-            fy = seeds.y[s]; ftx = seeds.tx[s]; fty = seeds.ty[s];
+            const SeedPre sp = pre.s == s ? pre : load_seed(seeds, s, true);
+            const float fx = sp.x, fq = sp.qop;
+            fy = sp.y; ftx = sp.tx; fty = sp.ty;
             const S2 s2 = extrapolate_seed(c, fx, fy, ftx, fty, fq);
             {
                 SeedRec &r = sh.rec[lane];
@@ -437,7 +457,11 @@ __device__ __forceinline__ void track_chunk(const DevConst &c, WarpShared<Idx> &
                 for (int j = lower_bound_x0(H.x0, a, b, xl); j < b && H.x0[j] <= xh; ++j) {
                     const double d = fabs(((double)H.x0[j] + off3) - s2.xc3);
                     if ((d <= s2.w0) & y_compatible(c, H, j, s2.y3)) {
-                        if (nF < max_first) my_slot[nF] = (Idx)j;
+                        if (nF < max_first) {
+                            my_slot[nF] = (Idx)j;
+                            prefetch_l1(H.z + j);
+                            prefetch_l1(H.w + j);
+                        }
                         ++nF;
                     }
                 }
@@ -525,7 +549,10 @@ __device__ __forceinline__ void track_chunk(const DevConst &c, WarpShared<Idx> &
                 for (int l = 0; l < 3; ++l) {
                     sh.near[3 * f + l][0] = (Idx)r[l].x;
                     sh.near[3 * f + l][1] = (Idx)r[l].y;
+                    if (r[l].x >= 0) { prefetch_l1(H.z + r[l].x); prefetch_l1(H.w + r[l].x); prefetch_l1(H.perm + r[l].x); }
+                    if (r[l].y >= 0) { prefetch_l1(H.z + r[l].y); prefetch_l1(H.w + r[l].y); prefetch_l1(H.perm + r[l].y); }
                 }
+                prefetch_l1(H.perm + j3);
                 const int nh = 1 + (r[0].x >= 0) + (r[1].x >= 0) + (r[2].x >= 0);
                 unsigned short ff = kFitNone;
                 if (nh >= c.min_hits) {
@@ -859,15 +886,21 @@ __device__ __forceinline__ void track_chunk_dv1(const DevConst &c, WarpShared<Id
 }
 
 // All seeds of one event: every warp of the block takes an equal share (at most 32 at a time).
+__device__ __forceinline__ int seed_chunk(int s_begin, int s_end)
+{
+    return min(32, (s_end - s_begin + kTrackWarps - 1) / kTrackWarps);
+}
+
 template <typename Idx, bool kDv1>
 __device__ __forceinline__ void track_event(const DevConst &c, TrackShared<Idx> &sh, const EventHits &H,
-                                            const ds_seeds &seeds, int s_begin, int s_end, const ds_tracks &out)
+                                            const ds_seeds &seeds, int s_begin, int s_end, const ds_tracks &out,
+                                            const SeedPre &pre)
 {
     const int wid = threadIdx.x >> 5;
-    const int chunk = min(32, (s_end - s_begin + kTrackWarps - 1) / kTrackWarps);
+    const int chunk = seed_chunk(s_begin, s_end);
     for (int cb = s_begin + wid * chunk; cb < s_end; cb += kTrackWarps * chunk) {
         if (kDv1) track_chunk_dv1<Idx>(c, sh.warp[wid], sh.tab, H, seeds, cb, min(cb + chunk, s_end), out);
-        else track_chunk<Idx>(c, sh.warp[wid], sh.tab, H, seeds, cb, min(cb + chunk, s_end), out);
+        else track_chunk<Idx>(c, sh.warp[wid], sh.tab, H, seeds, cb, min(cb + chunk, s_end), out, pre);
     }
 }
 
@@ -905,6 +938,13 @@ k_track(const __grid_constant__ DevConst c, const LayoutPtrs L, const ds_seeds s
             bulk_g2s(st_ymax, L.symax + h0a, bytes, bar);
         }
     }
+    // the lane's first seed, fetched now so that the load is in flight with the table and the hits
+    SeedPre pre;
+    {
+        const int chunk = seed_chunk(s_begin, s_end);
+        const int s = s_begin + (tid >> 5) * chunk + (tid & 31);
+        pre = load_seed(seeds, s, !kDv1 && (tid & 31) < chunk && s < s_end);
+    }
     const int nb = c.n_bins;
     const int32_t *gtab = L.bin_offsets + (size_t)e * (nb + 1);
     if (staged) {
@@ -928,10 +968,10 @@ k_track(const __grid_constant__ DevConst c, const LayoutPtrs L, const ds_seeds s
         mbar_wait(bar, 0);
         const int d = h0 - h0a;
         H.x0 = st_x0 + d; H.ymin = st_ymin + d; H.ymax = st_ymax + d;
-        track_event<uint16_t, kDv1>(c, *reinterpret_cast<Staged *>(smem_raw), H, seeds, s_begin, s_end, out);
+        track_event<uint16_t, kDv1>(c, *reinterpret_cast<Staged *>(smem_raw), H, seeds, s_begin, s_end, out, pre);
     } else {
         H.x0 = L.sx0 + h0; H.ymin = L.symin + h0; H.ymax = L.symax + h0;
-        track_event<int, kDv1>(c, *reinterpret_cast<Direct *>(smem_raw), H, seeds, s_begin, s_end, out);
+        track_event<int, kDv1>(c, *reinterpret_cast<Direct *>(smem_raw), H, seeds, s_begin, s_end, out, pre);
     }
 }
 
