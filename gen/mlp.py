@@ -20,3 +20,25 @@ def mlp_weights(seed: int, sizes=C.MLP_SIZES):
     out["mu"] = np.asarray(C.MLP_MU, dtype=np.float32)
     out["inv_sigma"] = (1.0 / np.asarray(C.MLP_SIGMA, dtype=np.float64)).astype(np.float32)
     return out
+
+
+# HLT1 line NNs (P:277-P:285): four networks 16 -> 32 -> 1; inputs and their normalisation: reading A-33
+LINE_SIZES = (16, 32, 1)
+LINE_MU = (0.0, 0.0, 0.0, 3.0, 0.0, 0.0, 0.0, 3.0, 0.0, 0.0, 1500.0, 1.0, 0.0, 0.0, 10.0, 1.0)
+LINE_SIGMA = (0.2, 0.1, 0.25, 3.0, 0.2, 0.1, 0.25, 3.0, 300.0, 200.0, 500.0, 1.0, 0.2, 0.1, 10.0, 1.0)
+
+
+def line_weights(seed: int):
+    """Four independent weight sets {W1 [32][16], b1 [32], W3 [32], b3 [1]} ~ N(0, 1/fan_in) (A-18) plus the common
+    input normalisation; the trained weights of the paper are not published."""
+    rng = np.random.default_rng(seed)
+    nets = []
+    for _ in range(4):
+        n_in, n_h, _o = LINE_SIZES
+        nets.append(dict(W1=rng.normal(0.0, n_in ** -0.5, (n_h, n_in)).astype(np.float32),
+                         b1=rng.normal(0.0, n_in ** -0.5, n_h).astype(np.float32),
+                         W3=rng.normal(0.0, n_h ** -0.5, n_h).astype(np.float32),
+                         b3=rng.normal(0.0, n_h ** -0.5, 1).astype(np.float32)))
+    mu = np.asarray(LINE_MU, dtype=np.float32)
+    inv_sigma = (1.0 / np.asarray(LINE_SIGMA, dtype=np.float64)).astype(np.float32)
+    return dict(nets=nets, mu=mu, inv_sigma=inv_sigma)

@@ -627,6 +627,51 @@ int64_t orc_clone_kill(const orc_params *p, int min_shared, int n_events, const 
     return n_killed;
 }
 
+/* ============================================================================================================
+ *  O-L  HLT1 line NNs on the two-track vertices (P:277-P:285): "four different fast NNs with similar
+ *  architectures to the one described in Sec. 2.2 ... a single hidden layer with 32 nodes and an output layer with a
+ *  single node ... The NN threshold for background suppression has been set to 0.5."  The inputs "include track
+ *  parameters of the two secondary tracks, vertex parameters, and parent track parameters"; the paper gives no list.
+ *  Reading A-33, 16 inputs: positive track (tx, ty, q/p, chi2), negative track (tx, ty, q/p, chi2), vertex
+ *  (x, y, z, DOCA), parent (tx, ty, p [GeV], pT [GeV]) with the parent momentum = sum of the two track momenta
+ *  p_i = 1/|q/p_i| along (tx_i, ty_i, 1).  Parity unpinned as far as the meaning of the inputs goes.
+ * ============================================================================================================ */
+void orc_line_features(double txa, double tya, double qa, double c2a, double txb, double tyb, double qb, double c2b,
+                       const double *vtx4, double *v)
+{
+    double pa = 1.0 / fabs(qa), pb = 1.0 / fabs(qb);                         /* GeV */
+    double na = sqrt(txa * txa + tya * tya + 1.0), nb = sqrt(txb * txb + tyb * tyb + 1.0);
+    double px = pa * txa / na + pb * txb / nb, py = pa * tya / na + pb * tyb / nb, pz = pa / na + pb / nb;
+    v[0] = txa; v[1] = tya; v[2] = qa; v[3] = c2a;
+    v[4] = txb; v[5] = tyb; v[6] = qb; v[7] = c2b;
+    v[8] = vtx4[0]; v[9] = vtx4[1]; v[10] = vtx4[2]; v[11] = vtx4[3];
+    v[12] = px / pz; v[13] = py / pz;
+    v[14] = sqrt(px * px + py * py + pz * pz);
+    v[15] = sqrt(px * px + py * py);
+}
+
+/* nets[4] = the four single-hidden-layer networks (n_h2 = 0); per vertex k: scores[4k + i], bits[k] = sum_i 2^i [score_i > thr].
+ * ia / ib index the per-seed track arrays; vtx4 = (x, y, z, doca) per vertex.  edge[k] = 1 if some score is within
+ * edge_rel of the threshold. */
+void orc_lines(const orc_mlp *nets, double thr, double edge_rel, int64_t n_vtx, const int32_t *ia, const int32_t *ib,
+               const double *vtx4, const double *tx, const double *ty, const double *qop, const double *chi2,
+               double *scores, int32_t *bits, int32_t *edge)
+{
+    int64_t k;
+    for (k = 0; k < n_vtx; ++k) {
+        double v[16];
+        int i, a = ia[k], b = ib[k];
+        orc_line_features(tx[a], ty[a], qop[a], chi2[a], tx[b], ty[b], qop[b], chi2[b], vtx4 + 4 * k, v);
+        bits[k] = 0; edge[k] = 0;
+        for (i = 0; i < 4; ++i) {
+            double sc = orc_mlp_eval(&nets[i], v);
+            scores[4 * k + i] = sc;
+            if (sc > thr) bits[k] |= 1 << i;
+            if (relm(sc, thr) < edge_rel) edge[k] = 1;
+        }
+    }
+}
+
 int orc_max_threads(void)
 {
 #ifdef _OPENMP

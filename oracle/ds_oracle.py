@@ -197,6 +197,30 @@ def clone_kill(tracks: dict, seed_offsets, params: dict, min_shared: int = 3) ->
     return killed
 
 
+def line_features(txa, tya, qa, c2a, txb, tyb, qb, c2b, vtx4) -> np.ndarray:
+    """The 16 inputs of the HLT1 line NNs for one vertex (reading A-33)."""
+    v = np.zeros(16)
+    vt = _d(vtx4)
+    lib().orc_line_features.argtypes = [ct.c_double] * 8 + [c_dp, c_dp]
+    lib().orc_line_features(txa, tya, qa, c2a, txb, tyb, qb, c2b, _p(vt), _p(v))
+    return v
+
+
+def lines(line_w: dict, tracks: dict, vtx: dict, thr: float = 0.5, edge_rel: float = 1e-5) -> dict:
+    """O-L (N4, P:277-P:285): the four line NNs on every vertex of `vtx` (ia, ib, x, y, z, doca) -> scores [n][4], bits, edge."""
+    nets = [Mlp(dict(w, mu=line_w["mu"], inv_sigma=line_w["inv_sigma"])) for w in line_w["nets"]]
+    arr = (OrcMlp * 4)(*[m.c for m in nets])
+    n = len(vtx["ia"])
+    ia, ib = _i(vtx["ia"]), _i(vtx["ib"])
+    v4 = _d(np.stack([vtx["x"], vtx["y"], vtx["z"], vtx["doca"]], axis=1)) if n else np.zeros((0, 4))
+    tx, ty, qop, chi2 = (_d(tracks[k]) for k in ("tx", "ty", "qop", "chi2"))
+    scores = np.zeros((n, 4))
+    bits, edge = np.zeros(n, dtype=np.int32), np.zeros(n, dtype=np.int32)
+    lib().orc_lines(arr, ct.c_double(thr), ct.c_double(edge_rel), ct.c_int64(n), _p(ia, c_ip), _p(ib, c_ip), _p(v4), _p(tx),
+                    _p(ty), _p(qop), _p(chi2), _p(scores), _p(bits, c_ip), _p(edge, c_ip))
+    return dict(scores=scores, bits=bits, edge=edge, _keep=nets)
+
+
 def vertex(tracks: dict, seed_offsets, geom: dict, params: dict, edge_rel: float = 1e-5, n_threads: int = 0,
            capacity: int | None = None) -> dict:
     """O-S8/O-S9 for all events on the given per-seed track arrays (x, y, tx, ty, qop, keep)."""

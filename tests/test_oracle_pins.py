@@ -807,3 +807,49 @@ def test_p13_dv1_superset_on_cfg1(orc_mlp):
     s0 = r0["chi2"].astype(np.float64) + P["miss_penalty"] * (4 - r0["nhits"])
     s1 = r1["chi2"].astype(np.float64) + P["miss_penalty"] * (4 - r1["nhits"])
     assert (s1[with_ax] <= s0[with_ax] + 1e-4).all()
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# P-14  HLT1 line NNs (P:277-P:285), reading A-33.  The meaning of the inputs is unpinned (the paper
+#       lists none); pinned here: the arithmetic of the features and of the four 16 -> 32 -> 1 networks.
+# ---------------------------------------------------------------------------------------------------------------
+def test_p14_line_features_closed_forms():
+    # two tracks of equal momentum mirrored in x: the parent flies along z, p = 2 p cos(angle), pT = 0
+    t, p = 0.1, 5.0
+    v = O.line_features(t, 0.0, 1 / p, 1.5, -t, 0.0, -1 / p, 2.5, [1.0, 2.0, 1500.0, 0.3])
+    assert v[:8].tolist() == [t, 0.0, 1 / p, 1.5, -t, 0.0, -1 / p, 2.5] and v[8:12].tolist() == [1.0, 2.0, 1500.0, 0.3]
+    assert abs(v[12]) < 1e-15 and abs(v[13]) < 1e-15 and v[15] < 1e-14
+    assert v[14] == pytest.approx(2 * p / np.sqrt(1 + t * t), rel=1e-14)
+    # one track much harder than the other: the parent takes its direction; momenta add as vectors
+    v = O.line_features(0.2, -0.1, 1 / 50.0, 0, -0.3, 0.25, -1 / 0.5, 0, [0, 0, 0, 0])
+    da, db = np.array([0.2, -0.1, 1.0]), np.array([-0.3, 0.25, 1.0])
+    P3 = 50.0 * da / np.linalg.norm(da) + 0.5 * db / np.linalg.norm(db)
+    assert v[12] == pytest.approx(P3[0] / P3[2], rel=1e-13) and v[13] == pytest.approx(P3[1] / P3[2], rel=1e-13)
+    assert v[14] == pytest.approx(np.linalg.norm(P3), rel=1e-13) and v[15] == pytest.approx(np.hypot(P3[0], P3[1]), rel=1e-13)
+
+
+def test_p14_lines_equal_numpy(orc_mlp):
+    d = gen.generate(1, n_events=30)
+    r = run(d, orc_mlp)
+    v = O.vertex(r, d["seed_offsets"], G, P)
+    lw = gen.line_weights(3)
+    out = O.lines(lw, r, v)
+    assert v["n"] > 100 and out["scores"].shape == (v["n"], 4)
+    tx, ty, q, c2 = (r[k].astype(np.float64) for k in ("tx", "ty", "qop", "chi2"))
+    a, b = v["ia"], v["ib"]
+    pa, pb = 1 / np.abs(q[a]), 1 / np.abs(q[b])
+    na, nb = np.sqrt(tx[a] ** 2 + ty[a] ** 2 + 1), np.sqrt(tx[b] ** 2 + ty[b] ** 2 + 1)
+    px, py, pz = pa * tx[a] / na + pb * tx[b] / nb, pa * ty[a] / na + pb * ty[b] / nb, pa / na + pb / nb
+    X = np.stack([tx[a], ty[a], q[a], c2[a], tx[b], ty[b], q[b], c2[b], v["x"], v["y"], v["z"], v["doca"], px / pz, py / pz,
+                  np.sqrt(px ** 2 + py ** 2 + pz ** 2), np.hypot(px, py)], axis=1)
+    F = (X - lw["mu"].astype(np.float64)) * lw["inv_sigma"].astype(np.float64)
+    for i, w in enumerate(lw["nets"]):
+        h = np.maximum(F @ w["W1"].astype(np.float64).T + w["b1"].astype(np.float64), 0.0)
+        sc = 1 / (1 + np.exp(-(h @ w["W3"].astype(np.float64) + float(w["b3"][0]))))
+        assert np.allclose(out["scores"][:, i], sc, rtol=1e-12)
+        assert np.array_equal((out["bits"] >> i) & 1, (sc > 0.5).astype(np.int32))
+    assert 0 < (out["bits"] != 0).sum() < v["n"] or v["n"] < 5     # random nets: some lines fire, not all
+    # zero weights: every score is exactly 0.5, which does not pass "> 0.5"
+    z = dict(nets=[{k: np.zeros_like(x) for k, x in w.items()} for w in lw["nets"]], mu=lw["mu"], inv_sigma=lw["inv_sigma"])
+    oz = O.lines(z, r, v)
+    assert (oz["scores"] == 0.5).all() and (oz["bits"] == 0).all() and (oz["edge"] == 1).all()
