@@ -127,6 +127,7 @@ def algorithmic_bytes(n_events, n_hits, n_seeds, n_found, n_keep, n_vtx):
         "k_vertex_scan": 16 * n_events,
         "k_vertex_write": 28 * n_keep + 40 * n_vtx,
         "k_clone": 28 * n_seeds,                                           # hit[4], chi2, nhits, found of every slot
+        "k_lines": (24 + 32 + 20) * n_vtx,                                 # vertex record, 2 x 4 track values, 4 scores + bits
     }
 
 
@@ -196,6 +197,8 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--lines", action="store_true",
+                    help="also run the four HLT1 line NNs on the vertices (SURVEY 8f N4, P:277-P:285) in our arm")
     ap.add_argument("--dv1", action="store_true",
                     help="Dv1 triplet search instead of the Dv0 first window (SURVEY 8f N2, P:107-P:111) in both arms")
     ap.add_argument("--clone-min-shared", type=int, default=0,
@@ -271,12 +274,22 @@ def main():
     vws = [ds.vertex_workspace(args.subbatch, max(n_seeds)) for _ in range(n_streams)]
     trk = [ds.empty_tracks(n) for n in n_seeds]
     vtx = [ds.empty_vertices(cap, args.subbatch) for _ in range(n_sub)]
+    line_out = None
+    if args.lines:
+        ds.upload_line_nets(gen.line_weights(0))
+        line_out = [dict(scores=torch.zeros((cap, 4), dtype=torch.float32, device=dev),
+                         bits=torch.zeros(cap, dtype=torch.int32, device=dev)) for _ in range(n_sub)]
+
+    def run_lines(i, s):
+        if line_out is not None:
+            pk.ds_lines(ds.h, trk[i], vtx[i], cap, args.subbatch, 0.5, line_out[i]["scores"], line_out[i]["bits"], s)
 
     def step():
         for i, d in enumerate(devd):
             s = streams[i % n_streams]
             ds.reconstruct(d["hits"], d["seeds"], d["hit_offsets"], d["seed_offsets"], out=trk[i], workspace=ws[i % n_streams], stream=s)
             ds.vertex(trk[i], d["seed_offsets"], out=vtx[i], workspace=vws[i % n_streams], stream=s)
+            run_lines(i, s)
 
     for _ in range(args.warmup):
         step()
@@ -315,6 +328,7 @@ def main():
         for i, d in enumerate(devd):
             ds.reconstruct(d["hits"], d["seeds"], d["hit_offsets"], d["seed_offsets"], out=trk[i], workspace=ws[0], stream=streams[0])
             ds.vertex(trk[i], d["seed_offsets"], out=vtx[i], workspace=vws[0], stream=streams[0])
+            run_lines(i, streams[0])
 
     barrier()
     for _ in range(args.steps):
@@ -406,7 +420,7 @@ def main():
                        "subbatches": n_sub, "events_per_subbatch": args.subbatch, "cuda_streams": n_streams,
                        "hits": sum(n_hits), "seeds": sum(n_seeds), "tracks_found": n_found, "tracks_kept": n_keep, "vertices": n_vtx,
                        "l2": "inputs larger than L2 (each sub-batch reads ~0.76 GB; 7.6 GB per step)",
-                       "magnet_polarity": args.magnet_polarity, "clone_min_shared": args.clone_min_shared, "dv1": bool(args.dv1),
+                       "magnet_polarity": args.magnet_polarity, "clone_min_shared": args.clone_min_shared, "dv1": bool(args.dv1), "lines": bool(args.lines),
                        "parallelism": f"dp{world} (events sharded, no data-path collective)"},
             "roofline": roofline, "whole_path_gbs": whole_gbs, "whole_path_frac": whole_gbs / peak, "kernels": kernels,
             "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,

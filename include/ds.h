@@ -42,6 +42,11 @@ enum {
 #define DS_MLP_H1 32
 #define DS_MLP_H2 16
 
+/* HLT1 line NNs on the vertices (P:277-P:285): four networks DS_LINE_IN -> DS_LINE_H -> 1 (inputs: reading A-33). */
+#define DS_LINE_IN 16
+#define DS_LINE_H 32
+#define DS_N_LINES 4
+
 /* S1 layout granularity: each (layer, y-sector) bin is cut into DS_XBINS equal x0 slices, see ds_layout. */
 #define DS_XBINS 16
 #define DS_MAX_SECTORS 16
@@ -72,6 +77,16 @@ typedef struct {
     float W3[DS_MLP_H2], b3;
     float mu[DS_MLP_IN], inv_sigma[DS_MLP_IN]; /* input k is fed as (v_k - mu_k) * inv_sigma_k */
 } ds_mlp;
+
+/* Weights of the four line NNs (HOST, POD), row-major [net][out][in]; input k of every network is fed as
+ * (v_k - mu_k) * inv_sigma_k.  Network order in the paper: K_S selection, Lambda selection, detached-vs-prompt
+ * K_S, detached-vs-prompt Lambda; the library only evaluates them. */
+typedef struct {
+    size_t struct_size;
+    float W1[DS_N_LINES][DS_LINE_H][DS_LINE_IN], b1[DS_N_LINES][DS_LINE_H];
+    float W3[DS_N_LINES][DS_LINE_H], b3[DS_N_LINES];
+    float mu[DS_LINE_IN], inv_sigma[DS_LINE_IN];
+} ds_line_nets;
 
 /* Algorithm parameters (HOST, POD, read at call time).  None of the values is printed in the paper. */
 typedef struct {
@@ -227,6 +242,19 @@ size_t ds_vertex_workspace_bytes(const ds_handle *h, int n_events, int64_t n_see
 int ds_vertex(ds_handle *h, const ds_tracks *trk, const int32_t *seed_offsets, int n_events, const ds_params *p,
               ds_vertices *out, void *workspace, size_t workspace_bytes, void *cuda_stream);
 
+/* ---- HLT1 line NNs on the vertices (P:277-P:285, A-33) ------------------------------------------- */
+
+/* Copy the four weight sets (HOST) into the handle.  Synchronous; may be called again. */
+int ds_upload_line_nets(ds_handle *h, const ds_line_nets *nets);
+
+/* For every vertex k written by ds_vertex (k < min(offsets[n_events], capacity), read on the device): the 16 inputs
+ * -- positive track (tx, ty, q/p, chi2), negative track (tx, ty, q/p, chi2) from `trk` via ia / ib, vertex (x, y, z,
+ * DOCA), parent (tx, ty, p [GeV], pT [GeV]; momentum sum of the two tracks) -- through the four networks (ReLU hidden
+ * layer, sigmoid): scores[4*k + i] (DEVICE float [4*capacity]) and bits[k] = sum_i 2^i [score_i > threshold] (DEVICE
+ * int32 [capacity]); the paper's threshold is 0.5.  DS_E_NOGEOM if no weights were uploaded. */
+int ds_lines(ds_handle *h, const ds_tracks *trk, const ds_vertices *vtx, int n_events, double threshold, float *scores,
+             int32_t *bits, void *cuda_stream);
+
 /* ---- whole path from HOST buffers ------------------------------------------------------------------------------ */
 
 /* ds_reconstruct + ds_vertex with every array pointer (hits, seeds, offsets, tracks, vertices) in HOST memory
@@ -240,7 +268,7 @@ int ds_process_host(ds_handle *h, const ds_hits *hits, const ds_seeds *seeds, co
 /* ---- per-kernel device timing (measurement aid; no effect on results) ------------------------------------------ */
 
 /* Kernels of the path, in launch order. */
-enum { DS_K_LAYOUT = 0, DS_K_TRACK, DS_K_MLP, DS_K_VTX_COUNT, DS_K_VTX_SCAN, DS_K_VTX_WRITE, DS_K_CLONE, DS_K_COUNT };
+enum { DS_K_LAYOUT = 0, DS_K_TRACK, DS_K_MLP, DS_K_VTX_COUNT, DS_K_VTX_SCAN, DS_K_VTX_WRITE, DS_K_CLONE, DS_K_LINES, DS_K_COUNT };
 
 typedef struct {
     size_t struct_size;

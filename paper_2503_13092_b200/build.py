@@ -11,7 +11,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libds.so")
-SOURCES = ["ds_api.cu", "ds_layout.cu", "ds_track.cu", "ds_clone.cu", "ds_mlp.cu", "ds_vertex.cu"]
+SOURCES = ["ds_api.cu", "ds_layout.cu", "ds_track.cu", "ds_clone.cu", "ds_mlp.cu", "ds_vertex.cu", "ds_lines.cu"]
 HEADERS = [os.path.join(CSRC, "ds_common.cuh"), os.path.join(HERE, "..", "include", "ds.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "--shared",
               "-Xcompiler", "-fPIC,-Wall,-Wextra", "-Xptxas", "-v", "-cudart", "static"]

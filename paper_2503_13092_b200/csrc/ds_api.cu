@@ -11,6 +11,8 @@ struct ds_handle {
     bool has_geom;
     ds_geometry geom;
     DevMlp *d_mlp;
+    DevLines *d_lines;   // nullptr until ds_upload_line_nets
+    int n_sm;
     // arena of the *_host path, grown on demand
     unsigned char *arena;
     size_t arena_bytes;
@@ -164,6 +166,9 @@ int ds_create(ds_handle **h, int cuda_device)
     p->has_geom = false;
     p->arena = nullptr;
     p->arena_bytes = 0;
+    p->d_lines = nullptr;
+    p->n_sm = 0;
+    cudaDeviceGetAttribute(&p->n_sm, cudaDevAttrMultiProcessorCount, cuda_device);
     if (cudaMalloc(&p->d_mlp, sizeof(DevMlp)) != cudaSuccess) {
         cudaGetLastError();
         delete p;
@@ -178,6 +183,7 @@ void ds_destroy(ds_handle *h)
     if (!h) return;
     DeviceGuard guard(h->device);
     if (h->d_mlp) cudaFree(h->d_mlp);
+    if (h->d_lines) cudaFree(h->d_lines);
     if (h->arena) cudaFree(h->arena);
     h->prof.destroy();
     delete h;
@@ -322,6 +328,41 @@ size_t ds_vertex_workspace_bytes(const ds_handle *h, int n_events, int64_t n_see
 {
     (void)h;
     return vertex_workspace_bytes(n_events, n_seeds);
+}
+
+int ds_upload_line_nets(ds_handle *h, const ds_line_nets *nets)
+{
+    if (!h || !nets || nets->struct_size != sizeof(ds_line_nets)) return DS_E_ARG;
+    DeviceGuard guard(h->device);
+    if (!guard.ok) return DS_E_CUDA;
+    static_assert(sizeof(DevLines) == sizeof(ds_line_nets) - offsetof(ds_line_nets, W1), "same layout after struct_size");
+    if (!h->d_lines && cudaMalloc(&h->d_lines, sizeof(DevLines)) != cudaSuccess) {
+        cudaGetLastError();
+        h->d_lines = nullptr;
+        return DS_E_CUDA;
+    }
+    if (cudaMemcpy(h->d_lines, &nets->W1, sizeof(DevLines), cudaMemcpyHostToDevice) != cudaSuccess) {
+        cudaGetLastError();
+        return DS_E_CUDA;
+    }
+    return DS_OK;
+}
+
+int ds_lines(ds_handle *h, const ds_tracks *trk, const ds_vertices *vtx, int n_events, double threshold, float *scores,
+             int32_t *bits, void *cuda_stream)
+{
+    if (!h || !trk || trk->n < 0 || n_events < 0 || !vertices_ok(vtx)) return DS_E_ARG;
+    if (trk->n > 0 && !(trk->tx && trk->ty && trk->qop && trk->chi2)) return DS_E_ARG;
+    if (vtx->capacity > 0 && (!scores || !bits)) return DS_E_ARG;
+    if (!h->d_lines) return DS_E_NOGEOM;
+    DeviceGuard guard(h->device);
+    if (!guard.ok) return DS_E_CUDA;
+    if (launch_lines(h->d_lines, *trk, *vtx, n_events, threshold, scores, bits, h->n_sm, (cudaStream_t)cuda_stream, h->prof) !=
+        cudaSuccess) {
+        cudaGetLastError();
+        return DS_E_CUDA;
+    }
+    return DS_OK;
 }
 
 int ds_vertex(ds_handle *h, const ds_tracks *trk, const int32_t *seed_offsets, int n_events, const ds_params *p,
@@ -477,7 +518,7 @@ int ds_profile_read(ds_handle *h, ds_profile *out)
 const char *ds_kernel_name(int k)
 {
     static const char *names[DS_K_COUNT] = {"k_layout", "k_track", "k_mlp", "k_vertex_count", "k_vertex_scan", "k_vertex_write",
-                                               "k_clone"};
+                                               "k_clone", "k_lines"};
     return (k >= 0 && k < DS_K_COUNT) ? names[k] : nullptr;
 }
 

@@ -47,6 +47,14 @@ struct DevMlp {
 };
 static_assert(sizeof(DevMlp) % 16 == 0, "DevMlp is copied as float4");
 
+// Device copy of the four HLT1 line NNs (global memory, staged to shared memory by k_lines)
+struct DevLines {
+    float W1[DS_N_LINES][DS_LINE_H][DS_LINE_IN], b1[DS_N_LINES][DS_LINE_H];
+    float W3[DS_N_LINES][DS_LINE_H], b3[DS_N_LINES];
+    float mu[DS_LINE_IN], inv_sigma[DS_LINE_IN];
+};
+static_assert(sizeof(DevLines) % 16 == 0, "DevLines is copied as float4");
+
 __device__ __forceinline__ int id_layer(int id) { return (id >> kIdLayerShift) & 3; }
 __device__ __forceinline__ int id_sector(int id) { return (id >> kIdSectorShift) & 15; }
 
@@ -172,6 +180,9 @@ cudaError_t launch_clone(const DevConst &c, const int32_t *seed_offsets, int n_e
 
 cudaError_t launch_mlp(const DevConst &c, const DevMlp *mlp, const ds_seeds &seeds, const ds_tracks &trk,
                        cudaStream_t st, Prof &prof);
+
+cudaError_t launch_lines(const DevLines *nets, const ds_tracks &trk, const ds_vertices &vtx, int n_events, double thr,
+                         float *scores, int32_t *bits, int n_sm, cudaStream_t st, Prof &prof);
 
 cudaError_t launch_vertex(const DevConst &c, const ds_tracks &trk, const int32_t *seed_offsets, int n_events,
                           const ds_vertices &out, void *workspace, cudaStream_t st, Prof &prof);

@@ -40,6 +40,16 @@ class DsMlp(ct.Structure):
                 ("mu", ct.c_float * DS_MLP_IN), ("inv_sigma", ct.c_float * DS_MLP_IN)]
 
 
+DS_LINE_IN, DS_LINE_H, DS_N_LINES = 16, 32, 4
+
+
+class DsLineNets(ct.Structure):
+    _fields_ = [("struct_size", ct.c_size_t),
+                ("W1", ct.c_float * (DS_N_LINES * DS_LINE_H * DS_LINE_IN)), ("b1", ct.c_float * (DS_N_LINES * DS_LINE_H)),
+                ("W3", ct.c_float * (DS_N_LINES * DS_LINE_H)), ("b3", ct.c_float * DS_N_LINES),
+                ("mu", ct.c_float * DS_LINE_IN), ("inv_sigma", ct.c_float * DS_LINE_IN)]
+
+
 class DsParams(ct.Structure):
     _fields_ = [("struct_size", ct.c_size_t), ("w0_a", ct.c_double), ("w0_b", ct.c_double), ("w0_max", ct.c_double),
                 ("w1_a", ct.c_double), ("w1_b", ct.c_double), ("y_tol", ct.c_double), ("w_mag", ct.c_double),
@@ -75,7 +85,7 @@ class DsVertices(ct.Structure):
                 ("offsets", ct.c_void_p), ("overflow", ct.c_void_p), ("capacity", ct.c_int64)]
 
 
-DS_K_COUNT = 7
+DS_K_COUNT = 8
 
 
 class DsProfile(ct.Structure):
@@ -125,6 +135,8 @@ def lib() -> ct.CDLL:
                                      ct.POINTER(DsParams), ct.POINTER(DsTracks), vp, ct.c_size_t, vp]
         L.ds_ghost_killer.argtypes = [vp, ct.POINTER(DsSeeds), ct.POINTER(DsParams), ct.POINTER(DsTracks), vp]
         L.ds_clone_kill.argtypes = [vp, vp, ct.c_int, ct.POINTER(DsParams), ct.POINTER(DsTracks), vp]
+        L.ds_upload_line_nets.argtypes = [vp, ct.POINTER(DsLineNets)]
+        L.ds_lines.argtypes = [vp, ct.POINTER(DsTracks), ct.POINTER(DsVertices), ct.c_int, ct.c_double, vp, vp, vp]
         L.ds_vertex_workspace_bytes.argtypes = [vp, ct.c_int, ct.c_int64]
         L.ds_vertex_workspace_bytes.restype = ct.c_size_t
         L.ds_vertex.argtypes = [vp, ct.POINTER(DsTracks), vp, ct.c_int, ct.POINTER(DsParams), ct.POINTER(DsVertices),
@@ -167,6 +179,22 @@ def make_mlp(w: dict) -> DsMlp:
             raise ValueError(f"mlp weight {k}: expected shape {shape}")
         getattr(o, k)[:] = a.tolist()
     o.b3 = float(np.asarray(w["b3"]).reshape(-1)[0])
+    return o
+
+
+def make_line_nets(w: dict) -> DsLineNets:
+    """w = gen.line_weights(): {"nets": 4 x {W1 [32][16], b1 [32], W3 [32], b3 [1]}, "mu" [16], "inv_sigma" [16]}."""
+    o = DsLineNets()
+    o.struct_size = ct.sizeof(DsLineNets)
+    if len(w["nets"]) != DS_N_LINES:
+        raise ValueError("four line networks expected")
+    for k, size in (("W1", DS_LINE_H * DS_LINE_IN), ("b1", DS_LINE_H), ("W3", DS_LINE_H), ("b3", 1)):
+        a = np.concatenate([np.ascontiguousarray(n[k], dtype=np.float32).reshape(-1) for n in w["nets"]])
+        if a.size != DS_N_LINES * size:
+            raise ValueError(f"line net weight {k}: wrong size")
+        getattr(o, k)[:] = a.tolist()
+    for k in ("mu", "inv_sigma"):
+        getattr(o, k)[:] = np.ascontiguousarray(w[k], dtype=np.float32).reshape(-1).tolist()
     return o
 
 
@@ -277,6 +305,17 @@ def ds_reconstruct(h, hits, seeds, hit_offsets, seed_offsets, n_events, params: 
                                 ct.byref(params), ct.byref(ts), _ptr(workspace),
                                 0 if workspace is None else workspace.numel() * workspace.element_size(),
                                 _stream_ptr(stream)), "ds_reconstruct")
+
+
+def ds_upload_line_nets(h, line_w: dict) -> None:
+    n = make_line_nets(line_w)
+    _check(lib().ds_upload_line_nets(h, ct.byref(n)), "ds_upload_line_nets")
+
+
+def ds_lines(h, tracks, vertices, capacity: int, n_events: int, threshold: float, scores, bits, stream=None) -> None:
+    ts, vs = _tracks(tracks), _vertices(vertices, capacity)
+    _check(lib().ds_lines(h, ct.byref(ts), ct.byref(vs), n_events, float(threshold), _ptr(scores), _ptr(bits),
+                          _stream_ptr(stream)), "ds_lines")
 
 
 def ds_clone_kill(h, seed_offsets, n_events: int, params: DsParams, tracks, stream=None) -> None:
@@ -434,6 +473,17 @@ class Downstream:
         if workspace is None:
             workspace = self.workspace(ne, hits["id"].numel(), seeds["x"].numel())
         ds_reconstruct(self.h, hits, seeds, hit_offsets, seed_offsets, ne, self.params, out, workspace, stream)
+        return out
+
+    def upload_line_nets(self, line_w: dict) -> None:
+        ds_upload_line_nets(self.h, line_w)
+
+    def lines(self, tracks: dict, vertices: dict, n_events: int, threshold: float = 0.5, stream=None) -> dict:
+        """HLT1 line NNs on the vertices ds_vertex wrote: {"scores": [capacity][4] fp32, "bits": [capacity] int32}."""
+        t, cap = self.torch, vertices["capacity"]
+        out = dict(scores=t.zeros((cap, DS_N_LINES), dtype=t.float32, device=self.device),
+                   bits=t.zeros(cap, dtype=t.int32, device=self.device))
+        ds_lines(self.h, tracks, vertices, cap, n_events, threshold, out["scores"], out["bits"], stream)
         return out
 
     def clone_kill(self, tracks: dict, seed_offsets, stream=None):

@@ -440,6 +440,32 @@ def test_clone_killing(ds, orc_mlp, cfg, n_events):
         assert np.array_equal(t2[k], exp[k]), k
 
 
+def test_line_nns(ds, orc_mlp):
+    """SURVEY §8f N4 (P:277-P:285, A-33): the four line NNs on the vertices ds_vertex wrote, against the oracle fed the
+    GPU's own tracks and vertices: scores within 1e-4 relative, decision bits exact except scores within 1e-5 of 0.5."""
+    d = gen.generate(1, n_events=300)
+    lw = gen.line_weights(3)
+    ds.upload_line_nets(lw)
+    hits, seeds = ds.to_device(d["hits"]), ds.to_device(d["seeds"])
+    ho, so = ds.to_device(dict(h=d["hit_offsets"], s=d["seed_offsets"])).values()
+    trk = ds.reconstruct(hits, seeds, ho, so)
+    vtx = ds.vertex(trk, so, capacity=1 << 14)
+    ln = to_host(ds.lines(trk, vtx, d["n_events"]))
+    t, v = to_host(trk), to_host(vtx)
+    n = int(v["offsets"][-1])
+    assert 100 < n <= 1 << 14
+    vv = {k: v[k][:n] for k in ("ia", "ib", "x", "y", "z", "doca")}
+    o = O.lines(lw, t, vv)
+    assert np.allclose(ln["scores"][:n], o["scores"], rtol=1e-4, atol=1e-6)
+    diff = ln["bits"][:n] != o["bits"]
+    assert not (diff & (o["edge"] == 0)).any() and diff.sum() <= max(1, n // 10000)
+    assert (ln["bits"][n:] == 0).all() and 0 < (o["bits"] != 0).sum() < n
+    # a capacity smaller than the vertex count: only the written vertices are scored
+    small = ds.vertex(trk, so, capacity=64)
+    l2 = to_host(ds.lines(trk, small, d["n_events"]))
+    assert np.array_equal(l2["bits"], ln["bits"][:64]) and np.allclose(l2["scores"], ln["scores"][:64], rtol=0, atol=0)
+
+
 def test_vertexing_large_events_in_a_small_event_batch(ds, orc_mlp):
     """A few cfg3 events (~500 seeds, thousands of pairs) among many empty ones: the batch averages few seeds per event
     and takes the warp-per-event vertex kernels, whose staging capacity and pair mask these events exceed.  The same
