@@ -42,3 +42,21 @@ def line_weights(seed: int):
     mu = np.asarray(LINE_MU, dtype=np.float32)
     inv_sigma = (1.0 / np.asarray(LINE_SIGMA, dtype=np.float64)).astype(np.float32)
     return dict(nets=nets, mu=mu, inv_sigma=inv_sigma)
+
+
+def embed_single_hidden(w1: dict, sizes=C.MLP_SIZES) -> dict:
+    """The paper's ghost killer has ONE hidden layer (8 -> 14 -> 1); the library's network is 8 -> 32 -> 16 -> 1
+    (BASELINE cfg0).  A single-hidden-layer network with n_h <= 16 units runs on it unchanged: its hidden units become
+    the first n_h units of layer 1 (the others get zero weights), layer 2 copies them through (ReLU of a non-negative
+    number is the number itself) and W3 is padded with zeros.  w1 = {W1 [n_h][8], b1 [n_h], W3 [n_h], b3 [1], mu, inv_sigma}."""
+    n_in, h1, h2, _ = sizes
+    n_h = w1["W1"].shape[0]
+    assert n_h <= h2 and w1["W1"].shape[1] == n_in
+    out = dict(W1=np.zeros((h1, n_in), np.float32), b1=np.zeros(h1, np.float32), W2=np.zeros((h2, h1), np.float32),
+               b2=np.zeros(h2, np.float32), W3=np.zeros(h2, np.float32), b3=np.asarray(w1["b3"], np.float32).reshape(1),
+               mu=w1["mu"], inv_sigma=w1["inv_sigma"])
+    out["W1"][:n_h] = w1["W1"]
+    out["b1"][:n_h] = w1["b1"]
+    out["W2"][np.arange(n_h), np.arange(n_h)] = 1.0
+    out["W3"][:n_h] = np.asarray(w1["W3"]).reshape(-1)
+    return out

@@ -280,6 +280,37 @@ def test_ghost_killer_alone(ds, orc_mlp, torch):
             assert 0.4 < keep[f].mean() < 0.6
 
 
+def test_paper_architecture_8_14_1(torch, mlp_w):
+    """the paper's ghost killer has one hidden layer of 14 units.  Embedded in the 8 -> 32 -> 16 -> 1
+    network of the library (gen.embed_single_hidden) it gives the scores of the oracle's single-hidden-layer evaluation."""
+    import paper_2503_13092_b200 as pk
+    rng = np.random.default_rng(14)
+    w1 = dict(W1=rng.normal(0, 8 ** -0.5, (14, 8)).astype(np.float32), b1=rng.normal(0, 8 ** -0.5, 14).astype(np.float32),
+              W3=rng.normal(0, 14 ** -0.5, 14).astype(np.float32), b3=rng.normal(0, 14 ** -0.5, 1).astype(np.float32),
+              mu=mlp_w["mu"], inv_sigma=mlp_w["inv_sigma"])
+    orc = O.Mlp(w1)                                                   # n_h2 = 0: W3 acts on the hidden layer
+    assert orc.c.n_h1 == 14 and orc.c.n_h2 == 0
+    n = 4000
+    trk = {k: (rng.normal(0, 1, n) * s + m).astype(np.float32)
+           for k, m, s in zip(("x", "y", "tx", "ty", "qop", "chi2"), C.MLP_MU[:6], C.MLP_SIGMA[:6])}
+    seeds = dict(x=trk["x"], y=trk["y"], tx=trk["tx"], ty=trk["ty"], qop=rng.normal(0, 0.25, n).astype(np.float32),
+                 chi2=(rng.chisquare(7, n) / 7).astype(np.float32))
+    d14 = pk.Downstream(G, gen.embed_single_hidden(w1), P)
+    try:
+        dev = d14.empty_tracks(n)
+        for k, a in trk.items():
+            dev[k].copy_(torch.as_tensor(a))
+        dev["found"].fill_(1)
+        d14.ghost_killer(d14.to_device(seeds), dev)
+        torch.cuda.synchronize()
+        score = dev["score"].cpu().numpy()
+    finally:
+        d14.close()
+    ref = np.array([orc.eval([trk["x"][i], trk["y"][i], trk["tx"][i], trk["ty"][i], trk["qop"][i], trk["chi2"][i],
+                              seeds["qop"][i], seeds["chi2"][i]]) for i in range(n)])
+    assert parity.close(score, ref, 1e-3).all() and 0.05 < ref.std()
+
+
 # ---- S8..S10 on hand-made tracks -----------------------------------------------------------------------------------------
 def _tracks_from(ds, torch, arr):
     n = len(arr["x"])

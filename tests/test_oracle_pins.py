@@ -853,3 +853,22 @@ def test_p14_lines_equal_numpy(orc_mlp):
     z = dict(nets=[{k: np.zeros_like(x) for k, x in w.items()} for w in lw["nets"]], mu=lw["mu"], inv_sigma=lw["inv_sigma"])
     oz = O.lines(z, r, v)
     assert (oz["scores"] == 0.5).all() and (oz["bits"] == 0).all() and (oz["edge"] == 1).all()
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# P-15  the paper's single-hidden-layer ghost killer 8 -> 14 -> 1 embedded in 8 -> 32 -> 16 -> 1
+# ---------------------------------------------------------------------------------------------------------------
+def test_p15_single_hidden_layer_embeds_exactly(mlp_w):
+    rng = np.random.default_rng(15)
+    w1 = dict(W1=rng.normal(0, 8 ** -0.5, (14, 8)).astype(np.float32), b1=rng.normal(0, 8 ** -0.5, 14).astype(np.float32),
+              W3=rng.normal(0, 14 ** -0.5, 14).astype(np.float32), b3=rng.normal(0, 14 ** -0.5, 1).astype(np.float32),
+              mu=mlp_w["mu"], inv_sigma=mlp_w["inv_sigma"])
+    one, emb = O.Mlp(w1), O.Mlp(gen.embed_single_hidden(w1))
+    assert (one.c.n_h1, one.c.n_h2, emb.c.n_h1, emb.c.n_h2) == (14, 0, 32, 16)
+    v = rng.normal(0, 1, (300, 8)) * np.array(C.MLP_SIGMA) + np.array(C.MLP_MU)
+    a = np.array([one.eval(x) for x in v])
+    assert np.array_equal(a, np.array([emb.eval(x) for x in v]))          # ReLU of a non-negative number, sums of exact zeros
+    # and the single-hidden-layer evaluation itself is the textbook formula
+    f = (v - w1["mu"].astype(np.float64)) * w1["inv_sigma"].astype(np.float64)
+    h = np.maximum(f @ w1["W1"].astype(np.float64).T + w1["b1"].astype(np.float64), 0)
+    assert np.allclose(a, 1 / (1 + np.exp(-(h @ w1["W3"].astype(np.float64) + float(w1["b3"][0])))), rtol=1e-13)
