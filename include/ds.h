@@ -100,8 +100,10 @@ typedef struct {
     int32_t max_first_hits;           /* closest UTbX hits tried per seed, 1..DS_MAX_FIRST_HITS       */
     double mlp_thr;
     int32_t mlp_keep_above;           /* 1: keep iff score > thr (BASELINE cfg3); 0: keep iff score < thr */
-    int32_t max_event_hits_hint;      /* expected upper bound of hits per event (0 = 4096).  Events above it are
-                                         still laid out correctly, on a slower path (see ds_layout).             */
+    int32_t max_event_hits_hint;      /* expected upper bound of hits per event (0 = 4096): sizes the per-event shared-memory
+                                         staging of the layout and tracking kernels (and with it the thread blocks per
+                                         SM, so a tight bound is faster).  Events above it give the same results on
+                                         slower global-memory paths.                                                */
     double doca_max, zv_min, zv_max;  /* vertex cuts (BASELINE cfg3)                                             */
     double m_pi, m_p, m_ks, m_lambda, dm_ks, dm_lambda; /* MeV                                                   */
     double n2_min;                    /* pairs with |d_a x d_b|^2 below this have no vertex       (A-14)        */
@@ -191,7 +193,8 @@ int ds_upload_geometry(ds_handle *h, const ds_geometry *g, const ds_mlp *m);
 /* ---- S1: layout (P:109-P:111 "UT hits are grouped into different Y sectors"; BASELINE north_star (1)) -------- */
 
 /* Segmented sort of every event's hits by (layer, sector, x0, id) plus the per-event bin table (see ds_layout_out).
- * One thread block per event: bin histogram in shared memory, exclusive scan, scatter, rank inside each bin.
+ * One thread block per event: the input arrays staged in shared memory by bulk async copies (16-byte aligned array
+ * pointers; otherwise by ordinary loads), bin histogram, exclusive scan, rank inside each bin, gathered coalesced stores.
  * Events with more hits than params->max_event_hits_hint (or than fit in shared memory) take an O(n^2) path that
  * is slower but gives the same result.  hit_offsets: DEVICE int32 [n_events+1], non-decreasing, [0] = 0,
  * [n_events] = hits->n.  No workspace. */
