@@ -75,7 +75,8 @@ __device__ __forceinline__ bool vertex_pair(const DevConst &c, const VtxTrack &a
     const double A = a.tx * a.tx + a.ty * a.ty + 1.0, B = a.tx * b.tx + a.ty * b.ty + 1.0, C = b.tx * b.tx + b.ty * b.ty + 1.0;
     const double rx = a.x - b.x, ry = a.y - b.y;
     const double Dd = a.tx * rx + a.ty * ry, Ee = b.tx * rx + b.ty * ry;
-    double sa = (B * Ee - C * Dd) / n2, sb = (A * Ee - B * Dd) / n2;
+    const double inv_n2 = 1.0 / n2;   // one division for both line parameters
+    double sa = (B * Ee - C * Dd) * inv_n2, sb = (A * Ee - B * Dd) * inv_n2;
     constexpr bool curved = kCurved;   // the launcher instantiates the straight-track kernels for magnet_polarity = 0
     if (curved) {
         // Newton-Raphson on F(u, v) = |Traj_a(z_ref + u) - Traj_b(z_ref + v)|^2 with the parabolas of Eq. 4, from the
@@ -101,8 +102,11 @@ __device__ __forceinline__ bool vertex_pair(const DevConst &c, const VtxTrack &a
     o.x = 0.5 * (qax + qbx);
     o.y = 0.5 * (qay + qby);
     o.z = 0.5 * (qaz + qbz);
-    o.doca = sqrt(dx * dx + dy * dy + dz * dz);
-    if (!(o.doca < c.doca_max && c.zv_min <= o.z && o.z <= c.zv_max)) return false;
+    // the cuts first, on the squared distance: most pairs end here, without the square root
+    const double d2 = dx * dx + dy * dy + dz * dz;
+    if (!(d2 < c.doca_max * c.doca_max && c.zv_min <= o.z && o.z <= c.zv_max)) return false;
+    o.doca = sqrt(d2);
+    if (!(o.doca < c.doca_max)) return false;   // the cut as defined (decides the last ulp)
     // invariant masses: same momentum sum under both hypotheses; proton = larger momentum (A-15)
     double atx = a.tx, btx = b.tx, ak = a.k, bk = b.k;
     if (curved) {   // slopes dx/dz at the vertex z (Eq. 2) and with them the direction normalisation
