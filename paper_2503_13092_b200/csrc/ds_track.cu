@@ -129,6 +129,9 @@ struct WarpShared {
     int best_fit[32];                     // per seed: first fit task with that score
     int n_best[32];                       // per seed: fits with that score (+ 2 for every first hit left to the seed's thread)
     int dv_off[32], dv_a[32];             // Dv1: first item and first UTbX candidate of the seed
+    float cand_z[kFirstCap];              // Dv1: items that passed the fp32 pre-test: z of the UTbX hit,
+    Idx cand_j3[kFirstCap];               //      the hit,
+    unsigned char cand_o[kFirstCap];      //      the seed (lane)
     // Dv1 keeps at most kFirstCap triplets in slot[]; the rest of it holds the fit queue (4 per triplet)
     __device__ __forceinline__ unsigned short *dv_task_ptr() { return reinterpret_cast<unsigned short *>(slot + kFirstCap); }
 };
@@ -826,14 +829,16 @@ __device__ __forceinline__ void track_chunk_dv1(const DevConst &c, WarpShared<Id
     int o_nx = 0, j3_nx = 0;
     float z3_nx = 0.f;
     if (lane < total) item(lane, o_nx, j3_nx, z3_nx);
-    for (int t0 = 0; t0 < total; t0 += 32) {
-        const int t = t0 + lane;
+    // T2: the exact (fp64) triplet test for the last `cnt` (<= 32) queued items, a lane each; triplets are compacted into the list
+    int n_cand = 0;
+    auto exact_round = [&](int cnt) {
+        __syncwarp();
         bool has = false;
-        const int o = o_nx, j3 = j3_nx;
-        const float z3 = z3_nx;
-        int j0 = -1;
-        if (t + 32 < total) item(t + 32, o_nx, j3_nx, z3_nx);
-        if (t < total) {
+        int o = 0, j3 = 0, j0 = -1;
+        float z3 = 0.f;
+        if (lane < cnt) {
+            const int q = n_cand - cnt + lane;
+            o = sh.cand_o[q]; j3 = (int)sh.cand_j3[q]; z3 = sh.cand_z[q];
             const SeedRec &t2 = sh.rec[o];
             if (y_compatible(c, H, j3, t2.y[3])) {
                 const double x3 = (double)H.x0[j3] + c.dxdy[3] * t2.y[3];
@@ -843,8 +848,8 @@ __device__ __forceinline__ void track_chunk_dv1(const DevConst &c, WarpShared<Id
                 has = j0 >= 0;
             }
         }
+        n_cand -= cnt;
         const unsigned m = __ballot_sync(FULL, has);
-        if (m == 0) continue;
         if (has) {
             const int f = n_trip + __popc(m & lanemask_lt());
             sh.fs[f] = (unsigned short)o;
@@ -854,11 +859,53 @@ __device__ __forceinline__ void track_chunk_dv1(const DevConst &c, WarpShared<Id
             sh.zw3[f] = make_float2(z3, 0.f);   // w of the UTbX hit is read by the fit
         }
         n_trip += __popc(m);
-        if (n_trip >= 32) {   // the list holds 64: room for one more round of items is guaranteed after this
+        if (n_trip >= 32) {   // the list holds 64: room for one more round is guaranteed after this
             dv1_flush<Idx>(c, sh, tab, H, n_trip, best);
             n_trip = 0;
         }
+    };
+    // T1: fp32 pre-test, a superset of the exact one (margins far above the fp32 rounding of the prediction, ~1e-3 mm):
+    // y-compatibility of the UTbX hit and "is there a UTaX hit near the line through the hit and the magnet point".
+    // About one item in eight passes; only those pay for the fp64 division and search.
+    const float ytol_f = (float)c.y_tol + 0.01f, zl0_f = (float)c.z_layer[0];
+    for (int t0 = 0; t0 < total; t0 += 32) {
+        const int t = t0 + lane;
+        const int o = o_nx, j3 = j3_nx;
+        const float z3 = z3_nx;
+        if (t + 32 < total) item(t + 32, o_nx, j3_nx, z3_nx);
+        bool cand = false;
+        if (t < total) {
+            const SeedRec &t2 = sh.rec[o];
+            const float y3 = (float)t2.y[3];
+            if (H.ymin[j3] - ytol_f <= y3 && y3 <= H.ymax[j3] + ytol_f) {
+                const float xm = (float)t2.xm, zm = (float)t2.zm;
+                const float x3 = H.x0[j3] + (float)(c.dxdy[3] * t2.y[3]);
+                const float xp = xm + (x3 - xm) * ((zl0_f - zm) / (z3 - zm));
+                const float tg = xp - (float)(c.dxdy[0] * t2.y[0]);                 // in x0 coordinates of UTaX
+                const float wf = (float)t2.w1 * 1.0001f + 0.05f + 4e-6f * fabsf(tg);
+                const float xl = tg - wf, xh = tg + wf;
+                const int bl = xbin(xl, c.xb_off, c.xb_scale), bh = xbin(xh, c.xb_off, c.xb_scale);
+                for (int sec = (int)t2.sec[0][0]; sec <= (int)t2.sec[0][1] && !cand; ++sec) {
+                    const int base = sec * kXBins;   // layer 0
+                    const int a = (int)tab[base + bl], b = (int)tab[base + bh + 1];
+                    const int j = lower_bound_x0(H.x0, a, b, xl);
+                    cand = j < b && H.x0[j] <= xh;
+                }
+                cand = cand || !(xp == xp);   // a prediction that is not a number goes to the exact test as it is
+            }
+        }
+        const unsigned m = __ballot_sync(FULL, cand);
+        if (m == 0) continue;
+        if (cand) {
+            const int q = n_cand + __popc(m & lanemask_lt());
+            sh.cand_o[q] = (unsigned char)o;
+            sh.cand_j3[q] = (Idx)j3;
+            sh.cand_z[q] = z3;
+        }
+        n_cand += __popc(m);
+        if (n_cand >= 32) exact_round(32);
     }
+    if (n_cand > 0) exact_round(n_cand);
     if (n_trip > 0) dv1_flush<Idx>(c, sh, tab, H, n_trip, best);
     // ---- track record ------------------------------------------------------------------------------------------------------------
     if (act) {
