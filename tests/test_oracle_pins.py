@@ -872,3 +872,13 @@ def test_p15_single_hidden_layer_embeds_exactly(mlp_w):
     f = (v - w1["mu"].astype(np.float64)) * w1["inv_sigma"].astype(np.float64)
     h = np.maximum(f @ w1["W1"].astype(np.float64).T + w1["b1"].astype(np.float64), 0)
     assert np.allclose(a, 1 / (1 + np.exp(-(h @ w1["W3"].astype(np.float64) + float(w1["b3"][0])))), rtol=1e-13)
+
+
+def test_p11_gamma_golden_values():
+    """tests/golden/eq3_gamma.txt: Eq. 3 worked out by hand from the constants the paper prints."""
+    import os
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "eq3_gamma.txt")
+    rows = [ln.split() for ln in open(path) if ln.strip() and not ln.startswith("#")]
+    assert len(rows) == 5
+    for mp, qop, g in rows:
+        assert O.gamma(dict(P, magnet_polarity=float(mp)), float(qop)) == pytest.approx(float(g), rel=1e-12, abs=1e-30)
