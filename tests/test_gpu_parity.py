@@ -497,6 +497,24 @@ def test_line_nns(ds, orc_mlp):
     assert np.array_equal(l2["bits"], ln["bits"][:64]) and np.allclose(l2["scores"], ln["scores"][:64], rtol=0, atol=0)
 
 
+@pytest.mark.parametrize("dv1", [0, 1])
+def test_results_do_not_depend_on_the_hint(ds, dv1):
+    """max_event_hits_hint only sizes the staging buffers: a hint far below the event size (global-memory paths of both
+    kernels), a tight one, the default and a generous one give the same records bit for bit."""
+    d = gen.generate(1, n_events=24)
+    ref = None
+    for hint in (64, int(np.diff(d["hit_offsets"]).max()), 0, 18000):
+        t, v = gpu_run(ds, d, params=dict(P, dv1=dv1, max_event_hits_hint=hint))
+        if ref is None:
+            ref = (t, v)
+            assert t["found"].sum() > 100 and v["n"] > 50
+            continue
+        for k in ref[0]:
+            assert np.array_equal(ref[0][k], t[k]), (hint, k)
+        for k in ("evt", "ia", "ib", "flags", "x", "y", "z", "doca", "m_pipi", "m_ppi", "offsets"):
+            assert np.array_equal(ref[1][k], v[k]), (hint, k)
+
+
 def test_vertexing_large_events_in_a_small_event_batch(ds, orc_mlp):
     """A few cfg3 events (~500 seeds, thousands of pairs) among many empty ones: the batch averages few seeds per event
     and takes the warp-per-event vertex kernels, whose staging capacity and pair mask these events exceed.  The same
