@@ -197,6 +197,9 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--cfg", type=int, default=4, choices=[1, 2, 3, 4],
+                    help="BASELINE configs[k] generator; 4 = the metric's workload.  3 (with --events 2000 --subbatch 2000): the "
+                         "vertexing stress, reported with the ALU fraction of the vertex kernels (SURVEY 8d)")
     ap.add_argument("--lines", action="store_true",
                     help="also run the four HLT1 line NNs on the vertices (SURVEY 8f N4, P:277-P:285) in our arm")
     ap.add_argument("--dv1", action="store_true",
@@ -208,6 +211,8 @@ def main():
     args = ap.parse_args()
     rank, world = int(os.environ.get("RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
     local = int(os.environ.get("LOCAL_RANK", 0))
+    global CFG
+    CFG = args.cfg
     if args.impl == "reference":
         return run_reference(args, rank)
     if args.warmup < 3:
@@ -269,7 +274,7 @@ def main():
     torch.cuda.synchronize()
     n_streams = max(1, args.streams)
     streams = [torch.cuda.Stream(device=dev) for _ in range(n_streams)]
-    cap = 1 << 20
+    cap = 1 << 20 if args.cfg != 3 else 1 << 24   # vertex capacity per sub-batch (cfg3: tens of thousands of pairs per event)
     ws = [ds.workspace(args.subbatch, max(n_hits), max(n_seeds)) for _ in range(n_streams)]
     vws = [ds.vertex_workspace(args.subbatch, max(n_seeds)) for _ in range(n_streams)]
     trk = [ds.empty_tracks(n) for n in n_seeds]
@@ -359,6 +364,24 @@ def main():
                 "timing": "CUDA events around every launch, one-stream pass of the same K steps right after the timed region"}
     whole_gbs = sum(alg.values()) * args.steps / (ms_total * 1e-3) / 1e9
 
+    # ---- cfg3: the vertex kernels are bound by plain fp64 arithmetic, not by HBM -----------------------------------
+    vertex_alu = None
+    if args.cfg == 3:
+        n_pairs = 0
+        for i, d in enumerate(devd):
+            so = d["seed_offsets"].cpu().numpy()
+            keep, q = trk[i]["keep"].cpu().numpy(), trk[i]["qop"].cpu().numpy()
+            pos = np.concatenate([[0], np.cumsum((keep == 1) & (q > 0))])
+            neg = np.concatenate([[0], np.cumsum((keep == 1) & (q < 0))])
+            n_pairs += int(((pos[so[1:]] - pos[so[:-1]]) * (neg[so[1:]] - neg[so[:-1]])).sum())
+        ms = sum(kernels[k]["ms_per_step"] for k in ("k_vertex_count", "k_vertex_write") if k in kernels)
+        flop = 130.0 * n_pairs * 2                      # ~130 flop per pair, evaluated in both kernels
+        peak_tf = 148 * 64 * 2 * (clocks.get("sm_mhz") or 1965.0) * 1e6 / 1e12
+        vertex_alu = {"bound": "alu", "pairs_per_step": n_pairs, "flop_per_pair": 130, "ms_per_step": ms,
+                      "achieved": flop / (ms * 1e-3) / 1e12, "peak": peak_tf, "unit": "TFLOP/s (fp64)",
+                      "frac": flop / (ms * 1e-3) / 1e12 / peak_tf,
+                      "peak_source": "nominal: 148 SMs x 64 fp64 FMA lanes x 2 x SM clock under load (not measured)"}
+
     # ---- end to end: pinned host buffers in, pinned host buffers out, through ds_process_host ----------------------------
     e2e = None
     if not args.no_e2e:
@@ -416,14 +439,16 @@ def main():
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
-            "config": {"workload": "BASELINE configs[4]: cfg-1 generator, seed 4, device-resident SoA", "events_per_gpu": events_rank,
+            "config": {"workload": ("BASELINE configs[4]: cfg-1 generator, seed 4, device-resident SoA" if CFG == 4 else
+                                    f"BASELINE configs[{CFG}] generator, device-resident SoA (not the metric's workload)"),
+                       "events_per_gpu": events_rank,
                        "subbatches": n_sub, "events_per_subbatch": args.subbatch, "cuda_streams": n_streams,
                        "hits": sum(n_hits), "seeds": sum(n_seeds), "tracks_found": n_found, "tracks_kept": n_keep, "vertices": n_vtx,
                        "l2": "inputs larger than L2 (each sub-batch reads ~0.76 GB; 7.6 GB per step)",
                        "magnet_polarity": args.magnet_polarity, "clone_min_shared": args.clone_min_shared, "dv1": bool(args.dv1), "lines": bool(args.lines),
                        "parallelism": f"dp{world} (events sharded, no data-path collective)"},
             "roofline": roofline, "whole_path_gbs": whole_gbs, "whole_path_frac": whole_gbs / peak, "kernels": kernels,
-            "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
+            "vertex_alu": vertex_alu, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
         }), flush=True)
     ds.close()
     if world > 1:
