@@ -187,7 +187,7 @@ __device__ __forceinline__ void block_ordered_offsets(bool f0, bool f1, int (*wa
 template <bool kCurved>
 __global__ void __launch_bounds__(kVtxThreads)
 k_vertex_count(const __grid_constant__ DevConst c, const ds_tracks trk, const int32_t *__restrict__ seed_offsets,
-               PairLists pl, int32_t *__restrict__ n_per_event)
+               PairLists pl, unsigned long long *__restrict__ masks, int32_t *__restrict__ n_per_event)
 {
     __shared__ VtxShared sh;
     __shared__ int warp_cnt[kVtxWarps][2];
@@ -223,14 +223,19 @@ k_vertex_count(const __grid_constant__ DevConst c, const ds_tracks trk, const in
     PairSource ps;
     ps.sh = staged ? &sh : nullptr; ps.list = list; ps.n_seeds = n_seeds; ps.nneg = nneg;
     const int64_t npairs = (int64_t)npos * nneg;
-    int mine = 0;
-    for (int64_t k = tid; k < npairs; k += kVtxThreads) {
+    int mine = 0, it = 0;
+    unsigned long long mask = 0ull;   // bit `it`: pair it * kVtxThreads + tid passes (the write kernel computes only those again)
+    for (int64_t k = tid; k < npairs; k += kVtxThreads, ++it) {
         VtxTrack ta, tb;
         int ia, ib;
         pair_tracks(c, trk, ps, k, ta, tb, ia, ib);
         VtxOut o;
-        mine += vertex_pair<kCurved>(c, ta, tb, o) ? 1 : 0;
+        if (vertex_pair<kCurved>(c, ta, tb, o)) {
+            ++mine;
+            if (it < 64) mask |= 1ull << it;
+        }
     }
+    masks[(size_t)e * kVtxThreads + tid] = mask;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) mine += __shfl_xor_sync(0xffffffffu, mine, o);
     if ((tid & 31) == 0) red[tid >> 5] = mine;
@@ -290,7 +295,7 @@ k_vertex_scan(const int32_t *__restrict__ n_per_event, int n_events, int64_t *__
 template <bool kCurved>
 __global__ void __launch_bounds__(kVtxThreads)
 k_vertex_write(const __grid_constant__ DevConst c, const ds_tracks trk, const int32_t *__restrict__ seed_offsets,
-               PairLists pl, const ds_vertices out)
+               PairLists pl, const unsigned long long *__restrict__ masks, const ds_vertices out)
 {
     __shared__ VtxShared sh;
     __shared__ int warp_cnt[kVtxWarps][2];
@@ -311,14 +316,17 @@ k_vertex_write(const __grid_constant__ DevConst c, const ds_tracks trk, const in
     PairSource ps;
     ps.sh = staged ? &sh : nullptr; ps.list = list; ps.n_seeds = n_seeds; ps.nneg = nneg;
     const int64_t npairs = (int64_t)npos * nneg;
+    const unsigned long long mask = masks[(size_t)e * kVtxThreads + tid];
     int64_t written = 0;
-    // S9 again, S10: block-ordered compaction of the passing pairs -> (ia, ib) order
-    for (int64_t tile = 0; tile < npairs; tile += kVtxThreads) {
+    int it = 0;
+    // S9 again for the pairs that passed (known from the count kernel's masks for the first 64 tiles), S10: block-ordered
+    // compaction -> (ia, ib) order
+    for (int64_t tile = 0; tile < npairs; tile += kVtxThreads, ++it) {
         const int64_t k = tile + tid;
         bool pass = false;
         VtxOut o;
         int ia = 0, ib = 0;
-        if (k < npairs) {
+        if (k < npairs && (it >= 64 || ((mask >> it) & 1ull))) {
             VtxTrack ta, tb;
             pair_tracks(c, trk, ps, k, ta, tb, ia, ib);
             pass = vertex_pair<kCurved>(c, ta, tb, o);
@@ -565,13 +573,13 @@ k_vertex_write_w(const __grid_constant__ DevConst c, const ds_tracks trk, const 
     }
 }
 
-// Workspace: list [n_seeds], npos [E], nneg [E] (both variants); masks [E][32] and group sums (warp-per-event variant)
+// Workspace: list [n_seeds], npos [E], nneg [E], pass masks [E][kVtxThreads] (the warp-per-event variant uses [E][32] of it), group sums
 static size_t up256v(size_t v) { return (v + 255) & ~(size_t)255; }
 
 size_t vertex_workspace_bytes(int n_events, int64_t n_seeds)
 {
     const size_t ne = (size_t)(n_events > 0 ? n_events : 1), ns = (size_t)(n_seeds > 0 ? n_seeds : 1);
-    return up256v(sizeof(int32_t) * ns) + 2 * up256v(sizeof(int32_t) * ne) + up256v(sizeof(unsigned long long) * 32 * ne) +
+    return up256v(sizeof(int32_t) * ns) + 2 * up256v(sizeof(int32_t) * ne) + up256v(sizeof(unsigned long long) * kVtxThreads * ne) +
            up256v(sizeof(int32_t) * ((ne + kGroup - 1) / kGroup));
 }
 
@@ -589,7 +597,7 @@ cudaError_t launch_vertex(const DevConst &c, const ds_tracks &trk, const int32_t
     pl.nneg = reinterpret_cast<int32_t *>(w);
     w += up256v(sizeof(int32_t) * ne);
     ww.masks = reinterpret_cast<unsigned long long *>(w);
-    w += up256v(sizeof(unsigned long long) * 32 * ne);
+    w += up256v(sizeof(unsigned long long) * kVtxThreads * ne);
     ww.group_sums = reinterpret_cast<int32_t *>(w);
     const size_t n_groups = (ne + kGroup - 1) / kGroup;
     cudaError_t err = cudaSuccess;
@@ -625,9 +633,9 @@ cudaError_t launch_vertex(const DevConst &c, const ds_tracks &trk, const int32_t
     }
     prof.begin(DS_K_VTX_COUNT, st);
     if (curved)
-        k_vertex_count<true><<<n_events, kVtxThreads, 0, st>>>(c, trk, seed_offsets, pl, out.n_per_event);
+        k_vertex_count<true><<<n_events, kVtxThreads, 0, st>>>(c, trk, seed_offsets, pl, ww.masks, out.n_per_event);
     else
-        k_vertex_count<false><<<n_events, kVtxThreads, 0, st>>>(c, trk, seed_offsets, pl, out.n_per_event);
+        k_vertex_count<false><<<n_events, kVtxThreads, 0, st>>>(c, trk, seed_offsets, pl, ww.masks, out.n_per_event);
     prof.end(st);
     err = cudaGetLastError();
     if (err != cudaSuccess) return err;
@@ -638,9 +646,9 @@ cudaError_t launch_vertex(const DevConst &c, const ds_tracks &trk, const int32_t
     if (err != cudaSuccess) return err;
     prof.begin(DS_K_VTX_WRITE, st);
     if (curved)
-        k_vertex_write<true><<<n_events, kVtxThreads, 0, st>>>(c, trk, seed_offsets, pl, out);
+        k_vertex_write<true><<<n_events, kVtxThreads, 0, st>>>(c, trk, seed_offsets, pl, ww.masks, out);
     else
-        k_vertex_write<false><<<n_events, kVtxThreads, 0, st>>>(c, trk, seed_offsets, pl, out);
+        k_vertex_write<false><<<n_events, kVtxThreads, 0, st>>>(c, trk, seed_offsets, pl, ww.masks, out);
     prof.end(st);
     return cudaGetLastError();
 }
