@@ -20,11 +20,6 @@
 
 namespace ds {
 
-#ifndef DS_TRACK_THREADS
-#define DS_TRACK_THREADS 160
-#endif
-constexpr int kTrackThreads = DS_TRACK_THREADS;
-constexpr int kTrackWarps = kTrackThreads / 32;
 constexpr int kMaxBins = 4 * DS_MAX_SECTORS * kXBins;
 
 struct S2 {
@@ -137,11 +132,11 @@ struct WarpShared {
 };
 static_assert((32 * kMaxFirst - kFirstCap) * 2 >= 4 * kFirstCap * 2, "slot[] holds the Dv1 triplets and their fit queue");
 
-// Block-shared state of k_track (carved from dynamic shared memory, followed by the staged hit arrays).
-template <typename Idx>
+// Block-shared state of k_track (carved from dynamic shared memory, followed by the staged hit arrays); W warps.
+template <typename Idx, int W>
 struct TrackShared {
     unsigned long long bar;
-    WarpShared<Idx> warp[kTrackWarps];
+    WarpShared<Idx> warp[W];
     Idx tab[kMaxBins + 1];                // the event's bin table
 };
 static_assert(kFirstCap <= 512 && kFitCap < 0xfff, "packing of task[] and ffit[]");
@@ -933,35 +928,36 @@ __device__ __forceinline__ void track_chunk_dv1(const DevConst &c, WarpShared<Id
 }
 
 // All seeds of one event: every warp of the block takes an equal share (at most 32 at a time).
+template <int W>
 __device__ __forceinline__ int seed_chunk(int s_begin, int s_end)
 {
-    return min(32, (s_end - s_begin + kTrackWarps - 1) / kTrackWarps);
+    return min(32, (s_end - s_begin + W - 1) / W);
 }
 
-template <typename Idx, bool kDv1>
-__device__ __forceinline__ void track_event(const DevConst &c, TrackShared<Idx> &sh, const EventHits &H,
+template <typename Idx, bool kDv1, int W>
+__device__ __forceinline__ void track_event(const DevConst &c, TrackShared<Idx, W> &sh, const EventHits &H,
                                             const ds_seeds &seeds, int s_begin, int s_end, const ds_tracks &out,
                                             const SeedPre &pre)
 {
     const int wid = threadIdx.x >> 5;
-    const int chunk = seed_chunk(s_begin, s_end);
-    for (int cb = s_begin + wid * chunk; cb < s_end; cb += kTrackWarps * chunk) {
+    const int chunk = seed_chunk<W>(s_begin, s_end);
+    for (int cb = s_begin + wid * chunk; cb < s_end; cb += W * chunk) {
         if (kDv1) track_chunk_dv1<Idx>(c, sh.warp[wid], sh.tab, H, seeds, cb, min(cb + chunk, s_end), out);
         else track_chunk<Idx>(c, sh.warp[wid], sh.tab, H, seeds, cb, min(cb + chunk, s_end), out, pre);
     }
 }
 
-#ifndef DS_TRACK_MINBLOCKS
-#define DS_TRACK_MINBLOCKS 3
-#endif
-template <bool kDv1>
-__global__ void __launch_bounds__(kTrackThreads, DS_TRACK_MINBLOCKS)
+// W warps per block: 5 when three blocks share an SM (the Run-3-like event sizes); events whose staging leaves room for
+// two blocks or one get 8 or 12 warps, so that an SM keeps about the same number of warps busy
+template <bool kDv1, int W, int kMinBlocks>
+__global__ void __launch_bounds__(32 * W, kMinBlocks)
 k_track(const __grid_constant__ DevConst c, const LayoutPtrs L, const ds_seeds seeds,
         const int32_t *__restrict__ hit_offsets, const int32_t *__restrict__ seed_offsets, const ds_tracks out, int cap)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    using Staged = TrackShared<uint16_t>;
-    using Direct = TrackShared<int>;
+    constexpr int kThreads = 32 * W;
+    using Staged = TrackShared<uint16_t, W>;
+    using Direct = TrackShared<int, W>;
     constexpr size_t kHitsAt = (sizeof(Staged) + 15) & ~(size_t)15;
     float *st_x0 = reinterpret_cast<float *>(smem_raw + kHitsAt);   // [cap], then ymin [cap], ymax [cap]
     float *st_ymin = st_x0 + cap, *st_ymax = st_ymin + cap;
@@ -988,7 +984,7 @@ k_track(const __grid_constant__ DevConst c, const LayoutPtrs L, const ds_seeds s
     // the lane's first seed, fetched now so that the load is in flight with the table and the hits
     SeedPre pre;
     {
-        const int chunk = seed_chunk(s_begin, s_end);
+        const int chunk = seed_chunk<W>(s_begin, s_end);
         const int s = s_begin + (tid >> 5) * chunk + (tid & 31);
         pre = load_seed(seeds, s, !kDv1 && (tid & 31) < chunk && s < s_end);
     }
@@ -996,16 +992,16 @@ k_track(const __grid_constant__ DevConst c, const LayoutPtrs L, const ds_seeds s
     const int32_t *gtab = L.bin_offsets + (size_t)e * (nb + 1);
     if (staged) {
         uint16_t *tab = reinterpret_cast<Staged *>(smem_raw)->tab;
-        constexpr int kPer = (kMaxBins + kTrackThreads) / kTrackThreads;
+        constexpr int kPer = (kMaxBins + kThreads) / kThreads;
         int v[kPer];
 #pragma unroll
-        for (int u = 0; u < kPer; ++u) v[u] = gtab[min(tid + u * kTrackThreads, nb)];
+        for (int u = 0; u < kPer; ++u) v[u] = gtab[min(tid + u * kThreads, nb)];
 #pragma unroll
         for (int u = 0; u < kPer; ++u)
-            if (tid + u * kTrackThreads <= nb) tab[tid + u * kTrackThreads] = (uint16_t)v[u];
+            if (tid + u * kThreads <= nb) tab[tid + u * kThreads] = (uint16_t)v[u];
     } else {
         int *tab = reinterpret_cast<Direct *>(smem_raw)->tab;
-        for (int b = tid; b <= nb; b += kTrackThreads) tab[b] = gtab[b];
+        for (int b = tid; b <= nb; b += kThreads) tab[b] = gtab[b];
     }
     __syncthreads();
 
@@ -1015,10 +1011,10 @@ k_track(const __grid_constant__ DevConst c, const LayoutPtrs L, const ds_seeds s
         mbar_wait(bar, 0);
         const int d = h0 - h0a;
         H.x0 = st_x0 + d; H.ymin = st_ymin + d; H.ymax = st_ymax + d;
-        track_event<uint16_t, kDv1>(c, *reinterpret_cast<Staged *>(smem_raw), H, seeds, s_begin, s_end, out, pre);
+        track_event<uint16_t, kDv1, W>(c, *reinterpret_cast<Staged *>(smem_raw), H, seeds, s_begin, s_end, out, pre);
     } else {
         H.x0 = L.sx0 + h0; H.ymin = L.symin + h0; H.ymax = L.symax + h0;
-        track_event<int, kDv1>(c, *reinterpret_cast<Direct *>(smem_raw), H, seeds, s_begin, s_end, out, pre);
+        track_event<int, kDv1, W>(c, *reinterpret_cast<Direct *>(smem_raw), H, seeds, s_begin, s_end, out, pre);
     }
 }
 
@@ -1030,28 +1026,38 @@ cudaError_t launch_track(const DevConst &c, const LayoutPtrs &lay, const ds_seed
     // staging capacity in hits (a multiple of 4, with room for the alignment slack): 12 bytes each; positions of a
     // staged event are stored as uint16_t with 0xffff = none
     const int hint = max_event_hits_hint > 0 ? max_event_hits_hint : 4096;
-    const size_t fixed = ((sizeof(TrackShared<uint16_t>) + 15) & ~(size_t)15);
-    int cap_max = (int)((227 * 1024 - fixed) / 12) & ~3;
-    if (cap_max > 65528) cap_max = 65528;
-    int cap = ((hint + 3) & ~3) + 8;
-    if (cap > cap_max) cap = cap_max;
-    size_t smem = fixed + (size_t)cap * 12;
-    if (smem < sizeof(TrackShared<int>)) smem = sizeof(TrackShared<int>);   // the layout of an event that is not staged
-    // opt in to the full 227 KB of dynamic shared memory; per device, cheap and the same value for every caller, so it is
-    // simply set at every launch (handles on several devices and host threads share this code)
-    auto launch = [&](auto kernel) -> cudaError_t {
+    auto launch = [&](auto kernel, size_t bytes_staged, size_t bytes_direct, int threads) -> cudaError_t {
+        const size_t fixed = (bytes_staged + 15) & ~(size_t)15;
+        int cap_max = (int)((227 * 1024 - fixed) / 12) & ~3;
+        if (cap_max > 65528) cap_max = 65528;
+        int cap = ((hint + 3) & ~3) + 8;
+        if (cap > cap_max) cap = cap_max;
+        size_t smem = fixed + (size_t)cap * 12;
+        if (smem < bytes_direct) smem = bytes_direct;   // the layout of an event that is not staged
+        // opt in to the full 227 KB of dynamic shared memory; per device, cheap and the same value for every caller, so
+        // it is simply set at every launch (handles on several devices and host threads share this code)
         cudaFuncAttributes fa;
         cudaError_t aerr = cudaFuncGetAttributes(&fa, kernel);
         if (aerr != cudaSuccess) return aerr;
         aerr = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - (int)fa.sharedSizeBytes);
         if (aerr != cudaSuccess) return aerr;
         prof.begin(DS_K_TRACK, st);
-        kernel<<<n_events, kTrackThreads, smem, st>>>(c, lay, seeds, hit_offsets, seed_offsets, out, cap);
+        kernel<<<n_events, threads, smem, st>>>(c, lay, seeds, hit_offsets, seed_offsets, out, cap);
         prof.end(st);
         return cudaGetLastError();
     };
+    // blocks per SM that the 5-warp layout would reach with this hint decide the warps per block
+    const size_t smem5 = ((sizeof(TrackShared<uint16_t, 5>) + 15) & ~(size_t)15) + (size_t)(((hint + 3) & ~3) + 8) * 12 + 1024;
+    const int per_sm = (int)((228 * 1024) / smem5);
     // Dv1 (triplet search, P:107-P:111) and Dv0 are separate instantiations: the Dv0 hot path carries none of the other's code
-    return c.dv1 ? launch(k_track<true>) : launch(k_track<false>);
+    if (per_sm >= 3)
+        return c.dv1 ? launch(k_track<true, 5, 3>, sizeof(TrackShared<uint16_t, 5>), sizeof(TrackShared<int, 5>), 160)
+                     : launch(k_track<false, 5, 3>, sizeof(TrackShared<uint16_t, 5>), sizeof(TrackShared<int, 5>), 160);
+    if (per_sm == 2)
+        return c.dv1 ? launch(k_track<true, 8, 2>, sizeof(TrackShared<uint16_t, 8>), sizeof(TrackShared<int, 8>), 256)
+                     : launch(k_track<false, 8, 2>, sizeof(TrackShared<uint16_t, 8>), sizeof(TrackShared<int, 8>), 256);
+    return c.dv1 ? launch(k_track<true, 12, 1>, sizeof(TrackShared<uint16_t, 12>), sizeof(TrackShared<int, 12>), 384)
+                 : launch(k_track<false, 12, 1>, sizeof(TrackShared<uint16_t, 12>), sizeof(TrackShared<int, 12>), 384);
 }
 
 }  // namespace ds
