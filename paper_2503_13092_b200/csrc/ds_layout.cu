@@ -94,7 +94,7 @@ __device__ __forceinline__ void stage_field(T *buf, const T *__restrict__ src, i
     }
 }
 
-__global__ void __launch_bounds__(kLayoutThreads)
+__global__ void __launch_bounds__(2 * kLayoutThreads)
 k_layout(const __grid_constant__ DevConst c, const LayoutPtrs p, const int32_t *__restrict__ hit_offsets, int cap, bool bulk)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -272,7 +272,9 @@ cudaError_t launch_layout(const DevConst &c, const LayoutPtrs &p, const int32_t 
                            reinterpret_cast<uintptr_t>(p.w) | reinterpret_cast<uintptr_t>(p.id);
     const bool bulk = (bits & 15) == 0;
     prof.begin(DS_K_LAYOUT, st);
-    k_layout<<<n_events, kLayoutThreads, smem, st>>>(c, p, hit_offsets, cap, bulk);
+    // events so large that one block fills an SM's shared memory get twice the threads (every loop strides by blockDim.x)
+    const int threads = smem + 1024 > (228 * 1024) / 2 ? 2 * kLayoutThreads : kLayoutThreads;
+    k_layout<<<n_events, threads, smem, st>>>(c, p, hit_offsets, cap, bulk);
     prof.end(st);
     return cudaGetLastError();
 }
