@@ -285,6 +285,11 @@ int ds_profile_enable(ds_handle *h, int on);
 /* Waits for all recorded events (blocks the calling thread until the bracketed kernels have finished), adds their
  * elapsed times into *out (HOST) and forgets them.  Counters start from zero at every call. */
 int ds_profile_read(ds_handle *h, ds_profile *out);
+/* Measured fp64 FMA throughput of the handle's device in TFLOP/s (a register-resident DFMA loop on every SM, timed with
+ * CUDA events; blocks the calling thread for a few milliseconds).  The denominator of the ALU fraction bench.py reports
+ * for the vertex kernels on BASELINE configs[3]. */
+int ds_measure_dfma_peak(ds_handle *h, double *tflops);
+
 /* Name of kernel k ("k_layout", ...), NULL if k is out of range. */
 const char *ds_kernel_name(int k);
 

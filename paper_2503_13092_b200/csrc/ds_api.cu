@@ -515,6 +515,47 @@ int ds_profile_read(ds_handle *h, ds_profile *out)
     return rc;
 }
 
+namespace {
+__global__ void k_fma_peak(double *out, int iters)
+{
+    double a0 = threadIdx.x * 1e-9, a1 = a0 + 1.0, a2 = a0 + 2.0, a3 = a0 + 3.0, a4 = a0 + 4.0, a5 = a0 + 5.0, a6 = a0 + 6.0, a7 = a0 + 7.0;
+    const double m = 1.0000001, b = 1e-9;
+    for (int i = 0; i < iters; ++i) {
+        a0 = fma(a0, m, b); a1 = fma(a1, m, b); a2 = fma(a2, m, b); a3 = fma(a3, m, b);
+        a4 = fma(a4, m, b); a5 = fma(a5, m, b); a6 = fma(a6, m, b); a7 = fma(a7, m, b);
+    }
+    if (a0 + a1 + a2 + a3 + a4 + a5 + a6 + a7 == -1.0) out[0] = a0;   // never true: keeps the loop alive
+}
+}  // namespace
+
+int ds_measure_dfma_peak(ds_handle *h, double *tflops)
+{
+    if (!h || !tflops) return DS_E_ARG;
+    DeviceGuard guard(h->device);
+    if (!guard.ok) return DS_E_CUDA;
+    double *d = nullptr;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    if (cudaMalloc(&d, sizeof(double)) != cudaSuccess || cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) {
+        cudaGetLastError();
+        if (d) cudaFree(d);
+        if (e0) cudaEventDestroy(e0);
+        return DS_E_CUDA;
+    }
+    const int sms = h->n_sm > 0 ? h->n_sm : 148, threads = 256, blocks = sms * 8, iters = 1 << 15;
+    k_fma_peak<<<blocks, threads>>>(d, 256);   // warm-up
+    cudaEventRecord(e0);
+    k_fma_peak<<<blocks, threads>>>(d, iters);
+    cudaEventRecord(e1);
+    float ms = 0.f;
+    const cudaError_t err = cudaEventSynchronize(e1) == cudaSuccess ? cudaEventElapsedTime(&ms, e0, e1) : cudaErrorUnknown;
+    cudaFree(d);
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    if (err != cudaSuccess || !(ms > 0.f)) { cudaGetLastError(); return DS_E_CUDA; }
+    *tflops = 2.0 * 8.0 * (double)iters * (double)threads * (double)blocks / ((double)ms * 1e-3) / 1e12;
+    return DS_OK;
+}
+
 const char *ds_kernel_name(int k)
 {
     static const char *names[DS_K_COUNT] = {"k_layout", "k_track", "k_mlp", "k_vertex_count", "k_vertex_scan", "k_vertex_write",

@@ -376,6 +376,14 @@ def ds_process_host(h, hits, seeds, hit_offsets, seed_offsets, n_events, params:
     return total.value
 
 
+def ds_measure_dfma_peak(h) -> float:
+    """Measured fp64 FMA throughput of the device in TFLOP/s."""
+    v = ct.c_double(0.0)
+    lib().ds_measure_dfma_peak.argtypes = [ct.c_void_p, ct.POINTER(ct.c_double)]
+    _check(lib().ds_measure_dfma_peak(h, ct.byref(v)), "ds_measure_dfma_peak")
+    return v.value
+
+
 def ds_profile_enable(h, on: bool) -> None:
     _check(lib().ds_profile_enable(h, 1 if on else 0), "ds_profile_enable")
 

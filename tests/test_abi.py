@@ -23,7 +23,7 @@ def test_exports_every_declared_symbol():
     names = declared_functions()
     assert {"ds_create", "ds_destroy", "ds_upload_geometry", "ds_layout", "ds_extrapolate", "ds_reconstruct",
             "ds_ghost_killer", "ds_clone_kill", "ds_upload_line_nets", "ds_lines", "ds_vertex", "ds_process_host", "ds_workspace_bytes", "ds_vertex_workspace_bytes",
-            "ds_profile_enable", "ds_profile_read", "ds_kernel_name", "ds_error_string", "ds_version"} <= set(names)
+            "ds_profile_enable", "ds_profile_read", "ds_measure_dfma_peak", "ds_kernel_name", "ds_error_string", "ds_version"} <= set(names)
     for n in names:
         assert hasattr(L, n), n
         assert hasattr(pk, n) or n in ("ds_kernel_name",), f"binding lacks {n}"
