@@ -317,16 +317,54 @@ k_vertex_write(const __grid_constant__ DevConst c, const ds_tracks trk, const in
     ps.sh = staged ? &sh : nullptr; ps.list = list; ps.n_seeds = n_seeds; ps.nneg = nneg;
     const int64_t npairs = (int64_t)npos * nneg;
     const unsigned long long mask = masks[(size_t)e * kVtxThreads + tid];
-    int64_t written = 0;
-    int it = 0;
-    // S9 again for the pairs that passed (known from the count kernel's masks for the first 64 tiles), S10: block-ordered
-    // compaction -> (ia, ib) order
-    for (int64_t tile = 0; tile < npairs; tile += kVtxThreads, ++it) {
+    // S10 for the first 64 tiles from the masks alone: per tile and warp the number of passing pairs (ballots, no pair
+    // arithmetic), one barrier, a prefix over (tile, warp) -- every passing pair then knows its output position, and S9 is
+    // computed again for those pairs only, each by the thread that owns it
+    __shared__ int s_cnt[64][kVtxWarps];   // then: offset of (tile, warp) inside the event
+    __shared__ int s_total;
+    const int lane = tid & 31, wid = tid >> 5;
+    const int64_t tiles = (npairs + kVtxThreads - 1) / kVtxThreads;
+    const int mtiles = (int)(tiles < 64 ? tiles : 64);
+    for (int it = 0; it < mtiles; ++it) {
+        const unsigned m = __ballot_sync(0xffffffffu, ((mask >> it) & 1ull) != 0);
+        if (lane == 0) s_cnt[it][wid] = __popc(m);
+    }
+    __syncthreads();
+    if (tid == 0) {
+        int run = 0;
+        for (int it = 0; it < mtiles; ++it)
+            for (int w = 0; w < kVtxWarps; ++w) {
+                const int n = s_cnt[it][w];
+                s_cnt[it][w] = run;
+                run += n;
+            }
+        s_total = run;
+    }
+    __syncthreads();
+    for (int it = 0; it < mtiles; ++it) {
+        const bool bit = ((mask >> it) & 1ull) != 0;
+        const unsigned m = __ballot_sync(0xffffffffu, bit);
+        if (!bit) continue;
+        VtxTrack ta, tb;
+        VtxOut o;
+        int ia, ib;
+        pair_tracks(c, trk, ps, (int64_t)it * kVtxThreads + tid, ta, tb, ia, ib);
+        vertex_pair<kCurved>(c, ta, tb, o);   // passes again: same arithmetic
+        const int64_t pos = o0 + s_cnt[it][wid] + __popc(m & lanemask_lt());
+        if (pos < out.capacity) {
+            out.evt[pos] = e; out.ia[pos] = ia; out.ib[pos] = ib; out.flags[pos] = o.flags;
+            out.x[pos] = (float)o.x; out.y[pos] = (float)o.y; out.z[pos] = (float)o.z; out.doca[pos] = (float)o.doca;
+            out.m_pipi[pos] = (float)o.m_pipi; out.m_ppi[pos] = (float)o.m_ppi;
+        }
+    }
+    // tiles beyond the reach of the mask: every pair again, block-ordered compaction tile by tile
+    int64_t written = s_total;
+    for (int64_t tile = (int64_t)64 * kVtxThreads; tile < npairs; tile += kVtxThreads) {
         const int64_t k = tile + tid;
         bool pass = false;
         VtxOut o;
         int ia = 0, ib = 0;
-        if (k < npairs && (it >= 64 || ((mask >> it) & 1ull))) {
+        if (k < npairs) {
             VtxTrack ta, tb;
             pair_tracks(c, trk, ps, k, ta, tb, ia, ib);
             pass = vertex_pair<kCurved>(c, ta, tb, o);
