@@ -327,6 +327,22 @@ def main():
     events_all = shard.sum_over_ranks(events_rank, dev)
     value = events_all * args.steps / (ms_total * 1e-3)
 
+    # ---- spread: the same step K more times, each timed on its own (median and best) ---------------------------------
+    per_step = []
+    for _ in range(args.steps):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(main_stream)
+        for s in streams:
+            s.wait_stream(main_stream)
+        step()
+        for s in streams:
+            main_stream.wait_stream(s)
+        b.record(main_stream)
+        torch.cuda.synchronize()
+        per_step.append(a.elapsed_time(b))
+    pk.ds_profile_read(ds.h)                      # drop the events of these steps
+    step_ms = {"median": statistics.median(per_step), "best": min(per_step), "n": len(per_step)}
+
     # ---- per-kernel pass: the same K steps, same launches, on ONE stream so that a kernel's event pair times that kernel
     #      alone (in the two-stream region above a pair also spans whatever the other stream runs at the same time) ----------
     def step_one_stream():
@@ -439,7 +455,7 @@ def main():
     if rank == 0:
         print(json.dumps({
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-            "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "ms_per_step": ms_total / args.steps, "step_ms": step_ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
             "config": {"workload": ("BASELINE configs[4]: cfg-1 generator, seed 4, device-resident SoA" if CFG == 4 else
                                     f"BASELINE configs[{CFG}] generator, device-resident SoA (not the metric's workload)"),
