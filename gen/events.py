@@ -382,3 +382,22 @@ def with_clone_seeds(d: dict, every: int = 3, seed: int = 7) -> dict:
             parts[k] += [v[a:b], c]
         new_so.append(new_so[-1] + (b - a) + len(dup))
     return dict(d, seeds={k: np.concatenate(v) for k, v in parts.items()}, seed_offsets=np.array(new_so, dtype=np.int32))
+
+
+def with_hit_jitter(d: dict, seed: int = 11, dz: float = 2.0, shrink: float = 20.0) -> dict:
+    """Per-hit z, weight and y range that differ from hit to hit (ds.h allows all three): z = plane z + U(-dz, dz), w drawn
+    from three values (1/0.054^2, 1/0.08^2, 1/0.03^2), [ymin, ymax] shrunk by U(0, shrink) on either side inside the sector.
+    The generated configurations give every hit of a layer the same z and w and the full sector range, which leaves the
+    per-hit reads of the kernels (and of the oracle) undiscriminated; this transform is the input of the tests that close
+    that.  Input recipe only."""
+    rng = np.random.default_rng(seed)
+    h = d["hits"]
+    n = len(h["id"])
+    dt = h["x0"].dtype
+    wvals = np.array([1.0 / 0.054 ** 2, 1.0 / 0.08 ** 2, 1.0 / 0.03 ** 2])
+    hits = dict(h)
+    hits["z"] = (h["z"].astype(np.float64) + rng.uniform(-dz, dz, n)).astype(dt)
+    hits["w"] = wvals[rng.integers(0, 3, n)].astype(dt)
+    hits["ymin"] = (h["ymin"].astype(np.float64) + rng.uniform(0.0, shrink, n)).astype(dt)
+    hits["ymax"] = (h["ymax"].astype(np.float64) - rng.uniform(0.0, shrink, n)).astype(dt)
+    return dict(d, hits=hits)

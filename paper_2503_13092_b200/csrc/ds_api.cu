@@ -399,9 +399,55 @@ int ds_process_host(ds_handle *h, const ds_hits *hits, const ds_seeds *seeds, co
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const size_t nh = (size_t)hits->n, ns = (size_t)seeds->n, ne = (size_t)n_events, cap = (size_t)out_vertices->capacity;
     const size_t ws_rec = layout_bytes(c.n_bins, n_events, hits->n), ws_vtx = vertex_workspace_bytes(n_events, seeds->n);
-    const size_t need = 6 * up256(4 * nh + 4) + 6 * up256(4 * ns + 4) + 2 * up256(4 * (ne + 1)) + 10 * up256(4 * ns + 4) +
-                        up256(16 * ns + 16) + 10 * up256(4 * cap + 4) + up256(4 * ne + 4) + up256(8 * (ne + 1)) + 256 +
-                        ws_rec + ws_vtx;
+    // The arena is carved by ONE piece of code, run twice: first on a null base to add up the bytes (so that the size
+    // can never disagree with the carving), then on the arena.
+    cudaError_t err = cudaSuccess;
+    ds_hits dh;
+    ds_seeds dsd;
+    ds_tracks dt;
+    ds_vertices dv;
+    const int32_t *d_hoff = nullptr, *d_soff = nullptr;
+    void *wrec = nullptr, *wvtx = nullptr;
+    auto carve = [&](unsigned char *base, bool copy) -> size_t {
+        size_t off = 0;
+        auto take = [&](size_t bytes) { unsigned char *r = base + off; off += up256(bytes); return r; };
+        auto h2d = [&](const void *src, size_t bytes) -> void * {
+            void *d = take(bytes + 4);
+            if (copy && bytes && err == cudaSuccess) err = cudaMemcpyAsync(d, src, bytes, cudaMemcpyHostToDevice, st);
+            return d;
+        };
+        dh.n = hits->n;
+        dh.x0 = (const float *)h2d(hits->x0, 4 * nh); dh.z = (const float *)h2d(hits->z, 4 * nh);
+        dh.ymin = (const float *)h2d(hits->ymin, 4 * nh); dh.ymax = (const float *)h2d(hits->ymax, 4 * nh);
+        dh.w = (const float *)h2d(hits->w, 4 * nh); dh.id = (const int32_t *)h2d(hits->id, 4 * nh);
+        dsd.n = seeds->n;
+        dsd.x = (const float *)h2d(seeds->x, 4 * ns); dsd.y = (const float *)h2d(seeds->y, 4 * ns);
+        dsd.tx = (const float *)h2d(seeds->tx, 4 * ns); dsd.ty = (const float *)h2d(seeds->ty, 4 * ns);
+        dsd.qop = (const float *)h2d(seeds->qop, 4 * ns);
+        {
+            void *d = h2d(seeds->chi2, seeds->chi2 ? 4 * ns : 0);
+            dsd.chi2 = seeds->chi2 ? (const float *)d : nullptr;
+        }
+        d_hoff = (const int32_t *)h2d(hit_offsets, 4 * (ne + 1));
+        d_soff = (const int32_t *)h2d(seed_offsets, 4 * (ne + 1));
+        dt.n = seeds->n;
+        dt.x = (float *)take(4 * ns + 4); dt.y = (float *)take(4 * ns + 4); dt.tx = (float *)take(4 * ns + 4);
+        dt.ty = (float *)take(4 * ns + 4); dt.qop = (float *)take(4 * ns + 4); dt.chi2 = (float *)take(4 * ns + 4);
+        dt.score = (float *)take(4 * ns + 4); dt.nhits = (int32_t *)take(4 * ns + 4); dt.found = (int32_t *)take(4 * ns + 4);
+        dt.keep = (int32_t *)take(4 * ns + 4); dt.hit = (int32_t *)take(16 * ns + 16);
+        dv.capacity = out_vertices->capacity;
+        dv.evt = (int32_t *)take(4 * cap + 4); dv.ia = (int32_t *)take(4 * cap + 4); dv.ib = (int32_t *)take(4 * cap + 4);
+        dv.x = (float *)take(4 * cap + 4); dv.y = (float *)take(4 * cap + 4); dv.z = (float *)take(4 * cap + 4);
+        dv.doca = (float *)take(4 * cap + 4); dv.m_pipi = (float *)take(4 * cap + 4); dv.m_ppi = (float *)take(4 * cap + 4);
+        dv.flags = (int32_t *)take(4 * cap + 4);
+        dv.n_per_event = (int32_t *)take(4 * ne + 4);
+        dv.offsets = (int64_t *)take(8 * (ne + 1));
+        dv.overflow = (int32_t *)take(256);
+        wrec = take(ws_rec);
+        wvtx = take(ws_vtx);
+        return off;
+    };
+    const size_t need = carve(nullptr, false);
     if (need > h->arena_bytes) {
         if (h->arena) cudaFree(h->arena);
         h->arena = nullptr;
@@ -413,46 +459,7 @@ int ds_process_host(ds_handle *h, const ds_hits *hits, const ds_seeds *seeds, co
         }
         h->arena_bytes = want;
     }
-    unsigned char *w = h->arena;
-    auto take = [&](size_t bytes) { unsigned char *r = w; w += up256(bytes); return r; };
-    cudaError_t err = cudaSuccess;
-    auto h2d = [&](const void *src, size_t bytes) -> void * {
-        void *d = take(bytes + 4);
-        if (bytes && err == cudaSuccess) err = cudaMemcpyAsync(d, src, bytes, cudaMemcpyHostToDevice, st);
-        return d;
-    };
-    ds_hits dh;
-    dh.n = hits->n;
-    dh.x0 = (const float *)h2d(hits->x0, 4 * nh); dh.z = (const float *)h2d(hits->z, 4 * nh);
-    dh.ymin = (const float *)h2d(hits->ymin, 4 * nh); dh.ymax = (const float *)h2d(hits->ymax, 4 * nh);
-    dh.w = (const float *)h2d(hits->w, 4 * nh); dh.id = (const int32_t *)h2d(hits->id, 4 * nh);
-    ds_seeds dsd;
-    dsd.n = seeds->n;
-    dsd.x = (const float *)h2d(seeds->x, 4 * ns); dsd.y = (const float *)h2d(seeds->y, 4 * ns);
-    dsd.tx = (const float *)h2d(seeds->tx, 4 * ns); dsd.ty = (const float *)h2d(seeds->ty, 4 * ns);
-    dsd.qop = (const float *)h2d(seeds->qop, 4 * ns);
-    {
-        void *d = h2d(seeds->chi2, seeds->chi2 ? 4 * ns : 0);
-        dsd.chi2 = seeds->chi2 ? (const float *)d : nullptr;
-    }
-    const int32_t *d_hoff = (const int32_t *)h2d(hit_offsets, 4 * (ne + 1));
-    const int32_t *d_soff = (const int32_t *)h2d(seed_offsets, 4 * (ne + 1));
-    ds_tracks dt;
-    dt.n = seeds->n;
-    dt.x = (float *)take(4 * ns + 4); dt.y = (float *)take(4 * ns + 4); dt.tx = (float *)take(4 * ns + 4);
-    dt.ty = (float *)take(4 * ns + 4); dt.qop = (float *)take(4 * ns + 4); dt.chi2 = (float *)take(4 * ns + 4);
-    dt.score = (float *)take(4 * ns + 4); dt.nhits = (int32_t *)take(4 * ns + 4); dt.found = (int32_t *)take(4 * ns + 4);
-    dt.keep = (int32_t *)take(4 * ns + 4); dt.hit = (int32_t *)take(16 * ns + 16);
-    ds_vertices dv;
-    dv.capacity = out_vertices->capacity;
-    dv.evt = (int32_t *)take(4 * cap + 4); dv.ia = (int32_t *)take(4 * cap + 4); dv.ib = (int32_t *)take(4 * cap + 4);
-    dv.x = (float *)take(4 * cap + 4); dv.y = (float *)take(4 * cap + 4); dv.z = (float *)take(4 * cap + 4);
-    dv.doca = (float *)take(4 * cap + 4); dv.m_pipi = (float *)take(4 * cap + 4); dv.m_ppi = (float *)take(4 * cap + 4);
-    dv.flags = (int32_t *)take(4 * cap + 4);
-    dv.n_per_event = (int32_t *)take(4 * ne + 4);
-    dv.offsets = (int64_t *)take(8 * (ne + 1));
-    dv.overflow = (int32_t *)take(256);
-    void *wrec = take(ws_rec), *wvtx = take(ws_vtx);
+    carve(h->arena, true);
     if (err != cudaSuccess) { cudaGetLastError(); return DS_E_CUDA; }
 
     LayoutPtrs L;

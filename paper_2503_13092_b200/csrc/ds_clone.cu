@@ -72,9 +72,9 @@ k_clone(const __grid_constant__ DevConst c, const int32_t *__restrict__ seed_off
         }
         return;
     }
-    // more found tracks than the staging holds: judge from the records; a removed track is first only marked (in a field
-    // the judgement does not read), the records change after every thread has read them
-    constexpr unsigned kMark = 0x7fc0c10eu;   // a NaN payload no sigmoid produces
+    // more found tracks than the staging holds: judge from the records; a removed track is first only marked (found = 2:
+    // the judgement only asks found != 0, and k_track has written the field), the records change after every thread has
+    // read them
     for (int i = tid; i < n; i += kCloneThreads) {
         if (!trk.found[s0 + i]) continue;
         const int4 hi = ghit[i];
@@ -85,11 +85,11 @@ k_clone(const __grid_constant__ DevConst c, const int32_t *__restrict__ seed_off
             const double sj = score_of(j);
             if (sj < si || (sj == si && j < i)) killed = true;
         }
-        if (killed) trk.score[s0 + i] = __uint_as_float(kMark);
+        if (killed) trk.found[s0 + i] = 2;
     }
     __syncthreads();
     for (int i = tid; i < n; i += kCloneThreads)
-        if (__float_as_uint(trk.score[s0 + i]) == kMark) reset(s0 + i);
+        if (trk.found[s0 + i] == 2) reset(s0 + i);
 }
 
 cudaError_t launch_clone(const DevConst &c, const int32_t *seed_offsets, int n_events, const ds_tracks &trk, cudaStream_t st,

@@ -91,6 +91,10 @@ __device__ __forceinline__ void mbar_init(unsigned long long *bar, int count)
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
 }
 
+// Orders this thread's earlier generic-proxy accesses to shared memory (and, after a barrier, those of the threads that
+// arrived at it) before its later async-proxy operations (bulk copies) on the same bytes.
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
 __device__ __forceinline__ void mbar_expect_tx(unsigned long long *bar, uint32_t bytes)
 {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_addr(bar)), "r"(bytes) : "memory");
@@ -157,6 +161,26 @@ struct Prof {
         pool.clear();
     }
 };
+
+// Opt a kernel in to the full 227 KB of dynamic shared memory, once per (kernel instantiation, device): `done` is a static
+// bit mask per instantiation (bit = device ordinal; devices >= 64 simply repeat the call), so the two runtime calls are
+// not paid at every launch.  Thread-safe: the attribute is idempotent, the mask only ever gains bits.
+template <typename K>
+inline cudaError_t opt_in_max_smem(K kernel, unsigned long long *done)
+{
+    int dev = 0;
+    cudaError_t err = cudaGetDevice(&dev);
+    if (err != cudaSuccess) return err;
+    const unsigned long long bit = dev < 64 ? 1ull << dev : 0ull;
+    if (bit && (__atomic_load_n(done, __ATOMIC_ACQUIRE) & bit)) return cudaSuccess;
+    cudaFuncAttributes fa;
+    err = cudaFuncGetAttributes(&fa, kernel);
+    if (err != cudaSuccess) return err;
+    err = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - (int)fa.sharedSizeBytes);
+    if (err != cudaSuccess) return err;
+    if (bit) __atomic_fetch_or(done, bit, __ATOMIC_RELEASE);
+    return cudaSuccess;
+}
 
 // ---- launchers (host side, defined in the .cu files; all enqueue on `st` and return the launch error) ------------
 struct LayoutPtrs {

@@ -83,6 +83,9 @@ __device__ __forceinline__ void stage_field(T *buf, const T *__restrict__ src, i
     const int h1dn = bulk ? max(h1 & ~3, h0a) : h0a;          // bulk part: [h0a, h1dn); it may start before h0
     if (threadIdx.x == 0) {
         const uint32_t bytes = 4u * (uint32_t)(h1dn - h0a);
+        // the buffer may have been written and read by ordinary (generic-proxy) accesses of the whole block before the
+        // __syncthreads that precedes this call: order them before the async-proxy write of the bulk copy
+        fence_proxy_async();
         mbar_expect_tx(bar, bytes);
         if (bytes) bulk_g2s(buf, src + h0a, bytes, bar);
     }
@@ -259,12 +262,8 @@ cudaError_t launch_layout(const DevConst &c, const LayoutPtrs &p, const int32_t 
     if (cap_max > 65532) cap_max = 65532;
     if (cap > cap_max) cap = cap_max;
     const size_t smem = layout_smem_bytes(cap, c.n_bins);
-    // opt in to the full 227 KB of dynamic shared memory; per device, cheap and the same value for every caller, so it is
-    // simply set at every launch (handles on several devices and host threads share this code)
-    cudaFuncAttributes fa;
-    cudaError_t aerr = cudaFuncGetAttributes(&fa, k_layout);
-    if (aerr != cudaSuccess) return aerr;
-    aerr = cudaFuncSetAttribute(k_layout, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - (int)fa.sharedSizeBytes);
+    static unsigned long long opted = 0;
+    const cudaError_t aerr = opt_in_max_smem(k_layout, &opted);
     if (aerr != cudaSuccess) return aerr;
     // the bulk copies need 16-byte aligned sources (offsets inside the arrays are handled by the kernel)
     const uintptr_t bits = reinterpret_cast<uintptr_t>(p.x0) | reinterpret_cast<uintptr_t>(p.z) |

@@ -1026,7 +1026,7 @@ cudaError_t launch_track(const DevConst &c, const LayoutPtrs &lay, const ds_seed
     // staging capacity in hits (a multiple of 4, with room for the alignment slack): 12 bytes each; positions of a
     // staged event are stored as uint16_t with 0xffff = none
     const int hint = max_event_hits_hint > 0 ? max_event_hits_hint : 4096;
-    auto launch = [&](auto kernel, size_t bytes_staged, size_t bytes_direct, int threads) -> cudaError_t {
+    auto launch = [&](auto kernel, unsigned long long *opted, size_t bytes_staged, size_t bytes_direct, int threads) -> cudaError_t {
         const size_t fixed = (bytes_staged + 15) & ~(size_t)15;
         int cap_max = (int)((227 * 1024 - fixed) / 12) & ~3;
         if (cap_max > 65528) cap_max = 65528;
@@ -1034,12 +1034,7 @@ cudaError_t launch_track(const DevConst &c, const LayoutPtrs &lay, const ds_seed
         if (cap > cap_max) cap = cap_max;
         size_t smem = fixed + (size_t)cap * 12;
         if (smem < bytes_direct) smem = bytes_direct;   // the layout of an event that is not staged
-        // opt in to the full 227 KB of dynamic shared memory; per device, cheap and the same value for every caller, so
-        // it is simply set at every launch (handles on several devices and host threads share this code)
-        cudaFuncAttributes fa;
-        cudaError_t aerr = cudaFuncGetAttributes(&fa, kernel);
-        if (aerr != cudaSuccess) return aerr;
-        aerr = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - (int)fa.sharedSizeBytes);
+        const cudaError_t aerr = opt_in_max_smem(kernel, opted);
         if (aerr != cudaSuccess) return aerr;
         prof.begin(DS_K_TRACK, st);
         kernel<<<n_events, threads, smem, st>>>(c, lay, seeds, hit_offsets, seed_offsets, out, cap);
@@ -1050,14 +1045,15 @@ cudaError_t launch_track(const DevConst &c, const LayoutPtrs &lay, const ds_seed
     const size_t smem5 = ((sizeof(TrackShared<uint16_t, 5>) + 15) & ~(size_t)15) + (size_t)(((hint + 3) & ~3) + 8) * 12 + 1024;
     const int per_sm = (int)((228 * 1024) / smem5);
     // Dv1 (triplet search, P:107-P:111) and Dv0 are separate instantiations: the Dv0 hot path carries none of the other's code
+    static unsigned long long opted[6] = {0, 0, 0, 0, 0, 0};
     if (per_sm >= 3)
-        return c.dv1 ? launch(k_track<true, 5, 3>, sizeof(TrackShared<uint16_t, 5>), sizeof(TrackShared<int, 5>), 160)
-                     : launch(k_track<false, 5, 3>, sizeof(TrackShared<uint16_t, 5>), sizeof(TrackShared<int, 5>), 160);
+        return c.dv1 ? launch(k_track<true, 5, 3>, &opted[0], sizeof(TrackShared<uint16_t, 5>), sizeof(TrackShared<int, 5>), 160)
+                     : launch(k_track<false, 5, 3>, &opted[1], sizeof(TrackShared<uint16_t, 5>), sizeof(TrackShared<int, 5>), 160);
     if (per_sm == 2)
-        return c.dv1 ? launch(k_track<true, 8, 2>, sizeof(TrackShared<uint16_t, 8>), sizeof(TrackShared<int, 8>), 256)
-                     : launch(k_track<false, 8, 2>, sizeof(TrackShared<uint16_t, 8>), sizeof(TrackShared<int, 8>), 256);
-    return c.dv1 ? launch(k_track<true, 12, 1>, sizeof(TrackShared<uint16_t, 12>), sizeof(TrackShared<int, 12>), 384)
-                 : launch(k_track<false, 12, 1>, sizeof(TrackShared<uint16_t, 12>), sizeof(TrackShared<int, 12>), 384);
+        return c.dv1 ? launch(k_track<true, 8, 2>, &opted[2], sizeof(TrackShared<uint16_t, 8>), sizeof(TrackShared<int, 8>), 256)
+                     : launch(k_track<false, 8, 2>, &opted[3], sizeof(TrackShared<uint16_t, 8>), sizeof(TrackShared<int, 8>), 256);
+    return c.dv1 ? launch(k_track<true, 12, 1>, &opted[4], sizeof(TrackShared<uint16_t, 12>), sizeof(TrackShared<int, 12>), 384)
+                 : launch(k_track<false, 12, 1>, &opted[5], sizeof(TrackShared<uint16_t, 12>), sizeof(TrackShared<int, 12>), 384);
 }
 
 }  // namespace ds

@@ -457,6 +457,15 @@ class Downstream:
         nbytes = ds_vertex_workspace_bytes(self.h, n_events, n_seeds)
         return self.torch.empty(nbytes, dtype=self.torch.uint8, device=self.device)
 
+    def _on_stream(self, tensor, stream):
+        """A temporary the library uses on `stream` after this Python call has returned: tell the caching allocator, so that
+        the block is not handed out again while the kernels still run on a stream other than the current one."""
+        if stream is not None and hasattr(stream, "cuda_stream"):
+            tensor.record_stream(stream)
+        elif isinstance(stream, int):
+            tensor.record_stream(self.torch.cuda.ExternalStream(stream, device=self.device))
+        return tensor
+
     # -- the calls ---------------------------------------------------------------------------------------------------
     def layout(self, hits: dict, hit_offsets, stream=None) -> dict:
         t = self.torch
@@ -479,7 +488,7 @@ class Downstream:
         if out is None:
             out = self.empty_tracks(seeds["x"].numel())
         if workspace is None:
-            workspace = self.workspace(ne, hits["id"].numel(), seeds["x"].numel())
+            workspace = self._on_stream(self.workspace(ne, hits["id"].numel(), seeds["x"].numel()), stream)
         ds_reconstruct(self.h, hits, seeds, hit_offsets, seed_offsets, ne, self.params, out, workspace, stream)
         return out
 
@@ -507,7 +516,7 @@ class Downstream:
         if out is None:
             out = self.empty_vertices(capacity if capacity is not None else 1 << 20, ne)
         if workspace is None:
-            workspace = self.vertex_workspace(ne, tracks["x"].numel())
+            workspace = self._on_stream(self.vertex_workspace(ne, tracks["x"].numel()), stream)
         ds_vertex(self.h, tracks, seed_offsets, ne, self.params, out, out["capacity"], workspace, stream)
         return out
 

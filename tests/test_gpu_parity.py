@@ -76,9 +76,12 @@ def check_both(ds, d, orc_mlp, params=None):
 
 
 # ---- S1 layout ---------------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("cfg,n_events,hint", [(0, 10, 0), (1, 64, 0), (2, 24, 0), (2, 24, 12288), (1, 8, 256)])
-def test_layout_equals_lexsort(ds, cfg, n_events, hint):
+@pytest.mark.parametrize("cfg,n_events,hint,jitter", [(0, 10, 0, 0), (1, 64, 0, 0), (2, 24, 0, 0), (2, 24, 12288, 0), (1, 8, 256, 0),
+                                                      (1, 64, 0, 1), (2, 12, 0, 1)])
+def test_layout_equals_lexsort(ds, cfg, n_events, hint, jitter):
     d = gen.generate(cfg, n_events=n_events)
+    if jitter:                                  # per-hit z, w, ymin, ymax all different: a gather from the wrong hit shows
+        d = gen.with_hit_jitter(d)
     ds.set_params(dict(P, max_event_hits_hint=hint))
     try:
         hits = ds.to_device(d["hits"])
@@ -147,27 +150,77 @@ def test_extrapolate_equals_oracle(ds):
 
 
 # ---- S1..S10 on the five configs ------------------------------------------------------------------------------------
-def test_cfg0_noise_free(ds, orc_mlp):
+def test_cfg0_noise_free(ds, orc_mlp, parity_counts):
     d = gen.generate(0)
     st, sv, t, v = check_both(ds, d, orc_mlp)
+    parity_counts("cfg0", events=10, tracks=st, vertices=sv)
     assert st["found"] == 200 and (t["nhits"] == 4).all()
     sp = d["truth"]["seed_particle"]
     assert (d["truth"]["hit_particle"][t["hit"]] == sp[:, None]).all()     # P-1 on the GPU output itself
 
 
 @pytest.mark.parametrize("cfg,n_events", [(1, 1000), (2, 1000), (3, 2000)])
-def test_full_configs(ds, orc_mlp, cfg, n_events):
+def test_full_configs(ds, orc_mlp, parity_counts, cfg, n_events):
     d = gen.generate(cfg, n_events=n_events, workers=4)
     hint = 16384 if cfg == 2 else 0
     st, sv, t, v = check_both(ds, d, orc_mlp, params=dict(P, max_event_hits_hint=hint))
     assert st["found"] > 10 * n_events and sv["n"] > n_events
+    parity_counts(f"cfg{cfg}", events=n_events, tracks=st, vertices=sv)
     print(f"cfg{cfg}: tracks {st}, vertices {sv}")
+
+
+@pytest.mark.parametrize("cfg,n_events,hint,dv1,chi2ndf_max", [
+    (1, 300, 0, 0, 5.0), (1, 300, 0, 0, 300.0), (1, 60, 0, 1, 300.0), (3, 30, 0, 0, 300.0),
+    (2, 16, 0, 0, 300.0), (2, 16, 12288, 0, 300.0), (2, 8, 0, 1, 300.0), (2, 8, 12288, 1, 300.0)])
+def test_per_hit_z_weight_and_y_range(ds, orc_mlp, parity_counts, cfg, n_events, hint, dv1, chi2ndf_max):
+    """Hits whose z, weight and [ymin, ymax] differ from hit to hit (gen.with_hit_jitter): every per-hit gather of the kernels
+    (the staged ymin / ymax, z and w of the first hit, of the fitted hits and of the Dv1 candidates) is now discriminated --
+    fetching another hit's value of the same layer changes a window decision or the fit.  Dv0 and Dv1, staged events and
+    events above the staging capacity (cfg2 with the default hint), with the default chi2 cut (most displaced candidates
+    fail it) and a loose one (they pass and reach the track record)."""
+    d = gen.with_hit_jitter(gen.generate(cfg, n_events=n_events))
+    pp = dict(P, dv1=dv1, max_event_hits_hint=hint, chi2ndf_max=chi2ndf_max)
+    st, sv, t, v = check_both(ds, d, orc_mlp, params=pp)
+    assert st["found"] > n_events
+    f = t["found"] == 1
+    zs = d["hits"]["z"][np.maximum(t["hit"][f], 0)]
+    assert len(np.unique(zs)) > 100 and len(np.unique(d["hits"]["w"])) == 3
+    parity_counts(f"jitter_cfg{cfg}_hint{hint}_dv1{dv1}_chi2{chi2ndf_max:g}", events=n_events, tracks=st, vertices=sv)
 
 
 def test_cfg2_oversize_path(ds, orc_mlp):
     """cfg2 events (~8000 hits) with the default 4096-hit hint: the layout takes its global-memory path."""
     d = gen.generate(2, n_events=12)
     check_both(ds, d, orc_mlp)
+
+
+def test_cfg4_full(ds, orc_mlp, parity_counts):
+    """BASELINE configs[4] in full: all 100 000 events, sub-batch by sub-batch (10 x 10 000 events, the launch configuration
+    bench.py times, max_event_hits_hint = the sub-batch's largest event), every seed and every vertex against the oracle
+    (OpenMP over events on the host cores)."""
+    import os
+    n_sub = C.CONFIGS[4].n_events // C.SUBBATCH_EVENTS
+    bps = C.SUBBATCH_EVENTS // C.BLOCK_EVENTS
+    tot_t = dict(n=0, found=0, edge_list=0, excused=0)
+    tot_v = dict(n=0, n_pairs=0, edge_list=0, excused=0)
+    for i in range(n_sub):
+        d = gen.generate(4, n_events=C.SUBBATCH_EVENTS, first_block=i * bps, workers=min(10, os.cpu_count() or 1))
+        pp = dict(P, max_event_hits_hint=int(np.diff(d["hit_offsets"]).max()))
+        t, v = gpu_run(ds, d, capacity=1 << 20, params=pp)
+        r = oracle_run(d, orc_mlp)
+        st = parity.compare_tracks(t, r)
+        ov = O.vertex(t, d["seed_offsets"], G, P)
+        sv = parity.compare_vertices(v, ov)
+        assert v["overflow"][0] == 0 and (np.diff(v["offsets"]) == v["n_per_event"][: d["n_events"]]).all()
+        for k in tot_t:
+            tot_t[k] += st[k]
+        for k in tot_v:
+            tot_v[k] += sv[k]
+        del d, t, v, r, ov
+    assert tot_t["n"] > 14e6 and tot_t["found"] > 2e6 and tot_v["n"] > 9e5
+    assert tot_t["excused"] <= 1e-4 * tot_t["n"] and tot_v["excused"] <= 1e-4 * tot_v["n_pairs"]
+    parity_counts("cfg4", events=C.CONFIGS[4].n_events, tracks=tot_t, vertices=tot_v)
+    print(f"cfg4: tracks {tot_t}, vertices {tot_v}")
 
 
 def test_cfg4_subbatch_sampled(ds, orc_mlp):
