@@ -104,26 +104,29 @@ bool vertices_ok(const ds_vertices *v)
            (v->evt && v->ia && v->ib && v->x && v->y && v->z && v->doca && v->m_pipi && v->m_ppi && v->flags);
 }
 
-// carve the S1 arrays out of a workspace
-size_t layout_bytes(int n_bins, int n_events, int64_t n_hits)
+// carve the internal S1 output (see LayoutPtrs) out of a workspace; returns the bytes used (ws may be null: sizing)
+size_t carve_layout(void *ws, int n_bins, int n_events, int64_t n_hits, LayoutPtrs &L)
 {
-    const size_t nh = (size_t)(n_hits > 0 ? n_hits : 1) + 4;
-    return 7 * up256(4 * nh) + up256(4 * (size_t)(n_events > 0 ? n_events : 1) * (n_bins + 1));
-}
-
-void carve_layout(void *ws, int n_bins, int n_events, int64_t n_hits, LayoutPtrs &L)
-{
-    const size_t nh = (size_t)(n_hits > 0 ? n_hits : 1) + 4;
-    unsigned char *w = static_cast<unsigned char *>(ws);
-    auto take = [&](size_t bytes) { unsigned char *r = w; w += up256(bytes); return r; };
+    const size_t nh = (size_t)(n_hits > 0 ? n_hits : 1) + 4, ne = (size_t)(n_events > 0 ? n_events : 1);
+    unsigned char *base = static_cast<unsigned char *>(ws);
+    size_t off = 0;
+    auto take = [&](size_t bytes) { unsigned char *r = base + off; off += up256(bytes); return r; };
     L.sx0 = reinterpret_cast<float *>(take(4 * nh));
-    L.sz = reinterpret_cast<float *>(take(4 * nh));
     L.symin = reinterpret_cast<float *>(take(4 * nh));
     L.symax = reinterpret_cast<float *>(take(4 * nh));
-    L.sw = reinterpret_cast<float *>(take(4 * nh));
-    L.sid = reinterpret_cast<int32_t *>(take(4 * nh));
-    L.perm = reinterpret_cast<int32_t *>(take(4 * nh));
-    L.bin_offsets = reinterpret_cast<int32_t *>(take(4 * (size_t)(n_events > 0 ? n_events : 1) * (n_bins + 1)));
+    L.aux = reinterpret_cast<float4 *>(take(16 * nh));
+    L.bin_offsets = reinterpret_cast<int32_t *>(take(4 * ne * (n_bins + 1)));
+    L.ybounds = reinterpret_cast<float2 *>(take(sizeof(float2) * ne * (n_bins / kXBins)));
+    L.uniform = reinterpret_cast<int32_t *>(take(4 * ne));
+    L.sz = L.sw = nullptr;
+    L.sid = L.perm = nullptr;
+    return off;
+}
+
+size_t layout_bytes(int n_bins, int n_events, int64_t n_hits)
+{
+    LayoutPtrs L;
+    return carve_layout(nullptr, n_bins, n_events, n_hits, L);
 }
 
 void set_inputs(LayoutPtrs &L, const ds_hits *hits)
@@ -235,6 +238,7 @@ int ds_layout(ds_handle *h, const ds_hits *hits, const int32_t *hit_offsets, int
     set_inputs(L, hits);
     L.sx0 = out->x0; L.sz = out->z; L.symin = out->ymin; L.symax = out->ymax; L.sw = out->w; L.sid = out->id;
     L.perm = out->perm; L.bin_offsets = out->bin_offsets;
+    L.aux = nullptr; L.ybounds = nullptr; L.uniform = nullptr;   // the public SoA form
     if (launch_layout(c, L, hit_offsets, n_events, p->max_event_hits_hint, (cudaStream_t)cuda_stream, h->prof) != cudaSuccess) {
         cudaGetLastError();
         return DS_E_CUDA;

@@ -183,11 +183,17 @@ inline cudaError_t opt_in_max_smem(K kernel, unsigned long long *done)
 }
 
 // ---- launchers (host side, defined in the .cu files; all enqueue on `st` and return the launch error) ------------
+// Inputs and outputs of k_layout.  Public form (ds_layout): sx0, sz, symin, symax, sw, sid, perm.  Internal form (inside
+// ds_reconstruct, aux != nullptr): sx0, aux = (z, w, perm, id) per sorted position, ybounds / uniform per event, and
+// symin / symax only for events whose hits do not all carry their sector's bounds (see ds_layout.cu).
 struct LayoutPtrs {
     const float *x0, *z, *ymin, *ymax, *w;
     const int32_t *id;
     float *sx0, *sz, *symin, *symax, *sw;
     int32_t *sid, *perm, *bin_offsets;
+    float4 *aux;
+    float2 *ybounds;
+    int32_t *uniform;
 };
 
 cudaError_t launch_layout(const DevConst &c, const LayoutPtrs &p, const int32_t *hit_offsets, int n_events,

@@ -14,12 +14,22 @@
 //   E  per array: out[q] = staged[src[q]], coalesced stores
 // Events larger than the shared-memory capacity chosen from the caller's hint take an O(n^2) rank over global
 // memory (phase A/B identical), which yields the same permutation.
+//
+// Two output forms.  ds_layout (public, S1 alone) writes the sorted SoA of include/ds.h: seven arrays.  Inside ds_reconstruct
+// (kInternal) the consumer is k_track, and the layout is the one it reads best:
+//   sx0    [n]  sorted x0 (the only array a window search scans)
+//   aux    [n]  float4 (z, w, perm, id) of the hit at a sorted position: read only for hits that passed a window, and then
+//               one 16-byte load brings all four (one DRAM sector instead of four)
+//   ybounds [E][4 * n_sectors] (ymin, ymax) of each (layer, sector), and uniform[e] = 1 iff every hit of the event carries
+//               exactly the bounds of its (layer, sector).  That is how detectors are built (A-2: a strip's y range is its
+//               sector's), so y-compatibility becomes one test per (seed, sector) instead of one per hit and k_track stages
+//               4 instead of 12 bytes per hit.  symin / symax (sorted per-hit bounds) are written only for events that are
+//               not uniform; k_track then tests every hit with its own bounds.
 #include "ds_common.cuh"
 
 namespace ds {
 
 constexpr int kLayoutThreads = 512;
-constexpr int kMaxBins = 4 * DS_MAX_SECTORS * kXBins;
 constexpr int kSub = 4;   // the sort cuts every x0 slice of the bin table into kSub sub-slices (a power of two)
 
 // Sort bin of a hit: (layer, sector, x0 sub-slice).  t = (x0 + off) * scale is the same fp32 value xbin() floors, and
@@ -97,12 +107,15 @@ __device__ __forceinline__ void stage_field(T *buf, const T *__restrict__ src, i
     }
 }
 
+template <bool kInternal>
 __global__ void __launch_bounds__(2 * kLayoutThreads)
 k_layout(const __grid_constant__ DevConst c, const LayoutPtrs p, const int32_t *__restrict__ hit_offsets, int cap, bool bulk)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ int warp_sums[33];
     __shared__ __align__(8) unsigned long long bars[3];
+    __shared__ float2 s_ref[kLayers * DS_MAX_SECTORS];   // kInternal: (ymin, ymax) of the first hit of each (layer, sector)
+    __shared__ int s_nonuni;
     const int nb = c.n_bins, nfine = nb * kSub;
     // cap is a multiple of 4, so every array starts on a 16-byte boundary
     float *s_x0 = reinterpret_cast<float *>(smem_raw);                 // [cap] x0, later ymin
@@ -191,31 +204,84 @@ k_layout(const __grid_constant__ DevConst c, const LayoutPtrs p, const int32_t *
         __syncthreads();
         for (int i = tid; i < n; i += blockDim.x) s_src[s_pk[i]] = (uint16_t)i;
         __syncthreads();
-        // E: z is loaded while perm, x0 and id go out; ymin, ymax, w follow into the buffers that fall free
-        stage_field(reinterpret_cast<float *>(s_buf), p.z, h0, n, bar_b, bulk);
-        for (int q = tid; q < n; q += blockDim.x) {
-            const int i = s_src[q];
-            p.perm[h0 + q] = h0 + i;
-            p.sx0[h0 + q] = s_x0[d + i];
-            p.sid[h0 + q] = s_id[d + i];
+        if (!kInternal) {
+            // E: z is loaded while perm, x0 and id go out; ymin, ymax, w follow into the buffers that fall free
+            stage_field(reinterpret_cast<float *>(s_buf), p.z, h0, n, bar_b, bulk);
+            for (int q = tid; q < n; q += blockDim.x) {
+                const int i = s_src[q];
+                p.perm[h0 + q] = h0 + i;
+                p.sx0[h0 + q] = s_x0[d + i];
+                p.sid[h0 + q] = s_id[d + i];
+            }
+            __syncthreads();
+            stage_field(s_x0, p.ymin, h0, n, bar_x, bulk);
+            stage_field(reinterpret_cast<float *>(s_id), p.ymax, h0, n, bar_i, bulk);
+            mbar_wait(bar_b, 0);
+            for (int q = tid; q < n; q += blockDim.x) p.sz[h0 + q] = reinterpret_cast<float *>(s_buf)[d + s_src[q]];
+            __syncthreads();
+            stage_field(reinterpret_cast<float *>(s_buf), p.w, h0, n, bar_b, bulk);
+            mbar_wait(bar_x, 1);
+            mbar_wait(bar_i, 1);
+            for (int q = tid; q < n; q += blockDim.x) {
+                const int i = d + s_src[q];
+                p.symin[h0 + q] = s_x0[i];
+                p.symax[h0 + q] = reinterpret_cast<float *>(s_id)[i];
+            }
+            __syncthreads();
+            mbar_wait(bar_b, 1);
+            for (int q = tid; q < n; q += blockDim.x) p.sw[h0 + q] = reinterpret_cast<float *>(s_buf)[d + s_src[q]];
+        } else {
+            // E (internal form): z and w are loaded (into the key and rank buffers, both free now) while x0 goes out; ymin
+            // follows into the x0 buffer while the aux records (z, w, perm, id) go out; ymax into the key buffer
+            float *b_z = reinterpret_cast<float *>(s_buf), *b_w = reinterpret_cast<float *>(s_pk);
+            stage_field(b_z, p.z, h0, n, bar_b, bulk);
+            stage_field(b_w, p.w, h0, n, bar_x, bulk);            // bar_x: second use (phase 1)
+            const int ncoarse = kLayers * c.n_sectors;
+            if (tid < kLayers * DS_MAX_SECTORS) s_ref[tid] = make_float2(0.f, 0.f);
+            if (tid == 0) s_nonuni = 0;
+            for (int q = tid; q < n; q += blockDim.x) p.sx0[h0 + q] = s_x0[d + s_src[q]];
+            __syncthreads();
+            stage_field(s_x0, p.ymin, h0, n, bar_i, bulk);        // bar_i: second use (phase 1)
+            mbar_wait(bar_b, 0);
+            mbar_wait(bar_x, 1);
+            for (int q = tid; q < n; q += blockDim.x) {
+                const int i = s_src[q];
+                p.aux[h0 + q] = make_float4(b_z[d + i], b_w[d + i], __int_as_float(h0 + i), __int_as_float(s_id[d + i]));
+            }
+            __syncthreads();
+            float *b_ymin = s_x0, *b_ymax = reinterpret_cast<float *>(s_buf);
+            stage_field(b_ymax, p.ymax, h0, n, bar_b, bulk);      // bar_b: second use (phase 1)
+            mbar_wait(bar_i, 1);
+            mbar_wait(bar_b, 1);
+            __syncthreads();   // the tail elements of ymax were stored by ordinary stores of other threads
+            // reference bounds of a (layer, sector): those of its first hit in sorted order; then every hit against them
+            if (tid < ncoarse) {
+                const int qb = hist[tid * (kXBins * kSub)], qe = hist[(tid + 1) * (kXBins * kSub)];
+                if (qb < qe) {
+                    const int i = s_src[qb];
+                    s_ref[tid] = make_float2(b_ymin[d + i], b_ymax[d + i]);
+                }
+            }
+            __syncthreads();
+            bool differs = false;
+            for (int i = tid; i < n; i += blockDim.x) {
+                const int id = s_id[d + i];
+                const float2 r = s_ref[id_layer(id) * c.n_sectors + min(id_sector(id), c.n_sectors - 1)];
+                differs |= (b_ymin[d + i] != r.x) | (b_ymax[d + i] != r.y);
+            }
+            if (differs) s_nonuni = 1;
+            __syncthreads();
+            const bool nonuni = s_nonuni != 0;
+            if (tid < ncoarse) p.ybounds[(size_t)e * ncoarse + tid] = s_ref[tid];
+            if (tid == 0) p.uniform[e] = nonuni ? 0 : 1;
+            if (nonuni) {
+                for (int q = tid; q < n; q += blockDim.x) {
+                    const int i = d + s_src[q];
+                    p.symin[h0 + q] = b_ymin[i];
+                    p.symax[h0 + q] = b_ymax[i];
+                }
+            }
         }
-        __syncthreads();
-        stage_field(s_x0, p.ymin, h0, n, bar_x, bulk);
-        stage_field(reinterpret_cast<float *>(s_id), p.ymax, h0, n, bar_i, bulk);
-        mbar_wait(bar_b, 0);
-        for (int q = tid; q < n; q += blockDim.x) p.sz[h0 + q] = reinterpret_cast<float *>(s_buf)[d + s_src[q]];
-        __syncthreads();
-        stage_field(reinterpret_cast<float *>(s_buf), p.w, h0, n, bar_b, bulk);
-        mbar_wait(bar_x, 1);
-        mbar_wait(bar_i, 1);
-        for (int q = tid; q < n; q += blockDim.x) {
-            const int i = d + s_src[q];
-            p.symin[h0 + q] = s_x0[i];
-            p.symax[h0 + q] = reinterpret_cast<float *>(s_id)[i];
-        }
-        __syncthreads();
-        mbar_wait(bar_b, 1);
-        for (int q = tid; q < n; q += blockDim.x) p.sw[h0 + q] = reinterpret_cast<float *>(s_buf)[d + s_src[q]];
     } else {
         // oversize event: rank over the whole event straight from global memory, scattered writes
         const float *x0 = p.x0 + h0;
@@ -236,13 +302,21 @@ k_layout(const __grid_constant__ DevConst c, const LayoutPtrs p, const int32_t *
                 rank += less ? 1 : 0;
             }
             const size_t q = (size_t)h0 + hist[b] + rank;
-            p.perm[q] = h0 + i;
             p.sx0[q] = xi;
-            p.sz[q] = p.z[h0 + i];
             p.symin[q] = p.ymin[h0 + i];
             p.symax[q] = p.ymax[h0 + i];
-            p.sw[q] = p.w[h0 + i];
-            p.sid[q] = ii;
+            if (kInternal) {
+                p.aux[q] = make_float4(p.z[h0 + i], p.w[h0 + i], __int_as_float(h0 + i), __int_as_float(ii));
+            } else {
+                p.perm[q] = h0 + i;
+                p.sz[q] = p.z[h0 + i];
+                p.sw[q] = p.w[h0 + i];
+                p.sid[q] = ii;
+            }
+        }
+        if (kInternal) {   // an event that is not staged is never declared uniform: k_track tests its hits one by one
+            if (tid < kLayers * c.n_sectors) p.ybounds[(size_t)e * (kLayers * c.n_sectors) + tid] = make_float2(0.f, 0.f);
+            if (tid == 0) p.uniform[e] = 0;
         }
     }
 }
@@ -262,8 +336,9 @@ cudaError_t launch_layout(const DevConst &c, const LayoutPtrs &p, const int32_t 
     if (cap_max > 65532) cap_max = 65532;
     if (cap > cap_max) cap = cap_max;
     const size_t smem = layout_smem_bytes(cap, c.n_bins);
-    static unsigned long long opted = 0;
-    const cudaError_t aerr = opt_in_max_smem(k_layout, &opted);
+    const bool internal = p.aux != nullptr;
+    static unsigned long long opted[2] = {0, 0};
+    const cudaError_t aerr = internal ? opt_in_max_smem(k_layout<true>, &opted[1]) : opt_in_max_smem(k_layout<false>, &opted[0]);
     if (aerr != cudaSuccess) return aerr;
     // the bulk copies need 16-byte aligned sources (offsets inside the arrays are handled by the kernel)
     const uintptr_t bits = reinterpret_cast<uintptr_t>(p.x0) | reinterpret_cast<uintptr_t>(p.z) |
@@ -273,7 +348,8 @@ cudaError_t launch_layout(const DevConst &c, const LayoutPtrs &p, const int32_t 
     prof.begin(DS_K_LAYOUT, st);
     // events so large that one block fills an SM's shared memory get twice the threads (every loop strides by blockDim.x)
     const int threads = smem + 1024 > (228 * 1024) / 2 ? 2 * kLayoutThreads : kLayoutThreads;
-    k_layout<<<n_events, threads, smem, st>>>(c, p, hit_offsets, cap, bulk);
+    if (internal) k_layout<true><<<n_events, threads, smem, st>>>(c, p, hit_offsets, cap, bulk);
+    else k_layout<false><<<n_events, threads, smem, st>>>(c, p, hit_offsets, cap, bulk);
     prof.end(st);
     return cudaGetLastError();
 }
