@@ -132,18 +132,18 @@ def algorithmic_bytes(n_events, n_hits, n_seeds, n_found, n_keep, n_vtx):
 
 
 # ---- the oracle arm --------------------------------------------------------------------------------------------------------
-def oracle_events_per_s(d, n_events):
-    """Time oracle.reconstruct + oracle.vertex on the first n_events events of d (all host cores, OpenMP)."""
+def oracle_events_per_s(d, n_events, n_threads=0):
+    """Time oracle.reconstruct + oracle.vertex on the first n_events events of d (n_threads = 0: all host cores, OpenMP)."""
     import gen
     from gen import constants as C
     from oracle import ds_oracle as O
     sub = gen.take_events(d, n_events)
     mlp = O.Mlp(gen.mlp_weights(0))
     t0 = time.perf_counter()
-    r = O.reconstruct(sub["hits"], sub["hit_offsets"], sub["seeds"], sub["seed_offsets"], C.GEOMETRY, C.PARAMS, mlp)
-    v = O.vertex(r, sub["seed_offsets"], C.GEOMETRY, C.PARAMS)
+    r = O.reconstruct(sub["hits"], sub["hit_offsets"], sub["seeds"], sub["seed_offsets"], C.GEOMETRY, C.PARAMS, mlp, n_threads=n_threads)
+    v = O.vertex(r, sub["seed_offsets"], C.GEOMETRY, C.PARAMS, n_threads=n_threads)
     dt = time.perf_counter() - t0
-    return n_events / dt, dt, O.max_threads(), int(r["found"].sum()), v["n"]
+    return n_events / dt, dt, (n_threads or O.max_threads()), int(r["found"].sum()), v["n"]
 
 
 def sized_sample(d, target_s, cap):
@@ -206,6 +206,12 @@ def main():
                     help="Dv1 triplet search instead of the Dv0 first window (SURVEY 8f N2, P:107-P:111) in both arms")
     ap.add_argument("--clone-min-shared", type=int, default=0,
                     help="3: clone killing across seeds between S6 and S7 (SURVEY 8f N3, P:115); 0 = BASELINE configs")
+    ap.add_argument("--mlp", default="cfg", choices=["cfg", "paper"],
+                    help="paper: the ghost killer is the paper's 8 -> 14 -> 1 network (P:121, SURVEY 8f N5) in our arm")
+    ap.add_argument("--mlp-fast-math", action="store_true",
+                    help="ghost-killer sigmoid by __expf / __fdividef as in the paper (P:157); the line then carries `mlp_variant` "
+                         "with the score differences against the IEEE path")
+    ap.add_argument("--no-legs", action="store_true", help="skip the short cfg3 / cfg2 legs that follow the cfg4 timing")
     ap.add_argument("--magnet-polarity", type=float, default=0.0,
                     help="+1 / -1: curved-track vertexing (SURVEY 8f N1, P:255-P:269) in both arms; 0 = BASELINE configs")
     args = ap.parse_args()
@@ -256,6 +262,8 @@ def main():
     max_event_hits = max(int(np.diff(d["hit_offsets"]).max()) for d in subs)
     params = dict(C.PARAMS, max_event_hits_hint=max_event_hits)
     ds = pk.Downstream(C.GEOMETRY, mlp_w, params, device=local)
+    if args.mlp == "paper":
+        ds.upload_mlp_single(gen.mlp_single_weights(0))
     host, devd = [], []
     for d in subs:
         hp = dict(hits={k: torch.from_numpy(v).pin_memory() for k, v in d["hits"].items()},
@@ -379,26 +387,114 @@ def main():
                 "share_of_step": kernels[dom]["ms_per_step"] / ksum,
                 "timing": "CUDA events around every launch, one-stream pass of the same K steps right after the timed region"}
     whole_gbs = sum(alg.values()) * args.steps / (ms_total * 1e-3) / 1e9
+    # the kernel BASELINE north_star sets the 40 % bar on: search + fit (S2..S6)
+    roofline_search_fit = None
+    if "k_track" in kernels:
+        kt = kernels["k_track"]
+        roofline_search_fit = {"bound": "hbm", "kernel": "k_track", "achieved": kt["achieved_gbs"], "peak": peak, "unit": "GB/s",
+                               "frac": kt["frac"], "traffic": kt["traffic"], "share_of_step": kt["ms_per_step"] / ksum}
 
     # ---- cfg3: the vertex kernels are bound by plain fp64 arithmetic, not by HBM -----------------------------------
-    vertex_alu = None
-    if args.cfg == 3:
+    def vertex_alu_of(kern, trk_list, dev_list, n_pass):
+        """fp64 ALU fraction of the vertex kernels: ~130 flop per pair.  The count kernel evaluates every
+        opposite-charge pair, the write kernel only the passing ones again."""
         n_pairs = 0
-        for i, d in enumerate(devd):
+        for t, d in zip(trk_list, dev_list):
             so = d["seed_offsets"].cpu().numpy()
-            keep, q = trk[i]["keep"].cpu().numpy(), trk[i]["qop"].cpu().numpy()
+            keep, q = t["keep"].cpu().numpy(), t["qop"].cpu().numpy()
             pos = np.concatenate([[0], np.cumsum((keep == 1) & (q > 0))])
             neg = np.concatenate([[0], np.cumsum((keep == 1) & (q < 0))])
             n_pairs += int(((pos[so[1:]] - pos[so[:-1]]) * (neg[so[1:]] - neg[so[:-1]])).sum())
-        ms = sum(kernels[k]["ms_per_step"] for k in ("k_vertex_count", "k_vertex_write") if k in kernels)
-        flop = 130.0 * n_pairs * 2                      # ~130 flop per pair, evaluated in both kernels
-        peak_nominal = 148 * 64 * 2 * (clocks.get("sm_mhz") or 1965.0) * 1e6 / 1e12
         peak_tf = pk.ds_measure_dfma_peak(ds.h)
-        vertex_alu = {"bound": "alu", "pairs_per_step": n_pairs, "flop_per_pair": 130, "ms_per_step": ms,
-                      "achieved": flop / (ms * 1e-3) / 1e12, "peak": peak_tf, "unit": "TFLOP/s (fp64)",
-                      "frac": flop / (ms * 1e-3) / 1e12 / peak_tf,
-                      "peak_source": "measured: ds_measure_dfma_peak (register-resident DFMA loop on every SM)",
-                      "peak_nominal": peak_nominal}
+        out = {"bound": "alu", "pairs_per_step": n_pairs, "passing_pairs_per_step": n_pass, "flop_per_pair": 130,
+               "unit": "TFLOP/s (fp64)", "peak": peak_tf,
+               "peak_source": "measured: ds_measure_dfma_peak (register-resident DFMA loop on every SM)",
+               "peak_nominal": 148 * 64 * 2 * (clocks.get("sm_mhz") or 1965.0) * 1e6 / 1e12}
+        if "k_vertex_count" in kern:
+            ms_c = kern["k_vertex_count"]["ms_per_step"]
+            out["count_kernel"] = {"ms_per_step": ms_c, "achieved": 130.0 * n_pairs / (ms_c * 1e-3) / 1e12}
+            out["count_kernel"]["frac"] = out["count_kernel"]["achieved"] / peak_tf
+        ms = sum(kern[k]["ms_per_step"] for k in ("k_vertex_count", "k_vertex_write") if k in kern)
+        flop = 130.0 * (n_pairs + n_pass)
+        out.update(ms_per_step=ms, achieved=flop / (ms * 1e-3) / 1e12, frac=flop / (ms * 1e-3) / 1e12 / peak_tf)
+        return out
+
+    vertex_alu = vertex_alu_of(kernels, trk, devd, n_vtx) if args.cfg == 3 else None
+
+    # ---- short legs on the other configurations, one stream, per-kernel events (not the metric: evidence for the kernels
+    #      whose regime cfg4 does not show -- the vertexing stress cfg3 and the high-occupancy cfg2) ---------------------------
+    legs = {}
+    if args.cfg == 4 and not args.no_legs and rank == 0:
+        for cfg_k, n_ev in ((3, 2000), (2, 1000)):
+            dl = gen.generate(cfg_k, n_events=n_ev, workers=workers)
+            dl.pop("truth", None)
+            mh = int(np.diff(dl["hit_offsets"]).max())
+            ds.set_params(dict(params, max_event_hits_hint=mh))
+            dd = dict(hits=ds.to_device(dl["hits"]), seeds=ds.to_device(dl["seeds"]),
+                      hit_offsets=ds.to_device(dict(h=dl["hit_offsets"]))["h"], seed_offsets=ds.to_device(dict(s=dl["seed_offsets"]))["s"])
+            nh_l, ns_l = int(dl["hit_offsets"][-1]), int(dl["seed_offsets"][-1])
+            t_l, v_l = ds.empty_tracks(ns_l), ds.empty_vertices(1 << 22, n_ev)
+            w_l, vw_l = ds.workspace(n_ev, nh_l, ns_l), ds.vertex_workspace(n_ev, ns_l)
+
+            def leg_step():
+                ds.reconstruct(dd["hits"], dd["seeds"], dd["hit_offsets"], dd["seed_offsets"], out=t_l, workspace=w_l, stream=streams[0])
+                ds.vertex(t_l, dd["seed_offsets"], out=v_l, workspace=vw_l, stream=streams[0])
+            for _ in range(3):
+                leg_step()
+            torch.cuda.synchronize()
+            pk.ds_profile_enable(ds.h, True)
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(streams[0])
+            for _ in range(args.steps):
+                leg_step()
+            b.record(streams[0])
+            torch.cuda.synchronize()
+            pl = pk.ds_profile_read(ds.h)
+            pk.ds_profile_enable(ds.h, False)
+            assert int(v_l["overflow"].item()) == 0
+            nf_l, nk_l, nv_l = int(t_l["found"].sum().item()), int(t_l["keep"].sum().item()), int(v_l["offsets"][-1].item())
+            alg_l = algorithmic_bytes(n_ev, nh_l, ns_l, nf_l, nk_l, nv_l)
+            kl = {}
+            for name, (ms, n) in pl.items():
+                if n:
+                    gbs = alg_l[name] * args.steps / n / (ms / n * 1e-3) / 1e9
+                    kl[name] = {"ms_per_launch": ms / n, "ms_per_step": ms / args.steps, "alg_bytes_per_launch": alg_l[name] * args.steps / n,
+                                "achieved_gbs": gbs, "frac": gbs / peak}
+            ms_l = a.elapsed_time(b) / args.steps
+            legs[f"cfg{cfg_k}"] = {"workload": f"BASELINE configs[{cfg_k}], {n_ev} events, one stream", "events": n_ev, "hits": nh_l, "seeds": ns_l,
+                                   "tracks_found": nf_l, "tracks_kept": nk_l, "vertices": nv_l, "ms_per_step": ms_l,
+                                   "events_per_s": n_ev / (ms_l * 1e-3), "kernels": kl}
+            if cfg_k == 3:
+                legs["cfg3"]["vertex_alu"] = vertex_alu_of(kl, [t_l], [dd], nv_l)
+            del dd, t_l, v_l, w_l, vw_l, dl
+        ds.set_params(params)
+
+    # ---- ghost-killer variants (SURVEY 8f N5): the other arithmetic flavour on the same tracks, k_mlp alone -------------------
+    mlp_variant = None
+    if args.mlp_fast_math and rank == 0:
+        ref_scores = [t["score"].clone() for t in trk]
+        ref_keep = [t["keep"].clone() for t in trk]
+        res = {}
+        for fast in (0, 1):
+            ds.set_params(dict(params, mlp_fast_math=fast))
+            pk.ds_profile_enable(ds.h, True)
+            for _ in range(args.steps):
+                for i, d in enumerate(devd):
+                    ds.ghost_killer(d["seeds"], trk[i], stream=streams[0])
+            torch.cuda.synchronize()
+            ms, n = pk.ds_profile_read(ds.h)["k_mlp"]
+            pk.ds_profile_enable(ds.h, False)
+            res[fast] = ms / n
+        dmax = max(float((t["score"] - r).abs().max().item()) for t, r in zip(trk, ref_scores))
+        flips = sum(int((t["keep"] != r).sum().item()) for t, r in zip(trk, ref_keep))
+        mlp_variant = {"network": "8-14-1 (P:121)" if args.mlp == "paper" else "8-32-16-1 (BASELINE cfg0)",
+                       "k_mlp_ms_per_launch_ieee": res[0], "k_mlp_ms_per_launch_fast_math": res[1],
+                       "max_abs_score_difference": dmax, "keep_decisions_flipped": flips, "tracks": n_found,
+                       "intrinsics": "__expf, __fdividef (P:157); no fp64 re-evaluation next to the threshold"}
+        ds.set_params(params)
+        for i, d in enumerate(devd):
+            ds.ghost_killer(d["seeds"], trk[i], stream=streams[0])
+        torch.cuda.synchronize()
 
     # ---- end to end: pinned host buffers in, pinned host buffers out, through ds_process_host ----------------------------
     e2e = None
@@ -444,13 +540,26 @@ def main():
         for h in handles:
             h.close()
 
-    # ---- the oracle beside it (rank 0, N = 1) ------------------------------------------------------------------------------
+    # ---- the oracle beside it (rank 0, N = 1): all host cores and one thread, on the first cfg4 sub-batch and on cfg1
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        n = sized_sample(first_sub, 15.0, args.subbatch)
-        v, dt, cores, _, _ = oracle_events_per_s(first_sub, n)
+        from oracle import ds_oracle as O
+        ncores = O.max_threads()
+        n = sized_sample(first_sub, 12.0, args.subbatch)
+        v, dt, cores, _, _ = oracle_events_per_s(first_sub, n, ncores)
         cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "seconds": dt,
-               "sample": f"first {n} events of cfg4 sub-batch 0 (oracle/ds_oracle.c, fp64, OpenMP over events)"}
+               "sample": f"first {n} events of cfg{CFG} sub-batch 0 (oracle/ds_oracle.c, fp64, OpenMP over events)"}
+        legs_cpu = {}
+        n1 = int(max(50, min(n, v / max(1, ncores) * 5.0)))
+        v1, dt1, _, _, _ = oracle_events_per_s(first_sub, n1, 1)
+        legs_cpu[f"cfg{CFG}_1_thread"] = {"value": v1, "cores": 1, "seconds": dt1, "sample": f"first {n1} events of cfg{CFG} sub-batch 0"}
+        d1 = gen.generate(1, n_events=1000, workers=workers)
+        va, dta, _, _, _ = oracle_events_per_s(d1, 1000, ncores)
+        legs_cpu["cfg1_all_cores"] = {"value": va, "cores": ncores, "seconds": dta, "sample": "BASELINE configs[1], 1000 events"}
+        n11 = int(max(50, min(1000, va / max(1, ncores) * 4.0)))
+        vb, dtb, _, _, _ = oracle_events_per_s(d1, n11, 1)
+        legs_cpu["cfg1_1_thread"] = {"value": vb, "cores": 1, "seconds": dtb, "sample": f"first {n11} events of BASELINE configs[1]"}
+        cpu["legs"] = legs_cpu
 
     if rank == 0:
         print(json.dumps({
@@ -463,9 +572,10 @@ def main():
                        "subbatches": n_sub, "events_per_subbatch": args.subbatch, "cuda_streams": n_streams,
                        "hits": sum(n_hits), "seeds": sum(n_seeds), "tracks_found": n_found, "tracks_kept": n_keep, "vertices": n_vtx,
                        "l2": "inputs larger than L2 (each sub-batch reads ~0.76 GB; 7.6 GB per step)",
-                       "magnet_polarity": args.magnet_polarity, "clone_min_shared": args.clone_min_shared, "dv1": bool(args.dv1), "lines": bool(args.lines),
+                       "magnet_polarity": args.magnet_polarity, "clone_min_shared": args.clone_min_shared, "dv1": bool(args.dv1), "lines": bool(args.lines), "mlp": args.mlp,
                        "parallelism": f"dp{world} (events sharded, no data-path collective)"},
-            "roofline": roofline, "whole_path_gbs": whole_gbs, "whole_path_frac": whole_gbs / peak, "kernels": kernels,
+            "roofline": roofline, "roofline_search_fit": roofline_search_fit, "legs": legs, "mlp_variant": mlp_variant,
+            "whole_path_gbs": whole_gbs, "whole_path_frac": whole_gbs / peak, "kernels": kernels,
             "vertex_alu": vertex_alu, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
         }), flush=True)
     ds.close()

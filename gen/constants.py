@@ -43,6 +43,8 @@ PARAMS = dict(
     # Dv1 triplet search (P:107-P:111): 1 = every UTbX hit of the y-compatible sectors starts a candidate
     # and the UTaX hit is mandatory; 0 = Dv0 (first window, <= 10 closest), the BASELINE configurations
     dv1=0,
+    # ghost-killer sigmoid by the paper's fast intrinsics; 0 = IEEE, the parity-tested path
+    mlp_fast_math=0,
 )
 
 # A-10: fixed input normalisation (mu, sigma) for [x, y, tx, ty, qop, chi2, qop_seed, chi2_seed]

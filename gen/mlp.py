@@ -60,3 +60,13 @@ def embed_single_hidden(w1: dict, sizes=C.MLP_SIZES) -> dict:
     out["W2"][np.arange(n_h), np.arange(n_h)] = 1.0
     out["W3"][:n_h] = np.asarray(w1["W3"]).reshape(-1)
     return out
+
+
+def mlp_single_weights(seed: int = 0, n_h: int = 14) -> dict:
+    """Random weights of the paper's single-hidden-layer ghost killer 8 -> 14 -> 1, drawn like mlp_weights (A-18):
+    N(0, 1/fan_in), order W1, b1, W3, b3, fp64 -> fp32; the input normalisation of A-10."""
+    rng = np.random.default_rng(seed + 1000)
+    n_in = C.MLP_SIZES[0]
+    return dict(W1=rng.normal(0.0, n_in ** -0.5, (n_h, n_in)).astype(np.float32), b1=rng.normal(0.0, n_in ** -0.5, n_h).astype(np.float32),
+                W3=rng.normal(0.0, n_h ** -0.5, n_h).astype(np.float32), b3=rng.normal(0.0, n_h ** -0.5, 1).astype(np.float32),
+                mu=np.asarray(C.MLP_MU, dtype=np.float32), inv_sigma=(1.0 / np.asarray(C.MLP_SIGMA, dtype=np.float64)).astype(np.float32))

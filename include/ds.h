@@ -41,6 +41,7 @@ enum {
 #define DS_MLP_IN 8
 #define DS_MLP_H1 32
 #define DS_MLP_H2 16
+#define DS_MLP_SINGLE_H 14 /* the paper's own ghost killer: one hidden layer of 14 neurons */
 
 /* HLT1 line NNs on the vertices (P:277-P:285): four networks DS_LINE_IN -> DS_LINE_H -> 1 (inputs: reading A-33). */
 #define DS_LINE_IN 16
@@ -77,6 +78,14 @@ typedef struct {
     float W3[DS_MLP_H2], b3;
     float mu[DS_MLP_IN], inv_sigma[DS_MLP_IN]; /* input k is fed as (v_k - mu_k) * inv_sigma_k */
 } ds_mlp;
+
+/* The paper's ghost killer 8 -> 14 -> 1, row-major [out][in]: W3 acts on the hidden layer. */
+typedef struct {
+    size_t struct_size;
+    float W1[DS_MLP_SINGLE_H][DS_MLP_IN], b1[DS_MLP_SINGLE_H];
+    float W3[DS_MLP_SINGLE_H], b3;
+    float mu[DS_MLP_IN], inv_sigma[DS_MLP_IN];
+} ds_mlp_single;
 
 /* Weights of the four line NNs (HOST, POD), row-major [net][out][in]; input k of every network is fed as
  * (v_k - mu_k) * inv_sigma_k.  Network order in the paper: K_S selection, Lambda selection, detached-vs-prompt
@@ -121,7 +130,10 @@ typedef struct {
                                          the seed's y-compatible sectors starts a candidate, which needs a UTaX hit within
                                          the refined window of the line through that hit and the magnet point; stereo
                                          hits, fit and choice as Dv0.  0: Dv0 (the BASELINE configurations)               */
-    int32_t pad_;
+    int32_t mlp_fast_math;            /* 1: sigmoid by the fast intrinsics __expf / __fdividef as in the paper and no
+                                         fp64 re-evaluation next to the threshold; scores then differ from an IEEE
+                                         evaluation by a few 1e-7 absolute and a keep decision on the threshold may flip.
+                                         0 (default): IEEE, the parity-tested path                                     */
 } ds_params;
 #define DS_MAX_FIRST_HITS 10
 
@@ -189,6 +201,11 @@ int ds_version(void);
 /* Copy geometry and ghost-killer weights (both HOST) into the handle; may be called again to replace them.
  * Synchronous.  DS_E_ARG on a wrong struct_size, n_sectors_y outside 1..DS_MAX_SECTORS or a non-positive height. */
 int ds_upload_geometry(ds_handle *h, const ds_geometry *g, const ds_mlp *m);
+
+/* Replace the handle's ghost killer by the paper's single-hidden-layer network (HOST weights; synchronous).  It stays in
+ * use by ds_reconstruct / ds_ghost_killer / ds_process_host until ds_upload_geometry is called again (which installs its
+ * 8 -> 32 -> 16 -> 1 network).  DS_E_ARG on a wrong struct_size. */
+int ds_upload_mlp_single(ds_handle *h, const ds_mlp_single *m);
 
 /* ---- S1: layout (P:109-P:111 "UT hits are grouped into different Y sectors"; BASELINE north_star (1)) -------- */
 

@@ -11,6 +11,8 @@ struct ds_handle {
     bool has_geom;
     ds_geometry geom;
     DevMlp *d_mlp;
+    DevMlpSingle *d_single;   // nullptr until ds_upload_mlp_single
+    bool use_single;          // the ghost killer in use is d_single (until the next ds_upload_geometry)
     DevLines *d_lines;   // nullptr until ds_upload_line_nets
     int n_sm;
     // arena of the *_host path, grown on demand
@@ -74,7 +76,7 @@ bool make_const(const ds_geometry &g, const ds_params *p, DevConst &c)
     c.dm_ks = p->dm_ks; c.dm_lambda = p->dm_lambda; c.n2_min = p->n2_min;
     c.vtx_mp = p->magnet_polarity; c.gamma_c0 = p->gamma_c0; c.gamma_c1 = p->gamma_c1;
     c.vtx_iters = p->vtx_newton_iters; c.clone_min_shared = p->clone_min_shared;
-    c.dv1 = p->dv1 != 0; c.pad3_ = 0;
+    c.dv1 = p->dv1 != 0; c.mlp_fast_math = p->mlp_fast_math != 0;
     return true;
 }
 
@@ -170,6 +172,8 @@ int ds_create(ds_handle **h, int cuda_device)
     p->arena = nullptr;
     p->arena_bytes = 0;
     p->d_lines = nullptr;
+    p->d_single = nullptr;
+    p->use_single = false;
     p->n_sm = 0;
     cudaDeviceGetAttribute(&p->n_sm, cudaDevAttrMultiProcessorCount, cuda_device);
     if (cudaMalloc(&p->d_mlp, sizeof(DevMlp)) != cudaSuccess) {
@@ -187,6 +191,7 @@ void ds_destroy(ds_handle *h)
     DeviceGuard guard(h->device);
     if (h->d_mlp) cudaFree(h->d_mlp);
     if (h->d_lines) cudaFree(h->d_lines);
+    if (h->d_single) cudaFree(h->d_single);
     if (h->arena) cudaFree(h->arena);
     h->prof.destroy();
     delete h;
@@ -220,6 +225,26 @@ int ds_upload_geometry(ds_handle *h, const ds_geometry *g, const ds_mlp *m)
     }
     h->geom = *g;
     h->has_geom = true;
+    h->use_single = false;
+    return DS_OK;
+}
+
+int ds_upload_mlp_single(ds_handle *h, const ds_mlp_single *m)
+{
+    if (!h || !m || m->struct_size != sizeof(ds_mlp_single)) return DS_E_ARG;
+    DeviceGuard guard(h->device);
+    if (!guard.ok) return DS_E_CUDA;
+    static_assert(sizeof(DevMlpSingle) <= sizeof(ds_mlp_single) - offsetof(ds_mlp_single, W1) && offsetof(DevMlpSingle, inv_sigma) == offsetof(ds_mlp_single, inv_sigma) - offsetof(ds_mlp_single, W1), "same layout after struct_size");
+    if (!h->d_single && cudaMalloc(&h->d_single, sizeof(DevMlpSingle)) != cudaSuccess) {
+        cudaGetLastError();
+        h->d_single = nullptr;
+        return DS_E_CUDA;
+    }
+    if (cudaMemcpy(h->d_single, &m->W1, sizeof(DevMlpSingle), cudaMemcpyHostToDevice) != cudaSuccess) {
+        cudaGetLastError();
+        return DS_E_CUDA;
+    }
+    h->use_single = true;
     return DS_OK;
 }
 
@@ -276,7 +301,7 @@ int ds_ghost_killer(ds_handle *h, const ds_seeds *seeds, const ds_params *p, ds_
     if (!make_const(h->geom, p, c)) return DS_E_ARG;
     DeviceGuard guard(h->device);
     if (!guard.ok) return DS_E_CUDA;
-    if (launch_mlp(c, h->d_mlp, *seeds, *trk, (cudaStream_t)cuda_stream, h->prof) != cudaSuccess) {
+    if (launch_mlp(c, h->d_mlp, h->use_single ? h->d_single : nullptr, *seeds, *trk, (cudaStream_t)cuda_stream, h->prof) != cudaSuccess) {
         cudaGetLastError();
         return DS_E_CUDA;
     }
@@ -320,7 +345,7 @@ int ds_reconstruct(ds_handle *h, const ds_hits *hits, const ds_seeds *seeds, con
     cudaError_t err = launch_layout(c, L, hit_offsets, n_events, p->max_event_hits_hint, st, h->prof);
     if (err == cudaSuccess) err = launch_track(c, L, *seeds, hit_offsets, seed_offsets, n_events, p->max_event_hits_hint, *out, st, h->prof);
     if (err == cudaSuccess) err = launch_clone(c, seed_offsets, n_events, *out, st, h->prof);
-    if (err == cudaSuccess) err = launch_mlp(c, h->d_mlp, *seeds, *out, st, h->prof);
+    if (err == cudaSuccess) err = launch_mlp(c, h->d_mlp, h->use_single ? h->d_single : nullptr, *seeds, *out, st, h->prof);
     if (err != cudaSuccess) {
         cudaGetLastError();
         return DS_E_CUDA;
@@ -472,7 +497,7 @@ int ds_process_host(ds_handle *h, const ds_hits *hits, const ds_seeds *seeds, co
     err = launch_layout(c, L, d_hoff, n_events, p->max_event_hits_hint, st, h->prof);
     if (err == cudaSuccess) err = launch_track(c, L, dsd, d_hoff, d_soff, n_events, p->max_event_hits_hint, dt, st, h->prof);
     if (err == cudaSuccess) err = launch_clone(c, d_soff, n_events, dt, st, h->prof);
-    if (err == cudaSuccess) err = launch_mlp(c, h->d_mlp, dsd, dt, st, h->prof);
+    if (err == cudaSuccess) err = launch_mlp(c, h->d_mlp, h->use_single ? h->d_single : nullptr, dsd, dt, st, h->prof);
     if (err == cudaSuccess) err = launch_vertex(c, dt, d_soff, n_events, dv, wvtx, st, h->prof);
     auto d2h = [&](void *dst, const void *src, size_t bytes) {
         if (bytes && err == cudaSuccess) err = cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToHost, st);

@@ -34,7 +34,7 @@ struct DevConst {
     double doca_max, zv_min, zv_max, m_pi, m_p, m_ks, m_lambda, dm_ks, dm_lambda, n2_min;
     double vtx_mp, gamma_c0, gamma_c1;   // curved-track vertexing: gamma = -vtx_mp * (gamma_c0 + gamma_c1 * qop / 1000)
     int vtx_iters, clone_min_shared;
-    int dv1, pad3_;
+    int dv1, mlp_fast_math;
 };
 
 // Device copy of the ghost-killer weights (global memory, staged to shared memory by the kernel).
@@ -46,6 +46,13 @@ struct DevMlp {
     float pad_[3];
 };
 static_assert(sizeof(DevMlp) % 16 == 0, "DevMlp is copied as float4");
+
+// Device copy of the paper's 8 -> 14 -> 1 ghost killer (ds_upload_mlp_single)
+struct DevMlpSingle {
+    float W1[DS_MLP_SINGLE_H * DS_MLP_IN], b1[DS_MLP_SINGLE_H];
+    float W3[DS_MLP_SINGLE_H], b3;
+    float mu[DS_MLP_IN], inv_sigma[DS_MLP_IN];
+};
 
 // Device copy of the four HLT1 line NNs (global memory, staged to shared memory by k_lines)
 struct DevLines {
@@ -208,8 +215,9 @@ cudaError_t launch_track(const DevConst &c, const LayoutPtrs &lay, const ds_seed
 cudaError_t launch_clone(const DevConst &c, const int32_t *seed_offsets, int n_events, const ds_tracks &trk, cudaStream_t st,
                          Prof &prof);
 
-cudaError_t launch_mlp(const DevConst &c, const DevMlp *mlp, const ds_seeds &seeds, const ds_tracks &trk,
-                       cudaStream_t st, Prof &prof);
+// single != nullptr: the paper's 8 -> 14 -> 1 network instead of mlp
+cudaError_t launch_mlp(const DevConst &c, const DevMlp *mlp, const DevMlpSingle *single, const ds_seeds &seeds,
+                       const ds_tracks &trk, cudaStream_t st, Prof &prof);
 
 cudaError_t launch_lines(const DevLines *nets, const ds_tracks &trk, const ds_vertices &vtx, int n_events, double thr,
                          float *scores, int32_t *bits, int n_sm, cudaStream_t st, Prof &prof);

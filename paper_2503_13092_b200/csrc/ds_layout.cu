@@ -332,7 +332,7 @@ cudaError_t launch_layout(const DevConst &c, const LayoutPtrs &p, const int32_t 
     // event are kept as uint16_t
     const int hint = max_event_hits_hint > 0 ? max_event_hits_hint : 4096;
     int cap = ((hint + 3) & ~3) + 8;
-    int cap_max = (int)((227 * 1024 - sizeof(int) * ((size_t)c.n_bins * kSub + 1) - 512) / 18) & ~3;   // 227 KB per CTA
+    int cap_max = (int)((227 * 1024 - sizeof(int) * ((size_t)c.n_bins * kSub + 1) - 1024) / 18) & ~3;   // 227 KB per CTA, static part included
     if (cap_max > 65532) cap_max = 65532;
     if (cap > cap_max) cap = cap_max;
     const size_t smem = layout_smem_bytes(cap, c.n_bins);

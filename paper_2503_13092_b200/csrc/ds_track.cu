@@ -3,24 +3,40 @@
 // per first hit a new trajectory through (hit, magnet point) and refined windows in UTaX/UTaU/UTbV keeping the
 // closest 1/2/2 hits; one final candidate per SciFi seed by score.  Readings A-1..A-9 in DESIGN.md.
 //
-// Mapping: one thread block per event.  The event's slice of the sorted x0 / ymin / ymax arrays (everything a window
-// search reads) is staged in shared memory by three 1-D bulk async copies (cp.async.bulk + mbarrier), issued by one
-// thread while the block loads the bin table.  The work is then flattened over the block in rounds of three phases:
+// Mapping: one thread block per event.  The event's slice of the sorted x0 array (what a window search scans) is staged in
+// shared memory by a 1-D bulk async copy (cp.async.bulk + mbarrier), issued by one thread while the block loads the bin
+// table and the event's per-sector y bounds.  y-compatibility: k_layout has checked whether every hit of the event carries
+// exactly the y range of its (layer, sector) (the normal case, A-2); then a seed tests each sector once (a bit mask per
+// layer, computed in phase A) and no per-hit bounds are read at all; otherwise every hit in a window is tested with its own
+// bounds from the sorted global arrays.  The work is then flattened over the block in rounds of three phases:
 //   A  thread per seed:      S2, first window in UTbX (S3) -> the seed's <= max_first first hits appended to a block-wide
 //                            list (block scan of the counts; only if more hits pass than are tried, a selection by
 //                            (distance, id))
 //   B  thread per first hit: the three refined windows (S4), the <= 4 fits (S5) -> best score of this first hit
 //   C  thread per seed:      best first hit (S6; exact score ties resolved by (more hits, ids)), the winner's fit is
 //                            evaluated once more and the track record written, coalesced over the seeds
-// z, w, id and perm are read from global memory only for hits that passed a window.  Events larger than the staging
-// buffer run the same code on the global arrays.
+// z, w, id and perm are read from global memory only for hits that passed a window: one 16-byte aux record per hit (see
+// ds_layout.cu).  Events larger than the staging buffer run the same code on the global arrays.
 // All of this arithmetic is fp64 in registers on fp32 inputs (the deciding comparisons must agree with an fp64
 // reference to ~1e-5 relative; fp32 would not: one ulp of x at 800 mm is 6e-5 mm).
+#include <cstdlib>
+
 #include "ds_common.cuh"
 
 namespace ds {
 
 constexpr int kMaxBins = 4 * DS_MAX_SECTORS * kXBins;
+
+// Development aid: DS_TRACK_BLOCKS=3|4 forces the blocks-per-SM configuration of k_track (0 / unset: automatic).
+static int track_blocks_override()
+{
+    static int v = -1;
+    if (v < 0) {
+        const char *e = getenv("DS_TRACK_BLOCKS");
+        v = e ? atoi(e) : 0;
+    }
+    return v;
+}
 
 struct S2 {
     double zm, xm, ym, y0, y1, y2, y3, txp, xc3, w0, w1;
@@ -74,6 +90,27 @@ __device__ __forceinline__ void sector_range(const DevConst &c, double y, int &s
     s_hi = (int)hi;
 }
 
+// Bit s set: sector s of `layer` is y-compatible with a track at height y.  kUni (every hit of the event carries the bounds
+// yb[layer * n_sectors + s] of its sector): the test of O-S3 itself, ymin - y_tol <= y <= ymax + y_tol, once per sector.
+// Otherwise the superset of sector_range; every hit is then tested with its own bounds.
+template <bool kUni>
+__device__ __forceinline__ unsigned sector_mask(const DevConst &c, const float2 *yb, int layer, double y)
+{
+    int lo, hi;
+    sector_range(c, y, lo, hi);
+    unsigned m = 0;
+    for (int s = lo; s <= hi; ++s) {
+        if (kUni) {
+            const float2 b = yb[layer * c.n_sectors + s];
+            const double ylo = (double)b.x - c.y_tol, yhi = (double)b.y + c.y_tol;
+            m |= ((ylo <= y) & (y <= yhi)) ? 1u << s : 0u;
+        } else {
+            m |= 1u << s;
+        }
+    }
+    return m;
+}
+
 // Positions [a, b) (relative to the event) of the x0 slices of (layer, sector) that the x0 interval [lo, hi] touches.
 template <typename Tab>
 __device__ __forceinline__ void slice_range(const DevConst &c, const Tab *tab, int layer, int sector, double lo,
@@ -100,15 +137,26 @@ struct FitRes {
 // type hit positions inside the event are stored in: uint16_t when the event is staged (it then has < 65535 hits),
 // int otherwise.  (Idx)-1 = none.
 // What the later phases need of a seed (S2, computed once in phase A): magnet point, y at the four planes, refined
-// window half-width, and the y-sector range of the refined window in UTaX, UTaU, UTbV (lo > hi: none).
+// window half-width, and the mask of y-compatible sectors of each layer (sector_mask).
 struct SeedRec {
     double xm, zm, w1, y[4];
-    unsigned char sec[3][2];
-    unsigned char pad_[2];
+    unsigned short mask[4];
+};
+static_assert(sizeof(SeedRec) == 64 && DS_MAX_SECTORS <= 16, "sector masks are 16 bits");
+
+// Dv1 only: the (seed, UTbX hit) items
+template <typename Idx, bool kDv1>
+struct DvShared {};
+template <typename Idx>
+struct DvShared<Idx, true> {
+    int dv_off[32], dv_a[32];             // first item and first UTbX candidate of the seed
+    float cand_z[kFirstCap];              // items that passed the fp32 pre-test: z of the UTbX hit,
+    Idx cand_j3[kFirstCap];               //      the hit,
+    unsigned char cand_o[kFirstCap];      //      the seed (lane)
 };
 
-template <typename Idx>
-struct WarpShared {
+template <typename Idx, bool kDv1>
+struct WarpShared : DvShared<Idx, kDv1> {
     FitRes res[kFitCap];                  // fit phase: result of fit task i
     SeedRec rec[32];
     float2 zw3[kFirstCap];                // (z, w) of the first hit
@@ -123,31 +171,33 @@ struct WarpShared {
     unsigned long long best_bits[32];     // per seed: smallest score among its fits (bits of the non-negative double)
     int best_fit[32];                     // per seed: first fit task with that score
     int n_best[32];                       // per seed: fits with that score (+ 2 for every first hit left to the seed's thread)
-    int dv_off[32], dv_a[32];             // Dv1: first item and first UTbX candidate of the seed
-    float cand_z[kFirstCap];              // Dv1: items that passed the fp32 pre-test: z of the UTbX hit,
-    Idx cand_j3[kFirstCap];               //      the hit,
-    unsigned char cand_o[kFirstCap];      //      the seed (lane)
     // Dv1 keeps at most kFirstCap triplets in slot[]; the rest of it holds the fit queue (4 per triplet)
     __device__ __forceinline__ unsigned short *dv_task_ptr() { return reinterpret_cast<unsigned short *>(slot + kFirstCap); }
 };
 static_assert((32 * kMaxFirst - kFirstCap) * 2 >= 4 * kFirstCap * 2, "slot[] holds the Dv1 triplets and their fit queue");
 
 // Block-shared state of k_track (carved from dynamic shared memory, followed by the staged hit arrays); W warps.
-template <typename Idx, int W>
+template <typename Idx, bool kDv1, int W>
 struct TrackShared {
     unsigned long long bar;
-    WarpShared<Idx> warp[W];
+    WarpShared<Idx, kDv1> warp[W];
+    float2 yb[kLayers * DS_MAX_SECTORS];  // (ymin, ymax) of each (layer, sector) of the event (uniform events)
     Idx tab[kMaxBins + 1];                // the event's bin table
 };
 static_assert(kFirstCap <= 512 && kFitCap < 0xfff, "packing of task[] and ffit[]");
 
-// The event's hits as the searches see them: x0 / ymin / ymax from the staging buffer (or global for an oversize
-// event), the rest always from global memory.  Indices are relative to the event's sorted slice.
+// The event's hits as the searches see them: x0 from the staging buffer (or global for an oversize event), the rest always
+// from global memory: the per-hit y bounds (read only when the event is not uniform) and the aux record (z, w, perm, id).
+// Indices are relative to the event's sorted slice.
 struct EventHits {
-    const float *x0, *ymin, *ymax;   // shared or global
-    const float *z, *w;              // global
-    const int32_t *id, *perm;        // global
+    const float *x0;             // shared or global
+    const float *ymin, *ymax;    // global
+    const float4 *aux;           // global
 };
+
+__device__ __forceinline__ float2 hit_zw(const EventHits &H, int j) { return *reinterpret_cast<const float2 *>(H.aux + j); }
+__device__ __forceinline__ int hit_perm(const EventHits &H, int j) { return __float_as_int(H.aux[j].z); }
+__device__ __forceinline__ int hit_id(const EventHits &H, int j) { return __float_as_int(H.aux[j].w); }
 
 template <typename Idx>
 __device__ __forceinline__ int idx_get(Idx v) { return v == (Idx)-1 ? -1 : (int)v; }
@@ -156,9 +206,12 @@ __device__ __forceinline__ int idx_get(Idx v) { return v == (Idx)-1 ? -1 : (int)
 // the window test that picked them.  The test issues an L1 prefetch so that the later read does not wait on DRAM.
 __device__ __forceinline__ void prefetch_l1(const void *p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
 
-// y-compatibility of hit j (O-S3: ymin - y_tol <= y <= ymax + y_tol); no short circuit: both loads are always issued
+// y-compatibility of hit j (O-S3: ymin - y_tol <= y <= ymax + y_tol); no short circuit: both loads are always issued.
+// kUni: decided per sector already (sector_mask), nothing to read.
+template <bool kUni>
 __device__ __forceinline__ bool y_compatible(const DevConst &c, const EventHits &H, int j, double y)
 {
+    if (kUni) return true;
     const double lo = (double)H.ymin[j] - c.y_tol, hi = (double)H.ymax[j] + c.y_tol;
     return (lo <= y) & (y <= hi);
 }
@@ -168,7 +221,7 @@ __device__ __forceinline__ bool closer(const EventHits &H, double d1, int j1, do
 {
     if (d1 != d2) return d1 < d2;
     if (j2 < 0) return true;
-    return H.id[j1] < H.id[j2];
+    return hit_id(H, j1) < hit_id(H, j2);
 }
 
 // fp32 superset test of "|x0 + off - x| <= w" (decided in fp64 afterwards): |x0 - t| <= w', with t = (float)(x - off)
@@ -198,9 +251,9 @@ __device__ __forceinline__ int lower_bound_x0(const float *x0, int a, int b, flo
 // S4: closest and second closest y-compatible hit of layer l (sectors tl..th) within w1 of the prediction xp;
 // -1 = none.  Inside a sector the hits are x0-sorted: binary search to the lower edge of the (fp32, widened) window,
 // then only the hits inside it are looked at in fp64.
-template <typename Tab>
+template <bool kUni, typename Tab>
 __device__ __forceinline__ int2 search_layer(const DevConst &c, const EventHits &H, const Tab *tab, int l, double xp,
-                                             double y, double w1, int tl, int th)
+                                             double y, double w1, unsigned mask)
 {
     int j0 = -1, j1 = -1;
     double d0 = 1e300, d1 = 1e300;
@@ -208,12 +261,13 @@ __device__ __forceinline__ int2 search_layer(const DevConst &c, const EventHits 
     const double lo = xp - off - w1, hi = xp - off + w1;
     const Prefilter pf = make_prefilter(xp - off, w1);
     const float xl = pf.t - pf.w, xh = pf.t + pf.w;
-    for (int sec = tl; sec <= th; ++sec) {
+    for (unsigned m = mask; m; m &= m - 1) {
+        const int sec = __ffs(m) - 1;
         int a, b;
         slice_range(c, tab, l, sec, lo, hi, a, b);
         for (int j = lower_bound_x0(H.x0, a, b, xl); j < b && H.x0[j] <= xh; ++j) {
             const double d = fabs(((double)H.x0[j] + off) - xp);
-            const bool pass = (d <= w1) & y_compatible(c, H, j, y);
+            const bool pass = (d <= w1) & y_compatible<kUni>(c, H, j, y);
             if (pass) {
                 if (closer(H, d, j, d0, j0)) {
                     d1 = d0; j1 = j0;
@@ -231,8 +285,8 @@ __device__ __forceinline__ int2 search_layer(const DevConst &c, const EventHits 
 // that touches one or two sectors: every sector is an x0-sorted range, so the closest hits are found by walking
 // outwards from the window centre, one left and one right head per sector, always taking the closest head.  Returns
 // false (dst not valid) when it meets equal x0 on a left side, where the walk order is not the id order.
-template <typename Idx>
-__device__ __noinline__ bool select_first_walk(const DevConst &c, const EventHits &H, const Idx *tab, int s_lo, int s_hi,
+template <bool kUni, typename Idx>
+__device__ __noinline__ bool select_first_walk(const DevConst &c, const EventHits &H, const Idx *tab, int sec_a, int sec_b,
                                                double off3, double xc, double w0, double y, int max_first, Idx *dst)
 {
     int hj[4], hend[4];
@@ -240,8 +294,9 @@ __device__ __noinline__ bool select_first_walk(const DevConst &c, const EventHit
 #pragma unroll
     for (int k = 0; k < 2; ++k) {
         int A = 0, B = 0;
-        if (s_lo + k <= s_hi) {
-            const int base = (3 * c.n_sectors + s_lo + k) * kXBins;
+        const int sec = k ? sec_b : sec_a;   // -1: none
+        if (sec >= 0) {
+            const int base = (3 * c.n_sectors + sec) * kXBins;
             A = tab[base];
             B = tab[base + kXBins];
         }
@@ -258,7 +313,7 @@ __device__ __noinline__ bool select_first_walk(const DevConst &c, const EventHit
         for (; j != end; j += step) {
             d = fabs(((double)H.x0[j] + off3) - xc);
             if (d > w0) { j = end; break; }
-            if (y_compatible(c, H, j, y)) break;
+            if (y_compatible<kUni>(c, H, j, y)) break;
         }
     };
 #pragma unroll
@@ -297,7 +352,7 @@ __device__ __noinline__ bool tie_better(const EventHits &H, const Candidate &p, 
     const int pj[4] = {p.j3, p.j0, p.j1, p.j2}, qj[4] = {q.j3, q.j0, q.j1, q.j2};
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
-        const int pi = pj[k] >= 0 ? H.id[pj[k]] : INT32_MAX, qi = qj[k] >= 0 ? H.id[qj[k]] : INT32_MAX;
+        const int pi = pj[k] >= 0 ? hit_id(H, pj[k]) : INT32_MAX, qi = qj[k] >= 0 ? hit_id(H, qj[k]) : INT32_MAX;
         if (pi != qi) return pi < qi;
     }
     return false;
@@ -310,7 +365,8 @@ __device__ __forceinline__ FitRes fit_combo(const DevConst &c, const EventHits &
 {
     // all loads first (z, w come from global memory)
     const int k0 = max(j0, 0), k1 = max(j1, 0), k2 = max(j2, 0);
-    const float fz0 = H.z[k0], fw0 = H.w[k0], fz1 = H.z[k1], fw1 = H.w[k1], fz2 = H.z[k2], fw2 = H.w[k2];
+    const float2 zw0 = hit_zw(H, k0), zw1 = hit_zw(H, k1), zw2 = hit_zw(H, k2);
+    const float fz0 = zw0.x, fw0 = zw0.y, fz1 = zw1.x, fw1 = zw1.y, fz2 = zw2.x, fw2 = zw2.y;
     const float fx0 = H.x0[k0], fx1 = H.x0[k1], fx2 = H.x0[k2], fx3 = H.x0[j3];
     const bool u0 = j0 >= 0, u1 = j1 >= 0, u2 = j2 >= 0;
     const int nh = 1 + u0 + u1 + u2;
@@ -353,8 +409,8 @@ __device__ __forceinline__ void write_not_found(const ds_tracks &out, int64_t s)
 
 // S6 in full for one seed (first hits f0 .. f0+nF-1 of the warp's list, seed in lane o): every combination in turn,
 // equal scores resolved by (more hits, ids) (A-9), combinations that the fit phase did not take fitted here.
-template <typename Idx>
-__device__ __noinline__ Candidate choose_general(const DevConst &c, const WarpShared<Idx> &sh, const EventHits &H, int f0,
+template <typename Idx, bool kDv1>
+__device__ __noinline__ Candidate choose_general(const DevConst &c, const WarpShared<Idx, kDv1> &sh, const EventHits &H, int f0,
                                                  int nF, int o)
 {
     Candidate best;
@@ -407,9 +463,10 @@ __device__ __forceinline__ SeedPre load_seed(const ds_seeds &seeds, int s, bool 
 //   F  lane per queued combination: fit (S5)
 //   C  lane per seed:       best candidate (S6), track record
 // A round takes the longest prefix of the remaining seeds whose first hits fit the warp's list.
-template <typename Idx>
-__device__ __forceinline__ void track_chunk(const DevConst &c, WarpShared<Idx> &sh, const Idx *tab, const EventHits &H,
-                                            const ds_seeds &seeds, int cb, int ce, const ds_tracks &out, const SeedPre &pre)
+template <typename Idx, bool kUni>
+__device__ __forceinline__ void track_chunk(const DevConst &c, WarpShared<Idx, false> &sh, const Idx *tab, const float2 *yb,
+                                            const EventHits &H, const ds_seeds &seeds, int cb, int ce, const ds_tracks &out,
+                                            const SeedPre &pre)
 {
     const unsigned FULL = 0xffffffffu;
     const int lane = threadIdx.x & 31;
@@ -431,34 +488,30 @@ __device__ __forceinline__ void track_chunk(const DevConst &c, WarpShared<Idx> &
             const float fx = sp.x, fq = sp.qop;
             fy = sp.y; ftx = sp.tx; fty = sp.ty;
             const S2 s2 = extrapolate_seed(c, fx, fy, ftx, fty, fq);
+            const unsigned mask3 = sector_mask<kUni>(c, yb, 3, s2.y3);
             {
                 SeedRec &r = sh.rec[lane];
                 r.xm = s2.xm; r.zm = s2.zm; r.w1 = s2.w1;
                 r.y[0] = s2.y0; r.y[1] = s2.y1; r.y[2] = s2.y2; r.y[3] = s2.y3;
 #pragma unroll
-                for (int l = 0; l < 3; ++l) {
-                    int tl, th;
-                    sector_range(c, l == 0 ? s2.y0 : (l == 1 ? s2.y1 : s2.y2), tl, th);
-                    r.sec[l][0] = (unsigned char)(th < tl ? 1 : tl);
-                    r.sec[l][1] = (unsigned char)(th < tl ? 0 : th);
-                }
+                for (int l = 0; l < 3; ++l)
+                    r.mask[l] = (unsigned short)sector_mask<kUni>(c, yb, l, l == 0 ? s2.y0 : (l == 1 ? s2.y1 : s2.y2));
+                r.mask[3] = (unsigned short)mask3;
             }
-            int s_lo, s_hi;
-            sector_range(c, s2.y3, s_lo, s_hi);
             const double off3 = c.dxdy[3] * s2.y3;
             const double lo3 = s2.xc3 - off3 - s2.w0, hi3 = s2.xc3 - off3 + s2.w0;
             const Prefilter pf = make_prefilter(s2.xc3 - off3, s2.w0);
             const float xl = pf.t - pf.w, xh = pf.t + pf.w;
-            for (int sec = s_lo; sec <= s_hi; ++sec) {
+            for (unsigned m = mask3; m; m &= m - 1) {
+                const int sec = __ffs(m) - 1;
                 int a, b;
                 slice_range(c, tab, 3, sec, lo3, hi3, a, b);
                 for (int j = lower_bound_x0(H.x0, a, b, xl); j < b && H.x0[j] <= xh; ++j) {
                     const double d = fabs(((double)H.x0[j] + off3) - s2.xc3);
-                    if ((d <= s2.w0) & y_compatible(c, H, j, s2.y3)) {
+                    if ((d <= s2.w0) & y_compatible<kUni>(c, H, j, s2.y3)) {
                         if (nF < max_first) {
                             my_slot[nF] = (Idx)j;
-                            prefetch_l1(H.z + j);
-                            prefetch_l1(H.w + j);
+                            prefetch_l1(H.aux + j);
                         }
                         ++nF;
                     }
@@ -467,20 +520,23 @@ __device__ __forceinline__ void track_chunk(const DevConst &c, WarpShared<Idx> &
             if (nF > max_first) {
                 // more hits in the window than are tried: the max_first closest by (distance, id)
                 bool done = false;
-                if (s_hi - s_lo <= 1)
-                    done = select_first_walk<Idx>(c, H, tab, s_lo, s_hi, off3, s2.xc3, s2.w0, s2.y3, max_first, my_slot);
+                if (__popc(mask3) <= 2) {
+                    const int sec_a = __ffs(mask3) - 1, sec_b = __ffs(mask3 & (mask3 - 1)) - 1;
+                    done = select_first_walk<kUni, Idx>(c, H, tab, sec_a, sec_b, off3, s2.xc3, s2.w0, s2.y3, max_first, my_slot);
+                }
                 if (!done) {   // general case: max_first selection passes over the window
                     double last_d = -1.0;
                     int last_j = -1;
                     for (int k = 0; k < max_first; ++k) {
                         double bd = 1e300;
                         int bj = -1;
-                        for (int sec = s_lo; sec <= s_hi; ++sec) {
+                        for (unsigned m = mask3; m; m &= m - 1) {
+                            const int sec = __ffs(m) - 1;
                             int a, b;
                             slice_range(c, tab, 3, sec, lo3, hi3, a, b);
                             for (int j = a; j < b; ++j) {
                                 const double d = fabs(((double)H.x0[j] + off3) - s2.xc3);
-                                if ((d <= s2.w0) & y_compatible(c, H, j, s2.y3)) {
+                                if ((d <= s2.w0) & y_compatible<kUni>(c, H, j, s2.y3)) {
                                     // strictly after the previous pick, and before the best so far
                                     const bool after = last_j < 0 || (j != last_j && closer(H, last_d, last_j, d, j));
                                     if (after && closer(H, d, j, bd, bj)) { bd = d; bj = j; }
@@ -512,10 +568,7 @@ __device__ __forceinline__ void track_chunk(const DevConst &c, WarpShared<Idx> &
             for (int k0 = 0; k0 < nFc; k0 += 5) {   // (z, w) of the first hits: five loads in flight at a time
                 float2 v[5];
 #pragma unroll
-                for (int u = 0; u < 5; ++u) {
-                    const int j = (int)my_slot[min(k0 + u, nFc - 1)];
-                    v[u] = make_float2(H.z[j], H.w[j]);
-                }
+                for (int u = 0; u < 5; ++u) v[u] = hit_zw(H, (int)my_slot[min(k0 + u, nFc - 1)]);
 #pragma unroll
                 for (int u = 0; u < 5; ++u) {
                     if (k0 + u < nFc) {
@@ -540,17 +593,16 @@ __device__ __forceinline__ void track_chunk(const DevConst &c, WarpShared<Idx> &
 #pragma unroll
                 for (int l = 0; l < 3; ++l) {
                     const double xp = t2.xm + txc * (c.z_layer[l] - t2.zm);
-                    r[l] = search_layer(c, H, tab, l, xp, t2.y[l], t2.w1, (int)t2.sec[l][0], (int)t2.sec[l][1]);
+                    r[l] = search_layer<kUni>(c, H, tab, l, xp, t2.y[l], t2.w1, (unsigned)t2.mask[l]);
                 }
                 r[0].y = -1;   // UTaX keeps the closest hit only
 #pragma unroll
                 for (int l = 0; l < 3; ++l) {
                     sh.near[3 * f + l][0] = (Idx)r[l].x;
                     sh.near[3 * f + l][1] = (Idx)r[l].y;
-                    if (r[l].x >= 0) { prefetch_l1(H.z + r[l].x); prefetch_l1(H.w + r[l].x); prefetch_l1(H.perm + r[l].x); }
-                    if (r[l].y >= 0) { prefetch_l1(H.z + r[l].y); prefetch_l1(H.w + r[l].y); prefetch_l1(H.perm + r[l].y); }
+                    if (r[l].x >= 0) prefetch_l1(H.aux + r[l].x);
+                    if (r[l].y >= 0) prefetch_l1(H.aux + r[l].y);
                 }
-                prefetch_l1(H.perm + j3);
                 const int nh = 1 + (r[0].x >= 0) + (r[1].x >= 0) + (r[2].x >= 0);
                 unsigned short ff = kFitNone;
                 if (nh >= c.min_hits) {
@@ -607,7 +659,7 @@ __device__ __forceinline__ void track_chunk(const DevConst &c, WarpShared<Idx> &
             Candidate best;
             best.score = kNoScore;
             if (general) {
-                best = choose_general<Idx>(c, sh, H, f0, nFc, lane);
+                best = choose_general<Idx, false>(c, sh, H, f0, nFc, lane);
             } else if (bt >= 0) {
                 const FitRes r = sh.res[bt];
                 const int tk = sh.task[bt], bf = tk & 511, i1 = (tk >> 9) & 1, i2 = (tk >> 10) & 1;
@@ -631,10 +683,10 @@ __device__ __forceinline__ void track_chunk(const DevConst &c, WarpShared<Idx> &
                 out.nhits[s] = best.nh;
                 out.found[s] = 1;
                 int4 hv;
-                hv.x = best.j0 >= 0 ? H.perm[best.j0] : -1;
-                hv.y = best.j1 >= 0 ? H.perm[best.j1] : -1;
-                hv.z = best.j2 >= 0 ? H.perm[best.j2] : -1;
-                hv.w = H.perm[best.j3];
+                hv.x = best.j0 >= 0 ? hit_perm(H, best.j0) : -1;
+                hv.y = best.j1 >= 0 ? hit_perm(H, best.j1) : -1;
+                hv.z = best.j2 >= 0 ? hit_perm(H, best.j2) : -1;
+                hv.w = hit_perm(H, best.j3);
                 reinterpret_cast<int4 *>(out.hit)[s] = hv;
             }
         }
@@ -656,7 +708,7 @@ __device__ __forceinline__ void track_chunk(const DevConst &c, WarpShared<Idx> &
 //      by the seed's lane with the best candidate it holds so far (exact ties: full (hits, ids) comparison)
 // and each seed's lane writes its track record at the end.
 template <typename Idx>
-__device__ __forceinline__ Candidate make_candidate(const WarpShared<Idx> &sh, const FitRes &r, int tk)
+__device__ __forceinline__ Candidate make_candidate(const WarpShared<Idx, true> &sh, const FitRes &r, int tk)
 {
     const int f = tk & 511, i1 = (tk >> 9) & 1, i2 = (tk >> 10) & 1;
     Candidate cand;
@@ -670,18 +722,18 @@ __device__ __forceinline__ Candidate make_candidate(const WarpShared<Idx> &sh, c
 }
 
 template <typename Idx>
-__device__ __forceinline__ FitRes fit_task(const DevConst &c, const WarpShared<Idx> &sh, const EventHits &H, int tk)
+__device__ __forceinline__ FitRes fit_task(const DevConst &c, const WarpShared<Idx, true> &sh, const EventHits &H, int tk)
 {
     const int f = tk & 511, i1 = (tk >> 9) & 1, i2 = (tk >> 10) & 1;
     const int j3 = (int)sh.slot[f];
     return fit_combo(c, H, sh.rec[sh.fs[f]], idx_get(sh.near[3 * f][0]), idx_get(sh.near[3 * f + 1][i1]),
-                     idx_get(sh.near[3 * f + 2][i2]), j3, (double)sh.zw3[f].x, (double)H.w[j3]);
+                     idx_get(sh.near[3 * f + 2][i2]), j3, (double)sh.zw3[f].x, (double)hit_zw(H, j3).y);
 }
 
 // S + F for the triplets [0, n_trip) of the warp's list (fs = owner lane, slot = UTbX hit, near[3f] = UTaX hit, zw3);
 // `best` is the candidate the calling lane's seed holds so far.
-template <typename Idx>
-__device__ __forceinline__ void dv1_flush(const DevConst &c, WarpShared<Idx> &sh, const Idx *tab, const EventHits &H,
+template <typename Idx, bool kUni>
+__device__ __forceinline__ void dv1_flush(const DevConst &c, WarpShared<Idx, true> &sh, const Idx *tab, const EventHits &H,
                                           int n_trip, Candidate &best)
 {
     const unsigned FULL = 0xffffffffu;
@@ -700,7 +752,7 @@ __device__ __forceinline__ void dv1_flush(const DevConst &c, WarpShared<Idx> &sh
             const double x3 = (double)H.x0[j3] + c.dxdy[3] * t2.y[3];
             const double txc = (x3 - t2.xm) / ((double)sh.zw3[f].x - t2.zm);
             const double xp = t2.xm + txc * (c.z_layer[l] - t2.zm);
-            r = search_layer(c, H, tab, l, xp, t2.y[l], t2.w1, (int)t2.sec[l][0], (int)t2.sec[l][1]);
+            r = search_layer<kUni>(c, H, tab, l, xp, t2.y[l], t2.w1, (unsigned)t2.mask[l]);
             sh.near[3 * f + l][0] = (Idx)r.x;
             sh.near[3 * f + l][1] = (Idx)r.y;
         }
@@ -766,9 +818,9 @@ __device__ __forceinline__ void dv1_flush(const DevConst &c, WarpShared<Idx> &sh
 }
 
 // Seeds [cb, ce) (at most 32) of one event with the Dv1 triplet search, by one warp on its own.
-template <typename Idx>
-__device__ __forceinline__ void track_chunk_dv1(const DevConst &c, WarpShared<Idx> &sh, const Idx *tab, const EventHits &H,
-                                                const ds_seeds &seeds, int cb, int ce, const ds_tracks &out)
+template <typename Idx, bool kUni>
+__device__ __forceinline__ void track_chunk_dv1(const DevConst &c, WarpShared<Idx, true> &sh, const Idx *tab, const float2 *yb,
+                                                const EventHits &H, const ds_seeds &seeds, int cb, int ce, const ds_tracks &out)
 {
     const unsigned FULL = 0xffffffffu;
     const int lane = threadIdx.x & 31;
@@ -785,15 +837,13 @@ __device__ __forceinline__ void track_chunk_dv1(const DevConst &c, WarpShared<Id
         r.xm = s2.xm; r.zm = s2.zm; r.w1 = s2.w1;
         r.y[0] = s2.y0; r.y[1] = s2.y1; r.y[2] = s2.y2; r.y[3] = s2.y3;
 #pragma unroll
-        for (int l = 0; l < 3; ++l) {
-            int tl, th;
-            sector_range(c, l == 0 ? s2.y0 : (l == 1 ? s2.y1 : s2.y2), tl, th);
-            r.sec[l][0] = (unsigned char)(th < tl ? 1 : tl);
-            r.sec[l][1] = (unsigned char)(th < tl ? 0 : th);
-        }
-        int s_lo, s_hi;
-        sector_range(c, s2.y3, s_lo, s_hi);
-        if (s_lo <= s_hi) {   // the sectors of a layer follow each other in the sorted slice: one range
+        for (int l = 0; l < 3; ++l)
+            r.mask[l] = (unsigned short)sector_mask<kUni>(c, yb, l, l == 0 ? s2.y0 : (l == 1 ? s2.y1 : s2.y2));
+        const unsigned mask3 = sector_mask<kUni>(c, yb, 3, s2.y3);
+        r.mask[3] = (unsigned short)mask3;
+        if (mask3) {   // the sectors of a layer follow each other in the sorted slice: one range from the lowest to the
+                       // highest compatible sector (a sector in between that is not compatible is sorted out per item)
+            const int s_lo = __ffs(mask3) - 1, s_hi = 31 - __clz(mask3);
             a_o = (int)tab[(3 * c.n_sectors + s_lo) * kXBins];
             n_o = (int)tab[(3 * c.n_sectors + s_hi + 1) * kXBins] - a_o;
         }
@@ -819,7 +869,7 @@ __device__ __forceinline__ void track_chunk_dv1(const DevConst &c, WarpShared<Id
         // last seed whose first item is <= t (seeds without items share the offset of the next); a lane's items only go up
         while (o < 31 && sh.dv_off[o + 1] <= t) ++o;
         j3 = sh.dv_a[o] + (t - sh.dv_off[o]);
-        z3 = H.z[j3];
+        z3 = H.aux[j3].x;
     };
     int o_nx = 0, j3_nx = 0;
     float z3_nx = 0.f;
@@ -835,11 +885,11 @@ __device__ __forceinline__ void track_chunk_dv1(const DevConst &c, WarpShared<Id
             const int q = n_cand - cnt + lane;
             o = sh.cand_o[q]; j3 = (int)sh.cand_j3[q]; z3 = sh.cand_z[q];
             const SeedRec &t2 = sh.rec[o];
-            if (y_compatible(c, H, j3, t2.y[3])) {
+            if (y_compatible<kUni>(c, H, j3, t2.y[3])) {   // kUni: the pre-test has decided it (exactly, by sector)
                 const double x3 = (double)H.x0[j3] + c.dxdy[3] * t2.y[3];
                 const double txc = (x3 - t2.xm) / ((double)z3 - t2.zm);
                 const double xp = t2.xm + txc * (c.z_layer[0] - t2.zm);
-                j0 = search_layer(c, H, tab, 0, xp, t2.y[0], t2.w1, (int)t2.sec[0][0], (int)t2.sec[0][1]).x;
+                j0 = search_layer<kUni>(c, H, tab, 0, xp, t2.y[0], t2.w1, (unsigned)t2.mask[0]).x;
                 has = j0 >= 0;
             }
         }
@@ -855,7 +905,7 @@ __device__ __forceinline__ void track_chunk_dv1(const DevConst &c, WarpShared<Id
         }
         n_trip += __popc(m);
         if (n_trip >= 32) {   // the list holds 64: room for one more round is guaranteed after this
-            dv1_flush<Idx>(c, sh, tab, H, n_trip, best);
+            dv1_flush<Idx, kUni>(c, sh, tab, H, n_trip, best);
             n_trip = 0;
         }
     };
@@ -872,7 +922,17 @@ __device__ __forceinline__ void track_chunk_dv1(const DevConst &c, WarpShared<Id
         if (t < total) {
             const SeedRec &t2 = sh.rec[o];
             const float y3 = (float)t2.y[3];
-            if (H.ymin[j3] - ytol_f <= y3 && y3 <= H.ymax[j3] + ytol_f) {
+            bool y_ok;
+            if (kUni) {   // the hit's sector: the last one of the seed's range that starts at or before the hit
+                const unsigned mask3 = t2.mask[3];
+                int sec = __ffs(mask3) - 1;
+                const int s_hi = 31 - __clz(mask3);
+                while (sec < s_hi && j3 >= (int)tab[(3 * c.n_sectors + sec + 1) * kXBins]) ++sec;
+                y_ok = (mask3 >> sec) & 1u;
+            } else {
+                y_ok = H.ymin[j3] - ytol_f <= y3 && y3 <= H.ymax[j3] + ytol_f;
+            }
+            if (y_ok) {
                 const float xm = (float)t2.xm, zm = (float)t2.zm;
                 const float x3 = H.x0[j3] + (float)(c.dxdy[3] * t2.y[3]);
                 const float xp = xm + (x3 - xm) * ((zl0_f - zm) / (z3 - zm));
@@ -880,8 +940,8 @@ __device__ __forceinline__ void track_chunk_dv1(const DevConst &c, WarpShared<Id
                 const float wf = (float)t2.w1 * 1.0001f + 0.05f + 4e-6f * fabsf(tg);
                 const float xl = tg - wf, xh = tg + wf;
                 const int bl = xbin(xl, c.xb_off, c.xb_scale), bh = xbin(xh, c.xb_off, c.xb_scale);
-                for (int sec = (int)t2.sec[0][0]; sec <= (int)t2.sec[0][1] && !cand; ++sec) {
-                    const int base = sec * kXBins;   // layer 0
+                for (unsigned m0 = t2.mask[0]; m0 && !cand; m0 &= m0 - 1) {
+                    const int base = (__ffs(m0) - 1) * kXBins;   // layer 0
                     const int a = (int)tab[base + bl], b = (int)tab[base + bh + 1];
                     const int j = lower_bound_x0(H.x0, a, b, xl);
                     cand = j < b && H.x0[j] <= xh;
@@ -901,7 +961,7 @@ __device__ __forceinline__ void track_chunk_dv1(const DevConst &c, WarpShared<Id
         if (n_cand >= 32) exact_round(32);
     }
     if (n_cand > 0) exact_round(n_cand);
-    if (n_trip > 0) dv1_flush<Idx>(c, sh, tab, H, n_trip, best);
+    if (n_trip > 0) dv1_flush<Idx, kUni>(c, sh, tab, H, n_trip, best);
     // ---- track record ------------------------------------------------------------------------------------------------------------
     if (act) {
         if (best.score == kNoScore) {
@@ -917,10 +977,10 @@ __device__ __forceinline__ void track_chunk_dv1(const DevConst &c, WarpShared<Id
             out.nhits[s] = best.nh;
             out.found[s] = 1;
             int4 hv;
-            hv.x = best.j0 >= 0 ? H.perm[best.j0] : -1;
-            hv.y = best.j1 >= 0 ? H.perm[best.j1] : -1;
-            hv.z = best.j2 >= 0 ? H.perm[best.j2] : -1;
-            hv.w = H.perm[best.j3];
+            hv.x = best.j0 >= 0 ? hit_perm(H, best.j0) : -1;
+            hv.y = best.j1 >= 0 ? hit_perm(H, best.j1) : -1;
+            hv.z = best.j2 >= 0 ? hit_perm(H, best.j2) : -1;
+            hv.w = hit_perm(H, best.j3);
             reinterpret_cast<int4 *>(out.hit)[s] = hv;
         }
     }
@@ -934,21 +994,22 @@ __device__ __forceinline__ int seed_chunk(int s_begin, int s_end)
     return min(32, (s_end - s_begin + W - 1) / W);
 }
 
-template <typename Idx, bool kDv1, int W>
-__device__ __forceinline__ void track_event(const DevConst &c, TrackShared<Idx, W> &sh, const EventHits &H,
+template <typename Idx, bool kDv1, bool kUni, int W>
+__device__ __forceinline__ void track_event(const DevConst &c, TrackShared<Idx, kDv1, W> &sh, const EventHits &H,
                                             const ds_seeds &seeds, int s_begin, int s_end, const ds_tracks &out,
                                             const SeedPre &pre)
 {
     const int wid = threadIdx.x >> 5;
     const int chunk = seed_chunk<W>(s_begin, s_end);
     for (int cb = s_begin + wid * chunk; cb < s_end; cb += W * chunk) {
-        if (kDv1) track_chunk_dv1<Idx>(c, sh.warp[wid], sh.tab, H, seeds, cb, min(cb + chunk, s_end), out);
-        else track_chunk<Idx>(c, sh.warp[wid], sh.tab, H, seeds, cb, min(cb + chunk, s_end), out, pre);
+        if constexpr (kDv1) track_chunk_dv1<Idx, kUni>(c, sh.warp[wid], sh.tab, sh.yb, H, seeds, cb, min(cb + chunk, s_end), out);
+        else track_chunk<Idx, kUni>(c, sh.warp[wid], sh.tab, sh.yb, H, seeds, cb, min(cb + chunk, s_end), out, pre);
     }
 }
 
-// W warps per block: 5 when three blocks share an SM (the Run-3-like event sizes); events whose staging leaves room for
-// two blocks or one get 8 or 12 warps, so that an SM keeps about the same number of warps busy
+// W warps per block and kMinBlocks blocks per SM follow the staging size (launch_track): the Run-3-like event sizes run
+// 5 warps x 4 blocks; events whose staging leaves room for fewer blocks get more warps per block, so that an SM keeps
+// about the same number of warps busy
 template <bool kDv1, int W, int kMinBlocks>
 __global__ void __launch_bounds__(32 * W, kMinBlocks)
 k_track(const __grid_constant__ DevConst c, const LayoutPtrs L, const ds_seeds seeds,
@@ -956,17 +1017,17 @@ k_track(const __grid_constant__ DevConst c, const LayoutPtrs L, const ds_seeds s
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     constexpr int kThreads = 32 * W;
-    using Staged = TrackShared<uint16_t, W>;
-    using Direct = TrackShared<int, W>;
+    using Staged = TrackShared<uint16_t, kDv1, W>;
+    using Direct = TrackShared<int, kDv1, W>;
     constexpr size_t kHitsAt = (sizeof(Staged) + 15) & ~(size_t)15;
-    float *st_x0 = reinterpret_cast<float *>(smem_raw + kHitsAt);   // [cap], then ymin [cap], ymax [cap]
-    float *st_ymin = st_x0 + cap, *st_ymax = st_ymin + cap;
+    float *st_x0 = reinterpret_cast<float *>(smem_raw + kHitsAt);   // [cap]
 
     const int e = blockIdx.x;
     const int tid = threadIdx.x;
     const int s_begin = seed_offsets[e], s_end = seed_offsets[e + 1];
     if (s_begin == s_end) return;
     const int h0 = hit_offsets[e], h1 = hit_offsets[e + 1];
+    const bool uni = L.uniform[e] != 0;
     // staged range: the event's slice widened to 16-byte boundaries (the sorted arrays are 256-byte aligned and padded)
     const int h0a = h0 & ~3, cnt = ((h1 + 3) & ~3) - h0a;
     const bool staged = cnt <= cap;   // cap < 65535 (see launch_track)
@@ -974,12 +1035,8 @@ k_track(const __grid_constant__ DevConst c, const LayoutPtrs L, const ds_seeds s
     if (tid == 0 && staged) {
         mbar_init(bar, 1);
         const uint32_t bytes = 4u * (uint32_t)cnt;
-        mbar_expect_tx(bar, 3u * bytes);
-        if (bytes) {
-            bulk_g2s(st_x0, L.sx0 + h0a, bytes, bar);
-            bulk_g2s(st_ymin, L.symin + h0a, bytes, bar);
-            bulk_g2s(st_ymax, L.symax + h0a, bytes, bar);
-        }
+        mbar_expect_tx(bar, bytes);
+        if (bytes) bulk_g2s(st_x0, L.sx0 + h0a, bytes, bar);
     }
     // the lane's first seed, fetched now so that the load is in flight with the table and the hits
     SeedPre pre;
@@ -990,32 +1047,87 @@ k_track(const __grid_constant__ DevConst c, const LayoutPtrs L, const ds_seeds s
     }
     const int nb = c.n_bins;
     const int32_t *gtab = L.bin_offsets + (size_t)e * (nb + 1);
+    const int nyb = kLayers * c.n_sectors;
     if (staged) {
-        uint16_t *tab = reinterpret_cast<Staged *>(smem_raw)->tab;
+        Staged &sh = *reinterpret_cast<Staged *>(smem_raw);
         constexpr int kPer = (kMaxBins + kThreads) / kThreads;
         int v[kPer];
 #pragma unroll
         for (int u = 0; u < kPer; ++u) v[u] = gtab[min(tid + u * kThreads, nb)];
+        float2 ybv = make_float2(0.f, 0.f);
+        if (tid < nyb) ybv = L.ybounds[(size_t)e * nyb + tid];
 #pragma unroll
         for (int u = 0; u < kPer; ++u)
-            if (tid + u * kThreads <= nb) tab[tid + u * kThreads] = (uint16_t)v[u];
+            if (tid + u * kThreads <= nb) sh.tab[tid + u * kThreads] = (uint16_t)v[u];
+        if (tid < nyb) sh.yb[tid] = ybv;
     } else {
-        int *tab = reinterpret_cast<Direct *>(smem_raw)->tab;
-        for (int b = tid; b <= nb; b += kThreads) tab[b] = gtab[b];
+        Direct &sh = *reinterpret_cast<Direct *>(smem_raw);
+        for (int b = tid; b <= nb; b += kThreads) sh.tab[b] = gtab[b];
+        if (tid < nyb) sh.yb[tid] = L.ybounds[(size_t)e * nyb + tid];
     }
     __syncthreads();
 
     EventHits H;
-    H.z = L.sz + h0; H.w = L.sw + h0; H.id = L.sid + h0; H.perm = L.perm + h0;
+    H.ymin = L.symin + h0; H.ymax = L.symax + h0; H.aux = L.aux + h0;
     if (staged) {
         mbar_wait(bar, 0);
-        const int d = h0 - h0a;
-        H.x0 = st_x0 + d; H.ymin = st_ymin + d; H.ymax = st_ymax + d;
-        track_event<uint16_t, kDv1, W>(c, *reinterpret_cast<Staged *>(smem_raw), H, seeds, s_begin, s_end, out, pre);
+        H.x0 = st_x0 + (h0 - h0a);
+        Staged &sh = *reinterpret_cast<Staged *>(smem_raw);
+        if (uni) track_event<uint16_t, kDv1, true, W>(c, sh, H, seeds, s_begin, s_end, out, pre);
+        else track_event<uint16_t, kDv1, false, W>(c, sh, H, seeds, s_begin, s_end, out, pre);
     } else {
-        H.x0 = L.sx0 + h0; H.ymin = L.symin + h0; H.ymax = L.symax + h0;
-        track_event<int, kDv1, W>(c, *reinterpret_cast<Direct *>(smem_raw), H, seeds, s_begin, s_end, out, pre);
+        H.x0 = L.sx0 + h0;
+        Direct &sh = *reinterpret_cast<Direct *>(smem_raw);
+        if (uni) track_event<int, kDv1, true, W>(c, sh, H, seeds, s_begin, s_end, out, pre);
+        else track_event<int, kDv1, false, W>(c, sh, H, seeds, s_begin, s_end, out, pre);
     }
+}
+
+// Threads and blocks per SM tried for a staging size, most blocks first (see launch_track)
+template <bool kDv1, int W, int kMinBlocks>
+static cudaError_t launch_one(const DevConst &c, const LayoutPtrs &lay, const ds_seeds &seeds, const int32_t *hit_offsets,
+                              const int32_t *seed_offsets, int n_events, int cap, size_t smem, const ds_tracks &out,
+                              cudaStream_t st, Prof &prof)
+{
+    static unsigned long long opted = 0;
+    const cudaError_t aerr = opt_in_max_smem(k_track<kDv1, W, kMinBlocks>, &opted);
+    if (aerr != cudaSuccess) return aerr;
+    prof.begin(DS_K_TRACK, st);
+    k_track<kDv1, W, kMinBlocks><<<n_events, 32 * W, smem, st>>>(c, lay, seeds, hit_offsets, seed_offsets, out, cap);
+    prof.end(st);
+    return cudaGetLastError();
+}
+
+template <bool kDv1, int W>
+static size_t track_smem(int cap)
+{
+    const size_t fixed = (sizeof(TrackShared<uint16_t, kDv1, W>) + 15) & ~(size_t)15;
+    const size_t staged = fixed + (size_t)cap * 4, direct = sizeof(TrackShared<int, kDv1, W>);
+    return staged > direct ? staged : direct;
+}
+
+template <bool kDv1>
+static cudaError_t launch_track_t(const DevConst &c, const LayoutPtrs &lay, const ds_seeds &seeds, const int32_t *hit_offsets,
+                                  const int32_t *seed_offsets, int n_events, int hint, const ds_tracks &out, cudaStream_t st,
+                                  Prof &prof)
+{
+    // staging capacity in hits (a multiple of 4, with room for the alignment slack): 4 bytes each; positions of a staged
+    // event are stored as uint16_t with 0xffff = none
+    int cap = ((hint + 3) & ~3) + 8;
+    const size_t kSm = 227 * 1024, kPerBlock = 1024;   // usable shared memory of an SM; reserved per resident block
+    // configuration: as many blocks per SM as the staging allows (more resident warps hide more latency)
+    const int want = track_blocks_override();
+    if ((want == 0 || want == 4) && 4 * (track_smem<kDv1, 5>(cap) + kPerBlock) <= kSm + 1024)
+        return launch_one<kDv1, 5, 4>(c, lay, seeds, hit_offsets, seed_offsets, n_events, cap, track_smem<kDv1, 5>(cap), out, st, prof);
+    if ((want == 0 || want == 3) && 3 * (track_smem<kDv1, 5>(cap) + kPerBlock) <= kSm + 1024)
+        return launch_one<kDv1, 5, 3>(c, lay, seeds, hit_offsets, seed_offsets, n_events, cap, track_smem<kDv1, 5>(cap), out, st, prof);
+    if (2 * (track_smem<kDv1, 8>(cap) + kPerBlock) <= kSm + 1024)
+        return launch_one<kDv1, 8, 2>(c, lay, seeds, hit_offsets, seed_offsets, n_events, cap, track_smem<kDv1, 8>(cap), out, st, prof);
+    const size_t fixed = (sizeof(TrackShared<uint16_t, kDv1, 12>) + 15) & ~(size_t)15;
+    int cap_max = (int)((kSm - fixed) / 4) & ~3;
+    if (cap_max > 65528) cap_max = 65528;
+    if (cap > cap_max) cap = cap_max;
+    return launch_one<kDv1, 12, 1>(c, lay, seeds, hit_offsets, seed_offsets, n_events, cap, track_smem<kDv1, 12>(cap), out, st, prof);
 }
 
 cudaError_t launch_track(const DevConst &c, const LayoutPtrs &lay, const ds_seeds &seeds, const int32_t *hit_offsets,
@@ -1023,37 +1135,10 @@ cudaError_t launch_track(const DevConst &c, const LayoutPtrs &lay, const ds_seed
                          cudaStream_t st, Prof &prof)
 {
     if (n_events <= 0) return cudaSuccess;
-    // staging capacity in hits (a multiple of 4, with room for the alignment slack): 12 bytes each; positions of a
-    // staged event are stored as uint16_t with 0xffff = none
     const int hint = max_event_hits_hint > 0 ? max_event_hits_hint : 4096;
-    auto launch = [&](auto kernel, unsigned long long *opted, size_t bytes_staged, size_t bytes_direct, int threads) -> cudaError_t {
-        const size_t fixed = (bytes_staged + 15) & ~(size_t)15;
-        int cap_max = (int)((227 * 1024 - fixed) / 12) & ~3;
-        if (cap_max > 65528) cap_max = 65528;
-        int cap = ((hint + 3) & ~3) + 8;
-        if (cap > cap_max) cap = cap_max;
-        size_t smem = fixed + (size_t)cap * 12;
-        if (smem < bytes_direct) smem = bytes_direct;   // the layout of an event that is not staged
-        const cudaError_t aerr = opt_in_max_smem(kernel, opted);
-        if (aerr != cudaSuccess) return aerr;
-        prof.begin(DS_K_TRACK, st);
-        kernel<<<n_events, threads, smem, st>>>(c, lay, seeds, hit_offsets, seed_offsets, out, cap);
-        prof.end(st);
-        return cudaGetLastError();
-    };
-    // blocks per SM that the 5-warp layout would reach with this hint decide the warps per block
-    const size_t smem5 = ((sizeof(TrackShared<uint16_t, 5>) + 15) & ~(size_t)15) + (size_t)(((hint + 3) & ~3) + 8) * 12 + 1024;
-    const int per_sm = (int)((228 * 1024) / smem5);
     // Dv1 (triplet search, P:107-P:111) and Dv0 are separate instantiations: the Dv0 hot path carries none of the other's code
-    static unsigned long long opted[6] = {0, 0, 0, 0, 0, 0};
-    if (per_sm >= 3)
-        return c.dv1 ? launch(k_track<true, 5, 3>, &opted[0], sizeof(TrackShared<uint16_t, 5>), sizeof(TrackShared<int, 5>), 160)
-                     : launch(k_track<false, 5, 3>, &opted[1], sizeof(TrackShared<uint16_t, 5>), sizeof(TrackShared<int, 5>), 160);
-    if (per_sm == 2)
-        return c.dv1 ? launch(k_track<true, 8, 2>, &opted[2], sizeof(TrackShared<uint16_t, 8>), sizeof(TrackShared<int, 8>), 256)
-                     : launch(k_track<false, 8, 2>, &opted[3], sizeof(TrackShared<uint16_t, 8>), sizeof(TrackShared<int, 8>), 256);
-    return c.dv1 ? launch(k_track<true, 12, 1>, &opted[4], sizeof(TrackShared<uint16_t, 12>), sizeof(TrackShared<int, 12>), 384)
-                 : launch(k_track<false, 12, 1>, &opted[5], sizeof(TrackShared<uint16_t, 12>), sizeof(TrackShared<int, 12>), 384);
+    return c.dv1 ? launch_track_t<true>(c, lay, seeds, hit_offsets, seed_offsets, n_events, hint, out, st, prof)
+                 : launch_track_t<false>(c, lay, seeds, hit_offsets, seed_offsets, n_events, hint, out, st, prof);
 }
 
 }  // namespace ds

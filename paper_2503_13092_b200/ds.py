@@ -40,6 +40,16 @@ class DsMlp(ct.Structure):
                 ("mu", ct.c_float * DS_MLP_IN), ("inv_sigma", ct.c_float * DS_MLP_IN)]
 
 
+DS_MLP_SINGLE_H = 14
+
+
+class DsMlpSingle(ct.Structure):
+    _fields_ = [("struct_size", ct.c_size_t),
+                ("W1", ct.c_float * (DS_MLP_SINGLE_H * DS_MLP_IN)), ("b1", ct.c_float * DS_MLP_SINGLE_H),
+                ("W3", ct.c_float * DS_MLP_SINGLE_H), ("b3", ct.c_float),
+                ("mu", ct.c_float * DS_MLP_IN), ("inv_sigma", ct.c_float * DS_MLP_IN)]
+
+
 DS_LINE_IN, DS_LINE_H, DS_N_LINES = 16, 32, 4
 
 
@@ -59,7 +69,7 @@ class DsParams(ct.Structure):
                 ("zv_max", ct.c_double), ("m_pi", ct.c_double), ("m_p", ct.c_double), ("m_ks", ct.c_double),
                 ("m_lambda", ct.c_double), ("dm_ks", ct.c_double), ("dm_lambda", ct.c_double), ("n2_min", ct.c_double),
                 ("magnet_polarity", ct.c_double), ("gamma_c0", ct.c_double), ("gamma_c1", ct.c_double),
-                ("vtx_newton_iters", ct.c_int32), ("clone_min_shared", ct.c_int32), ("dv1", ct.c_int32), ("pad_", ct.c_int32)]
+                ("vtx_newton_iters", ct.c_int32), ("clone_min_shared", ct.c_int32), ("dv1", ct.c_int32), ("mlp_fast_math", ct.c_int32)]
 
 
 class DsHits(ct.Structure):
@@ -127,6 +137,7 @@ def lib() -> ct.CDLL:
         L.ds_error_string.argtypes = [ct.c_int]
         L.ds_error_string.restype = ct.c_char_p
         L.ds_upload_geometry.argtypes = [vp, ct.POINTER(DsGeometry), ct.POINTER(DsMlp)]
+        L.ds_upload_mlp_single.argtypes = [vp, ct.POINTER(DsMlpSingle)]
         L.ds_layout.argtypes = [vp, ct.POINTER(DsHits), vp, ct.c_int, ct.POINTER(DsParams), ct.POINTER(DsLayoutOut), vp]
         L.ds_extrapolate.argtypes = [vp, ct.POINTER(DsSeeds), ct.POINTER(DsParams), vp, vp]
         L.ds_workspace_bytes.argtypes = [vp, ct.c_int, ct.c_int64, ct.c_int64]
@@ -177,6 +188,20 @@ def make_mlp(w: dict) -> DsMlp:
         a = np.ascontiguousarray(w[k], dtype=np.float32).reshape(-1)
         if a.size != int(np.prod(shape)):
             raise ValueError(f"mlp weight {k}: expected shape {shape}")
+        getattr(o, k)[:] = a.tolist()
+    o.b3 = float(np.asarray(w["b3"]).reshape(-1)[0])
+    return o
+
+
+def make_mlp_single(w: dict) -> DsMlpSingle:
+    """w: W1 [14][8], b1 [14], W3 [14], b3 [1], mu [8], inv_sigma [8] (the paper's 8 -> 14 -> 1 network)."""
+    o = DsMlpSingle()
+    o.struct_size = ct.sizeof(DsMlpSingle)
+    for k, size in (("W1", DS_MLP_SINGLE_H * DS_MLP_IN), ("b1", DS_MLP_SINGLE_H), ("W3", DS_MLP_SINGLE_H), ("mu", DS_MLP_IN),
+                    ("inv_sigma", DS_MLP_IN)):
+        a = np.ascontiguousarray(w[k], dtype=np.float32).reshape(-1)
+        if a.size != size:
+            raise ValueError(f"single-hidden-layer mlp weight {k}: expected {size} values")
         getattr(o, k)[:] = a.tolist()
     o.b3 = float(np.asarray(w["b3"]).reshape(-1)[0])
     return o
@@ -244,6 +269,11 @@ def ds_destroy(h) -> None:
 def ds_upload_geometry(h, geometry: dict, mlp: dict) -> None:
     g, m = make_geometry(geometry), make_mlp(mlp)
     _check(lib().ds_upload_geometry(h, ct.byref(g), ct.byref(m)), "ds_upload_geometry")
+
+
+def ds_upload_mlp_single(h, mlp: dict) -> None:
+    m = make_mlp_single(mlp)
+    _check(lib().ds_upload_mlp_single(h, ct.byref(m)), "ds_upload_mlp_single")
 
 
 def _hits(hits) -> DsHits:
@@ -491,6 +521,10 @@ class Downstream:
             workspace = self._on_stream(self.workspace(ne, hits["id"].numel(), seeds["x"].numel()), stream)
         ds_reconstruct(self.h, hits, seeds, hit_offsets, seed_offsets, ne, self.params, out, workspace, stream)
         return out
+
+    def upload_mlp_single(self, mlp: dict) -> None:
+        """Switch the ghost killer to the paper's 8 -> 14 -> 1 network (until the geometry is uploaded again)."""
+        ds_upload_mlp_single(self.h, mlp)
 
     def upload_line_nets(self, line_w: dict) -> None:
         ds_upload_line_nets(self.h, line_w)

@@ -22,7 +22,7 @@ def test_exports_every_declared_symbol():
     L = pk.lib()
     names = declared_functions()
     assert {"ds_create", "ds_destroy", "ds_upload_geometry", "ds_layout", "ds_extrapolate", "ds_reconstruct",
-            "ds_ghost_killer", "ds_clone_kill", "ds_upload_line_nets", "ds_lines", "ds_vertex", "ds_process_host", "ds_workspace_bytes", "ds_vertex_workspace_bytes",
+            "ds_ghost_killer", "ds_clone_kill", "ds_upload_line_nets", "ds_upload_mlp_single", "ds_lines", "ds_vertex", "ds_process_host", "ds_workspace_bytes", "ds_vertex_workspace_bytes",
             "ds_profile_enable", "ds_profile_read", "ds_measure_dfma_peak", "ds_kernel_name", "ds_error_string", "ds_version"} <= set(names)
     for n in names:
         assert hasattr(L, n), n
@@ -32,15 +32,16 @@ def test_exports_every_declared_symbol():
 def test_header_is_plain_c_and_struct_sizes_match(tmp_path):
     import paper_2503_13092_b200.ds as B
     prog = tmp_path / "sz.c"
-    prog.write_text('#include <stdio.h>\n#include "ds.h"\nint main(void){printf("%zu %zu %zu %zu %zu %zu %zu %zu %zu\\n",'
+    prog.write_text('#include <stdio.h>\n#include "ds.h"\nint main(void){printf("%zu %zu %zu %zu %zu %zu %zu %zu %zu %zu %zu\\n",'
                     "sizeof(ds_geometry),sizeof(ds_mlp),sizeof(ds_params),sizeof(ds_hits),sizeof(ds_seeds),"
-                    "sizeof(ds_tracks),sizeof(ds_vertices),sizeof(ds_layout_out),sizeof(ds_profile));return 0;}\n")
+                    "sizeof(ds_tracks),sizeof(ds_vertices),sizeof(ds_layout_out),sizeof(ds_profile),sizeof(ds_mlp_single),"
+                    "sizeof(ds_line_nets));return 0;}\n")
     exe = tmp_path / "sz"
     subprocess.run(["gcc", "-std=c99", "-Wall", "-Wextra", "-Werror", "-pedantic", "-I", os.path.join(ROOT, "include"),
                     "-o", str(exe), str(prog)], check=True)
     sizes = [int(x) for x in subprocess.run([str(exe)], check=True, capture_output=True, text=True).stdout.split()]
     mine = [ct.sizeof(t) for t in (B.DsGeometry, B.DsMlp, B.DsParams, B.DsHits, B.DsSeeds, B.DsTracks, B.DsVertices,
-                                   B.DsLayoutOut, B.DsProfile)]
+                                   B.DsLayoutOut, B.DsProfile, B.DsMlpSingle, B.DsLineNets)]
     assert sizes == mine
 
 

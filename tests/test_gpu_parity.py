@@ -334,8 +334,11 @@ def test_ghost_killer_alone(ds, orc_mlp, torch):
 
 
 def test_paper_architecture_8_14_1(torch, mlp_w):
-    """the paper's ghost killer has one hidden layer of 14 units.  Embedded in the 8 -> 32 -> 16 -> 1
-    network of the library (gen.embed_single_hidden) it gives the scores of the oracle's single-hidden-layer evaluation."""
+    """the paper's ghost killer has one hidden layer of 14 units.  Its own kernel instantiation
+    (ds_upload_mlp_single -> k_mlp<14, 0>) and, as a cross-check, the exact embedding into the 8 -> 32 -> 16 -> 1 network
+    (gen.embed_single_hidden) both give the scores of the oracle's single-hidden-layer evaluation; the fast-math flavour
+    (__expf, __fdividef) stays within 2e-6 absolute of it, which is outside the bit-exact keep decision only for
+    scores on the threshold."""
     import paper_2503_13092_b200 as pk
     rng = np.random.default_rng(14)
     w1 = dict(W1=rng.normal(0, 8 ** -0.5, (14, 8)).astype(np.float32), b1=rng.normal(0, 8 ** -0.5, 14).astype(np.float32),
@@ -348,20 +351,56 @@ def test_paper_architecture_8_14_1(torch, mlp_w):
            for k, m, s in zip(("x", "y", "tx", "ty", "qop", "chi2"), C.MLP_MU[:6], C.MLP_SIGMA[:6])}
     seeds = dict(x=trk["x"], y=trk["y"], tx=trk["tx"], ty=trk["ty"], qop=rng.normal(0, 0.25, n).astype(np.float32),
                  chi2=(rng.chisquare(7, n) / 7).astype(np.float32))
-    d14 = pk.Downstream(G, gen.embed_single_hidden(w1), P)
-    try:
-        dev = d14.empty_tracks(n)
+    ref = np.array([orc.eval([trk["x"][i], trk["y"][i], trk["tx"][i], trk["ty"][i], trk["qop"][i], trk["chi2"][i],
+                              seeds["qop"][i], seeds["chi2"][i]]) for i in range(n)])
+    assert 0.05 < ref.std()
+
+    def scores(dsx):
+        dev = dsx.empty_tracks(n)
         for k, a in trk.items():
             dev[k].copy_(torch.as_tensor(a))
         dev["found"].fill_(1)
-        d14.ghost_killer(d14.to_device(seeds), dev)
+        dsx.ghost_killer(dsx.to_device(seeds), dev)
         torch.cuda.synchronize()
-        score = dev["score"].cpu().numpy()
+        return dev["score"].cpu().numpy(), dev["keep"].cpu().numpy()
+
+    med = float(np.median(ref))
+    pm = dict(P, mlp_thr=med)
+    d14 = pk.Downstream(G, gen.embed_single_hidden(w1), pm)
+    try:
+        s_emb, k_emb = scores(d14)                                    # embedded in the 8 -> 32 -> 16 -> 1 kernel
+        d14.upload_mlp_single(w1)
+        s_one, k_one = scores(d14)                                    # k_mlp<14, 0, false>
+        d14.set_params(dict(pm, mlp_fast_math=1))
+        s_fast, k_fast = scores(d14)                                  # k_mlp<14, 0, true>
+        pk.ds_upload_geometry(d14.h, G, mlp_w)                        # back to the 8 -> 32 -> 16 -> 1 network of cfg0
+        d14.set_params(P)
+        s_back, _ = scores(d14)
     finally:
         d14.close()
-    ref = np.array([orc.eval([trk["x"][i], trk["y"][i], trk["tx"][i], trk["ty"][i], trk["qop"][i], trk["chi2"][i],
-                              seeds["qop"][i], seeds["chi2"][i]]) for i in range(n)])
-    assert parity.close(score, ref, 1e-3).all() and 0.05 < ref.std()
+    for sc, kp in ((s_emb, k_emb), (s_one, k_one)):
+        assert parity.close(sc, ref, 1e-3).all()
+        margin = np.abs(ref - med) / med
+        assert (kp == (ref > med))[margin >= 1e-5].all() and 0.4 < kp.mean() < 0.6
+    assert np.abs(s_fast - ref).max() < 2e-6 and (k_fast != (ref > med)).sum() <= 2
+    full = O.Mlp(mlp_w)
+    ref_full = np.array([full.eval([trk["x"][i], trk["y"][i], trk["tx"][i], trk["ty"][i], trk["qop"][i], trk["chi2"][i],
+                                    seeds["qop"][i], seeds["chi2"][i]]) for i in range(0, n, 40)])
+    assert parity.close(s_back[::40], ref_full, 1e-3).all()
+
+
+def test_fast_math_ghost_killer_on_tracks(ds, orc_mlp):
+    """mlp_fast_math = 1 on the 8 -> 32 -> 16 -> 1 network through ds_reconstruct: same tracks, scores within 2e-6 absolute of
+    the IEEE path, keep decisions equal except scores within 1e-5 of the threshold."""
+    d = gen.generate(1, n_events=200)
+    t0, _ = gpu_run(ds, d)
+    t1, _ = gpu_run(ds, d, params=dict(P, mlp_fast_math=1))
+    for k in ("x", "tx", "qop", "chi2", "found", "nhits", "hit"):
+        assert np.array_equal(t0[k], t1[k]), k
+    f = t0["found"] == 1
+    assert f.sum() > 3000 and np.abs(t0["score"][f] - t1["score"][f]).max() < 2e-6
+    diff = t0["keep"] != t1["keep"]
+    assert (np.abs(t0["score"][diff] - P["mlp_thr"]) < 1e-5 * P["mlp_thr"]).all()
 
 
 # ---- S8..S10 on hand-made tracks -----------------------------------------------------------------------------------------
