@@ -126,6 +126,8 @@ def algorithmic_bytes(n_events, n_hits, n_seeds, n_found, n_keep, n_vtx):
         "k_vertex_count": 28 * n_keep + 8 * n_seeds + 4 * n_events,
         "k_vertex_scan": 16 * n_events,
         "k_vertex_write": 28 * n_keep + 40 * n_vtx,
+        # S1..S6 in one launch: the S1 and S2..S6 figures of SURVEY 8d together (what the unfused algorithm moves)
+        "k_event": 52 * n_hits + 57 * 4 * n_events + 20 * n_hits + 28 * n_seeds + 52 * n_seeds + 16 * n_found,
         "k_clone": 28 * n_seeds,                                           # hit[4], chi2, nhits, found of every slot
         "k_lines": (24 + 32 + 20) * n_vtx,                                 # vertex record, 2 x 4 track values, 4 scores + bits
     }

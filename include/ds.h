@@ -288,7 +288,7 @@ int ds_process_host(ds_handle *h, const ds_hits *hits, const ds_seeds *seeds, co
 /* ---- per-kernel device timing (measurement aid; no effect on results) ------------------------------------------ */
 
 /* Kernels of the path, in launch order. */
-enum { DS_K_LAYOUT = 0, DS_K_TRACK, DS_K_MLP, DS_K_VTX_COUNT, DS_K_VTX_SCAN, DS_K_VTX_WRITE, DS_K_CLONE, DS_K_LINES, DS_K_COUNT };
+enum { DS_K_LAYOUT = 0, DS_K_TRACK, DS_K_MLP, DS_K_VTX_COUNT, DS_K_VTX_SCAN, DS_K_VTX_WRITE, DS_K_CLONE, DS_K_LINES, DS_K_EVENT, DS_K_COUNT };
 
 typedef struct {
     size_t struct_size;

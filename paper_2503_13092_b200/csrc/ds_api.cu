@@ -1,5 +1,6 @@
 // C ABI of libds (include/ds.h): handle, argument checks, workspace carving, launch order, host-buffer path.
 // No arithmetic of the method lives here.
+#include <cstdlib>
 #include <new>
 
 #include "ds_common.cuh"
@@ -37,6 +38,17 @@ struct DeviceGuard {
         if (prev >= 0) cudaSetDevice(prev);
     }
 };
+
+// Development aid: DS_FUSED=0 takes k_layout + k_track for every event (the path of Dv1 and of oversize events)
+bool fused_off()
+{
+    static int v = -1;
+    if (v < 0) {
+        const char *e = getenv("DS_FUSED");
+        v = (e && e[0] == '0') ? 1 : 0;
+    }
+    return v == 1;
+}
 
 inline size_t up256(size_t v) { return (v + 255) & ~(size_t)255; }
 
@@ -120,6 +132,7 @@ size_t carve_layout(void *ws, int n_bins, int n_events, int64_t n_hits, LayoutPt
     L.bin_offsets = reinterpret_cast<int32_t *>(take(4 * ne * (n_bins + 1)));
     L.ybounds = reinterpret_cast<float2 *>(take(sizeof(float2) * ne * (n_bins / kXBins)));
     L.uniform = reinterpret_cast<int32_t *>(take(4 * ne));
+    L.redo = reinterpret_cast<int32_t *>(take(4 * ne));
     L.sz = L.sw = nullptr;
     L.sid = L.perm = nullptr;
     return off;
@@ -134,6 +147,23 @@ size_t layout_bytes(int n_bins, int n_events, int64_t n_hits)
 void set_inputs(LayoutPtrs &L, const ds_hits *hits)
 {
     L.x0 = hits->x0; L.z = hits->z; L.ymin = hits->ymin; L.ymax = hits->ymax; L.w = hits->w; L.id = hits->id;
+}
+
+// S1..S6.  Dv0: k_event does S1..S6 for every event that fits its staging capacity and marks the others in L.redo; k_layout
+// + k_track then run for the marked events only (their blocks for the other events leave at once).  Dv1: k_layout + k_track.
+cudaError_t reconstruct_launches(ds_handle *h, const DevConst &c, const LayoutPtrs &L, const ds_hits &hits, const ds_seeds &seeds,
+                                 const int32_t *hit_offsets, const int32_t *seed_offsets, int n_events, int hint, const ds_tracks &out,
+                                 cudaStream_t st)
+{
+    const int32_t *only = nullptr;
+    cudaError_t err = cudaSuccess;
+    if (!c.dv1 && !fused_off()) {
+        err = launch_event(c, hits, seeds, hit_offsets, seed_offsets, n_events, hint, out, L.redo, st, h->prof);
+        only = L.redo;
+    }
+    if (err == cudaSuccess) err = launch_layout(c, L, hit_offsets, n_events, hint, only, st, h->prof);
+    if (err == cudaSuccess) err = launch_track(c, L, seeds, hit_offsets, seed_offsets, n_events, hint, only, out, st, h->prof);
+    return err;
 }
 
 }  // namespace
@@ -263,8 +293,8 @@ int ds_layout(ds_handle *h, const ds_hits *hits, const int32_t *hit_offsets, int
     set_inputs(L, hits);
     L.sx0 = out->x0; L.sz = out->z; L.symin = out->ymin; L.symax = out->ymax; L.sw = out->w; L.sid = out->id;
     L.perm = out->perm; L.bin_offsets = out->bin_offsets;
-    L.aux = nullptr; L.ybounds = nullptr; L.uniform = nullptr;   // the public SoA form
-    if (launch_layout(c, L, hit_offsets, n_events, p->max_event_hits_hint, (cudaStream_t)cuda_stream, h->prof) != cudaSuccess) {
+    L.aux = nullptr; L.ybounds = nullptr; L.uniform = nullptr; L.redo = nullptr;   // the public SoA form
+    if (launch_layout(c, L, hit_offsets, n_events, p->max_event_hits_hint, nullptr, (cudaStream_t)cuda_stream, h->prof) != cudaSuccess) {
         cudaGetLastError();
         return DS_E_CUDA;
     }
@@ -342,8 +372,7 @@ int ds_reconstruct(ds_handle *h, const ds_hits *hits, const ds_seeds *seeds, con
     LayoutPtrs L;
     set_inputs(L, hits);
     carve_layout(workspace, c.n_bins, n_events, hits->n, L);
-    cudaError_t err = launch_layout(c, L, hit_offsets, n_events, p->max_event_hits_hint, st, h->prof);
-    if (err == cudaSuccess) err = launch_track(c, L, *seeds, hit_offsets, seed_offsets, n_events, p->max_event_hits_hint, *out, st, h->prof);
+    cudaError_t err = reconstruct_launches(h, c, L, *hits, *seeds, hit_offsets, seed_offsets, n_events, p->max_event_hits_hint, *out, st);
     if (err == cudaSuccess) err = launch_clone(c, seed_offsets, n_events, *out, st, h->prof);
     if (err == cudaSuccess) err = launch_mlp(c, h->d_mlp, h->use_single ? h->d_single : nullptr, *seeds, *out, st, h->prof);
     if (err != cudaSuccess) {
@@ -494,8 +523,7 @@ int ds_process_host(ds_handle *h, const ds_hits *hits, const ds_seeds *seeds, co
     LayoutPtrs L;
     set_inputs(L, &dh);
     carve_layout(wrec, c.n_bins, n_events, hits->n, L);
-    err = launch_layout(c, L, d_hoff, n_events, p->max_event_hits_hint, st, h->prof);
-    if (err == cudaSuccess) err = launch_track(c, L, dsd, d_hoff, d_soff, n_events, p->max_event_hits_hint, dt, st, h->prof);
+    err = reconstruct_launches(h, c, L, dh, dsd, d_hoff, d_soff, n_events, p->max_event_hits_hint, dt, st);
     if (err == cudaSuccess) err = launch_clone(c, d_soff, n_events, dt, st, h->prof);
     if (err == cudaSuccess) err = launch_mlp(c, h->d_mlp, h->use_single ? h->d_single : nullptr, dsd, dt, st, h->prof);
     if (err == cudaSuccess) err = launch_vertex(c, dt, d_soff, n_events, dv, wvtx, st, h->prof);
@@ -595,7 +623,7 @@ int ds_measure_dfma_peak(ds_handle *h, double *tflops)
 const char *ds_kernel_name(int k)
 {
     static const char *names[DS_K_COUNT] = {"k_layout", "k_track", "k_mlp", "k_vertex_count", "k_vertex_scan", "k_vertex_write",
-                                               "k_clone", "k_lines"};
+                                               "k_clone", "k_lines", "k_event"};
     return (k >= 0 && k < DS_K_COUNT) ? names[k] : nullptr;
 }
 

@@ -16,6 +16,7 @@ constexpr int kMaxFirst = DS_MAX_FIRST_HITS;
 constexpr int kIdLayerShift = 24;
 constexpr int kIdSectorShift = 20;
 constexpr int kIdSeqMask = (1 << 20) - 1;
+constexpr int kRedoGrid = 2 * 148;   // blocks of k_layout / k_track when they only take the events k_event has left over
 
 // Geometry + parameters as the kernels see them (passed by value as a __grid_constant__ kernel argument).
 struct DevConst {
@@ -71,6 +72,17 @@ __device__ __forceinline__ int xbin(float x0, float off, float scale)
 {
     float t = floorf((x0 + off) * scale);
     t = fminf(fmaxf(t, 0.0f), (float)(kXBins - 1));
+    return (int)t;
+}
+
+// The same for a table with kSlices = kXBins * k slices per (layer, sector) (k a power of two): slice of x0 =
+// clamp(floor(k * t)) with t = (x0 + off) * scale the fp32 value xbin() floors; k * t is exact, so slice / k = xbin.
+template <int kSlices>
+__device__ __forceinline__ int xslice(float x0, float off, float scale)
+{
+    static_assert(kSlices % kXBins == 0, "slices refine the DS_XBINS slices of the public table");
+    float t = floorf((x0 + off) * scale * (float)(kSlices / kXBins));
+    t = fminf(fmaxf(t, 0.0f), (float)(kSlices - 1));
     return (int)t;
 }
 
@@ -201,16 +213,23 @@ struct LayoutPtrs {
     float4 *aux;
     float2 *ybounds;
     int32_t *uniform;
+    int32_t *redo;   // [E] written by k_event: 1 = the event is left to k_layout + k_track
 };
 
+// only != nullptr (here and in launch_track): only the events e with only[e] != 0 are processed
 cudaError_t launch_layout(const DevConst &c, const LayoutPtrs &p, const int32_t *hit_offsets, int n_events,
-                          int max_event_hits_hint, cudaStream_t st, Prof &prof);
+                          int max_event_hits_hint, const int32_t *only, cudaStream_t st, Prof &prof);
+
+// S1..S6 in one kernel (ds_event.cu), Dv0 only; redo[e] = 1 for the events it leaves to k_layout + k_track
+cudaError_t launch_event(const DevConst &c, const ds_hits &hits, const ds_seeds &seeds, const int32_t *hit_offsets,
+                         const int32_t *seed_offsets, int n_events, int max_event_hits_hint, const ds_tracks &out, int32_t *redo,
+                         cudaStream_t st, Prof &prof);
 
 cudaError_t launch_extrapolate(const DevConst &c, const ds_seeds &seeds, double *out, cudaStream_t st);
 
 cudaError_t launch_track(const DevConst &c, const LayoutPtrs &lay, const ds_seeds &seeds, const int32_t *hit_offsets,
-                         const int32_t *seed_offsets, int n_events, int max_event_hits_hint, const ds_tracks &out,
-                         cudaStream_t st, Prof &prof);
+                         const int32_t *seed_offsets, int n_events, int max_event_hits_hint, const int32_t *only,
+                         const ds_tracks &out, cudaStream_t st, Prof &prof);
 
 cudaError_t launch_clone(const DevConst &c, const int32_t *seed_offsets, int n_events, const ds_tracks &trk, cudaStream_t st,
                          Prof &prof);

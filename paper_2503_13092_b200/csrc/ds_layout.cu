@@ -25,91 +25,15 @@
 //               sector's), so y-compatibility becomes one test per (seed, sector) instead of one per hit and k_track stages
 //               4 instead of 12 bytes per hit.  symin / symax (sorted per-hit bounds) are written only for events that are
 //               not uniform; k_track then tests every hit with its own bounds.
-#include "ds_common.cuh"
+#include "ds_sort.cuh"
 
 namespace ds {
 
 constexpr int kLayoutThreads = 512;
-constexpr int kSub = 4;   // the sort cuts every x0 slice of the bin table into kSub sub-slices (a power of two)
-
-// Sort bin of a hit: (layer, sector, x0 sub-slice).  t = (x0 + off) * scale is the same fp32 value xbin() floors, and
-// 4t is exact, so floor(floor(kSub * t) / kSub) = floor(t): sub-slice s lies in table slice s / kSub, clamps included.
-__device__ __forceinline__ int fine_bin(const DevConst &c, int id, float x0)
-{
-    int sec = min(id_sector(id), c.n_sectors - 1);
-    float t = floorf((x0 + c.xb_off) * c.xb_scale * (float)kSub);
-    t = fminf(fmaxf(t, 0.0f), (float)(kXBins * kSub - 1));
-    return (id_layer(id) * c.n_sectors + sec) * (kXBins * kSub) + (int)t;
-}
-
-// exclusive scan of v[0..n) in place (n <= a few thousand), v[n] = total.  All threads of the block call it.
-__device__ void block_exclusive_scan(int *v, int n, int *warp_sums)
-{
-    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5, nw = blockDim.x >> 5;
-    const int per = (n + blockDim.x - 1) / blockDim.x;
-    const int b = tid * per, e = min(b + per, n);
-    int s = 0;
-    for (int k = b; k < e; ++k) s += v[k];
-    int inc = s;
-#pragma unroll
-    for (int d = 1; d < 32; d <<= 1) {
-        int t = __shfl_up_sync(0xffffffffu, inc, d);
-        if (lane >= d) inc += t;
-    }
-    if (lane == 31) warp_sums[wid] = inc;
-    __syncthreads();
-    if (wid == 0) {
-        int ws = lane < nw ? warp_sums[lane] : 0, wi = ws;
-#pragma unroll
-        for (int d = 1; d < 32; d <<= 1) {
-            int t = __shfl_up_sync(0xffffffffu, wi, d);
-            if (lane >= d) wi += t;
-        }
-        if (lane < nw) warp_sums[lane] = wi - ws;
-        if (lane == 31) warp_sums[32] = wi;
-    }
-    __syncthreads();
-    int run = warp_sums[wid] + inc - s;
-    for (int k = b; k < e; ++k) {
-        int t = v[k];
-        v[k] = run;
-        run += t;
-    }
-    if (tid == 0) v[n] = warp_sums[32];
-    __syncthreads();
-}
-
-// Stage global src[h0 .. h0+n) into a shared buffer so that element i sits at buf[(h0 & 3) + i]: the part of the slice
-// between 16-byte boundaries by one bulk async copy that completes on `bar` (issued by thread 0, which also arms the
-// barrier), the up to three elements after the last boundary by ordinary loads (threads 32..34).  With `bulk` false
-// (a source pointer that is not 16-byte aligned) everything is loaded by ordinary loads and the barrier only armed.
-// Every thread of the block calls it; the buffer must be free (a __syncthreads after its last reader), and a
-// __syncthreads plus mbar_wait(bar) must precede the first read.
-template <typename T>
-__device__ __forceinline__ void stage_field(T *buf, const T *__restrict__ src, int h0, int n, unsigned long long *bar,
-                                            bool bulk)
-{
-    const int d = h0 & 3, h0a = h0 - d, h1 = h0 + n;
-    const int h1dn = bulk ? max(h1 & ~3, h0a) : h0a;          // bulk part: [h0a, h1dn); it may start before h0
-    if (threadIdx.x == 0) {
-        const uint32_t bytes = 4u * (uint32_t)(h1dn - h0a);
-        // the buffer may have been written and read by ordinary (generic-proxy) accesses of the whole block before the
-        // __syncthreads that precedes this call: order them before the async-proxy write of the bulk copy
-        fence_proxy_async();
-        mbar_expect_tx(bar, bytes);
-        if (bytes) bulk_g2s(buf, src + h0a, bytes, bar);
-    }
-    if (bulk) {
-        const int t = (int)threadIdx.x - 32;
-        if (t >= 0 && h1dn + t < h1 && h1dn + t >= h0) buf[h1dn + t - h0a] = src[h1dn + t];
-    } else {
-        for (int i = threadIdx.x; i < n; i += blockDim.x) buf[d + i] = src[h0 + i];
-    }
-}
-
 template <bool kInternal>
 __global__ void __launch_bounds__(2 * kLayoutThreads)
-k_layout(const __grid_constant__ DevConst c, const LayoutPtrs p, const int32_t *__restrict__ hit_offsets, int cap, bool bulk)
+k_layout(const __grid_constant__ DevConst c, const LayoutPtrs p, const int32_t *__restrict__ hit_offsets, int n_events, int cap,
+         bool bulk, const int32_t *__restrict__ only)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ int warp_sums[33];
@@ -126,14 +50,19 @@ k_layout(const __grid_constant__ DevConst c, const LayoutPtrs p, const int32_t *
     int *hist = reinterpret_cast<int *>(s_src + cap);                  // [nfine + 1]
     unsigned long long *bar_x = &bars[0], *bar_i = &bars[1], *bar_b = &bars[2];
 
-    const int e = blockIdx.x;
+    // one event per block; with `only` (the events k_event has left over) a small grid walks the event list and a block may
+    // meet several marked events: the launcher then passes cap = 0, so that none of them takes the staged path (whose
+    // mbarriers are armed once per block)
+    for (int e = blockIdx.x; e < n_events; e += gridDim.x) {
+    if (only && only[e] == 0) continue;
+    __syncthreads();   // the previous event of this block is finished
     const int h0 = hit_offsets[e];
     const int n = hit_offsets[e + 1] - h0;
     const int tid = threadIdx.x;
     const int d = h0 & 3;
     const bool fast = n + 3 <= cap;
 
-    if (tid == 0) {
+    if (tid == 0 && fast) {
         mbar_init(bar_x, 1);
         mbar_init(bar_i, 1);
         mbar_init(bar_b, 1);
@@ -319,13 +248,14 @@ k_layout(const __grid_constant__ DevConst c, const LayoutPtrs p, const int32_t *
             if (tid == 0) p.uniform[e] = 0;
         }
     }
+    }   // events of this block
 }
 
 
 static size_t layout_smem_bytes(int cap, int n_bins) { return (size_t)cap * 18 + sizeof(int) * ((size_t)n_bins * kSub + 1) + 16; }
 
 cudaError_t launch_layout(const DevConst &c, const LayoutPtrs &p, const int32_t *hit_offsets, int n_events,
-                          int max_event_hits_hint, cudaStream_t st, Prof &prof)
+                          int max_event_hits_hint, const int32_t *only, cudaStream_t st, Prof &prof)
 {
     if (n_events <= 0) return cudaSuccess;
     // staging capacity in hits: a multiple of 4 with room for the alignment slack, 18 bytes each; hit indices inside an
@@ -348,8 +278,10 @@ cudaError_t launch_layout(const DevConst &c, const LayoutPtrs &p, const int32_t 
     prof.begin(DS_K_LAYOUT, st);
     // events so large that one block fills an SM's shared memory get twice the threads (every loop strides by blockDim.x)
     const int threads = smem + 1024 > (228 * 1024) / 2 ? 2 * kLayoutThreads : kLayoutThreads;
-    if (internal) k_layout<true><<<n_events, threads, smem, st>>>(c, p, hit_offsets, cap, bulk);
-    else k_layout<false><<<n_events, threads, smem, st>>>(c, p, hit_offsets, cap, bulk);
+    const int grid = only ? (n_events < kRedoGrid ? n_events : kRedoGrid) : n_events;
+    if (only) cap = 0;
+    if (internal) k_layout<true><<<grid, threads, smem, st>>>(c, p, hit_offsets, n_events, cap, bulk, only);
+    else k_layout<false><<<grid, threads, smem, st>>>(c, p, hit_offsets, n_events, cap, bulk, only);
     prof.end(st);
     return cudaGetLastError();
 }

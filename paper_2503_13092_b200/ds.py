@@ -95,7 +95,7 @@ class DsVertices(ct.Structure):
                 ("offsets", ct.c_void_p), ("overflow", ct.c_void_p), ("capacity", ct.c_int64)]
 
 
-DS_K_COUNT = 8
+DS_K_COUNT = 9
 
 
 class DsProfile(ct.Structure):
