@@ -89,6 +89,7 @@ bool make_const(const ds_geometry &g, const ds_params *p, DevConst &c)
     c.vtx_mp = p->magnet_polarity; c.gamma_c0 = p->gamma_c0; c.gamma_c1 = p->gamma_c1;
     c.vtx_iters = p->vtx_newton_iters; c.clone_min_shared = p->clone_min_shared;
     c.dv1 = p->dv1 != 0; c.mlp_fast_math = p->mlp_fast_math != 0;
+    c.y_rsec = (int)(p->y_tol / g.sector_height + 1e-9) + 1; c.pad2_ = 0;
     return true;
 }
 

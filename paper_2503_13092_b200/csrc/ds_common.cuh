@@ -36,6 +36,7 @@ struct DevConst {
     double vtx_mp, gamma_c0, gamma_c1;   // curved-track vertexing: gamma = -vtx_mp * (gamma_c0 + gamma_c1 * qop / 1000)
     int vtx_iters, clone_min_shared;
     int dv1, mlp_fast_math;
+    int y_rsec, pad2_;   // sectors on either side of the one a y falls into that can be y-compatible: floor(y_tol / height) + 1
 };
 
 // Device copy of the ghost-killer weights (global memory, staged to shared memory by the kernel).

@@ -20,14 +20,35 @@
 //          order (distance, id, index in the caller's arrays), so the result does not depend on that order
 //   z      bulk copy of z into the buffer the unsorted x0 leaves free (read through src[]), in flight during the first searches
 //   track  S2..S6 by the block's warps, each on its share of the event's seeds (event_chunk)
+#include <cstdlib>
+
 #include "ds_sort.cuh"
 #include "ds_track.cuh"
 
 namespace ds {
 
 constexpr int kFine = kXBins * kSub;   // x0 slices per (layer, sector) of the sort = of the table the searches use here
-static_assert(kFine == 64, "coarse bin = fine bin >> 6");
-constexpr int kSelCap = 128;           // hits of an over-full first window that the warp ranks together
+constexpr int kFineLog2 = kFine == 64 ? 6 : (kFine == 32 ? 5 : (kFine == 128 ? 7 : -1));
+static_assert((1 << kFineLog2) == kFine, "coarse bin = fine bin >> kFineLog2");
+constexpr int kSelCap = 64;            // hits of an over-full first window that the warp ranks together
+
+// State of one warp of k_event (cf. WarpShared of ds_track.cuh; no fit results are kept: the lane that fits the best
+// combination of a seed writes the track record itself)
+struct EventWarp {
+    SeedRec rec[32];
+    unsigned long long best_bits[32];     // per seed: smallest score among its fits (bits of the non-negative double)
+    uint16_t near[3 * kFirstCap][2];      // phase B: closest / second closest hit of (first hit, layer); phase A: ranking lists
+    float z3[kFirstCap];                  // z of the first hit
+    int n_best[32];                       // per seed: fits with that score (+ 2 for every first hit left to the seed's thread)
+    int n_fit;                            // fit tasks appended this round (may exceed kFitCap)
+    int fit_end;                          // tasks [0, fit_end) are queued; later appends did not fit the queue
+    uint16_t slot[32 * kMaxFirst];        // phase A: the seed's first hits (positions in the event's bin-ordered x0)
+    unsigned short foff[32];              // where the seed's first hits start in the round's list
+    unsigned short fs[kFirstCap];         // first-hit list: index into slot[]
+    unsigned short ffit[kFirstCap];       // first fit task of the first hit (| combinations << 12), kFitNone or kFitInline
+    unsigned short task[kFitCap];         // fit task: first hit | i1 << 9 | i2 << 10
+};
+static_assert(sizeof(EventWarp) % 8 == 0 && sizeof(EventWarp::near) >= kSelCap * (sizeof(double) + sizeof(uint16_t)), "ranking lists fit near[]");
 
 struct EventHead {
     unsigned long long bars[5];
@@ -35,6 +56,7 @@ struct EventHead {
     int nonuni;
     int pad_;
     float2 yb[kLayers * DS_MAX_SECTORS];   // (ymin, ymax) of each (layer, sector)
+    double2 ye[kLayers * DS_MAX_SECTORS];  // uniform events: (ymin - y_tol, ymax + y_tol), what a track's y is compared with
 };
 
 // Byte offsets of the regions of the dynamic shared memory; cap is a multiple of 8.
@@ -43,24 +65,29 @@ struct EventHead {
 //   Y   ymax, then src (uint16, first half)    P  id, then bin << 20 | slot
 //   WS  the warps' lists (S2..S6): from the second half of Y over P, both dead by then
 struct EventLayout {
-    size_t HI, S, Z, Y, P, WS, total;
+    uint32_t HI, S, Z, Y, P, WS, total;
 };
 
 template <int W>
-__host__ __device__ inline EventLayout event_layout(int cap, int nfine)
+static EventLayout event_layout(int cap, int nfine)
 {
-    auto up16 = [](size_t v) { return (v + 15) & ~(size_t)15; };
+    auto up16 = [](size_t v) { return (uint32_t)((v + 15) & ~(size_t)15); };
     EventLayout L;
-    const size_t c4 = 4 * (size_t)cap;
+    const uint32_t c4 = 4 * (uint32_t)cap;
     L.HI = up16(sizeof(EventHead));
     L.S = L.HI + up16(4 * ((size_t)nfine / 2 + 1));
     L.Z = L.S + c4;
     L.Y = L.Z + c4;
     L.P = L.Y + c4;
     L.WS = L.Y + c4 / 2;
-    const size_t sort_end = L.P + c4, ws_end = L.WS + W * sizeof(WarpShared<uint16_t, false>);
+    const uint32_t sort_end = L.P + c4, ws_end = L.WS + W * (uint32_t)sizeof(EventWarp);
     L.total = sort_end > ws_end ? sort_end : ws_end;
     return L;
+}
+
+__device__ __forceinline__ void stage_words(void *buf, const void *src, int h0, int n, unsigned long long *bar, bool bulk)
+{
+    stage_field(static_cast<uint32_t *>(buf), static_cast<const uint32_t *>(src), h0, n, bar, bulk);
 }
 
 __device__ __forceinline__ void l2_prefetch(const void *p, uint32_t bytes)
@@ -74,29 +101,43 @@ struct EventCtx {
     HitsFused H;
     const uint16_t *tab;   // bin starts, kFine slices per (layer, sector)
     const float2 *yb;      // (ymin, ymax) of each (layer, sector)
+    const double2 *ye;     // (ymin - y_tol, ymax + y_tol) of each (layer, sector)
     bool uni;              // every hit carries the bounds of its (layer, sector)
     int rsec;              // sectors looked at on either side of the one a track's y falls into
 };
+
+// Events whose hits do not all carry their sector's bounds (rare: out of line): the sectors a track at height y can touch;
+// every hit is then tested with its own bounds
+__device__ __forceinline__ unsigned ev_sector_mask_any(const DevConst &c, int layer, double y)
+{
+    return sector_mask<false>(c, nullptr, layer, y);
+}
+
+__device__ __forceinline__ bool ev_y_hit(const DevConst &c, const float *gymin, const float *gymax, int i, double y)
+{
+    const double lo = (double)gymin[i] - c.y_tol, hi = (double)gymax[i] + c.y_tol;
+    return (lo <= y) & (y <= hi);
+}
 
 // Bit s set: sector s of `layer` is y-compatible with a track at height y (see sector_mask of ds_track.cuh).  Uniform
 // event: the test of O-S3 itself (ymin - y_tol <= y <= ymax + y_tol) on the sectors around the one y falls into.
 __device__ __forceinline__ unsigned ev_sector_mask(const DevConst &c, const EventCtx &E, int layer, double y)
 {
-    if (!E.uni) return sector_mask<false>(c, E.yb, layer, y);
+    if (!E.uni) return ev_sector_mask_any(c, layer, y);
     const int sc = __double2int_rd((y - c.y0) * c.inv_h);   // NaN -> 0: the tests below then fail
     const int lo = max(sc - E.rsec, 0), hi = min(sc + E.rsec, c.n_sectors - 1);
     unsigned m = 0;
+#pragma unroll 1
     for (int s = lo; s <= hi; ++s) {
-        const float2 b = E.yb[layer * c.n_sectors + s];
-        const double ylo = (double)b.x - c.y_tol, yhi = (double)b.y + c.y_tol;
-        m |= ((ylo <= y) & (y <= yhi)) ? 1u << s : 0u;
+        const double2 b = E.ye[layer * c.n_sectors + s];
+        m |= ((b.x <= y) & (y <= b.y)) ? 1u << s : 0u;
     }
     return m;
 }
 
 __device__ __forceinline__ bool ev_y_ok(const DevConst &c, const EventCtx &E, int j, double y)
 {
-    return E.uni || y_compatible<false>(c, E.H, j, y);
+    return E.uni || ev_y_hit(c, E.H.gymin, E.H.gymax, (int)E.H.src[j], y);
 }
 
 // Positions [a, b) of the slices of (layer, sector) that the (widened, fp32) window of pf touches
@@ -118,6 +159,7 @@ __device__ __forceinline__ int2 ev_search(const DevConst &c, const EventCtx &E, 
     for (unsigned m = mask; m; m &= m - 1) {
         int a, b;
         ev_slices(c, E, l, __ffs(m) - 1, fl, fh, a, b);
+#pragma unroll 1
         for (int j = a; j < b; ++j) {
             const float xj = E.H.x0[j];
             if (!(fabsf(xj - pf.t) <= pf.w)) continue;
@@ -162,11 +204,114 @@ __device__ __noinline__ void ev_select_serial(const DevConst &c, const EventCtx 
     }
 }
 
+// S6 output: the track of seed s from its best candidate (state at z_ref; y and ty are the seed's, A-8)
+__device__ __forceinline__ void ev_write_track(const DevConst &c, const HitsFused &H, const ds_seeds &seeds, const ds_tracks &out, int s,
+                                               const Candidate &best)
+{
+    const double ys = (double)seeds.y[s], txs = (double)seeds.tx[s], tys = (double)seeds.ty[s];
+    out.x[s] = (float)best.a;
+    out.y[s] = (float)(ys + tys * (c.z_ref - c.z_seed));
+    out.tx[s] = (float)best.b;
+    out.ty[s] = (float)tys;
+    out.qop[s] = (float)((txs - best.b) / c.kick);
+    out.chi2[s] = (float)best.chi2;
+    out.nhits[s] = best.nh;
+    out.found[s] = 1;
+    int4 hv;
+    hv.x = best.j0 >= 0 ? hit_perm(H, best.j0) : -1;
+    hv.y = best.j1 >= 0 ? hit_perm(H, best.j1) : -1;
+    hv.z = best.j2 >= 0 ? hit_perm(H, best.j2) : -1;
+    hv.w = hit_perm(H, best.j3);
+    reinterpret_cast<int4 *>(out.hit)[s] = hv;
+}
+
+// S6 in full for one seed (first hits f0 .. f0+nF-1 of the warp's list, seed in lane o): every combination fitted in turn,
+// equal scores resolved by (more hits, ids, indices) (A-9)
+__device__ __forceinline__ Candidate ev_choose_general(const DevConst &c, const EventWarp &sh, const HitsFused &H, int f0, int nF, int o)
+{
+    Candidate best;
+    best.score = kNoScore; best.a = 0.0; best.b = 0.0; best.chi2 = 0.0;
+    best.nh = 0; best.j0 = -1; best.j1 = -1; best.j2 = -1; best.j3 = -1;
+    const SeedRec &s2 = sh.rec[o];
+    for (int k = 0; k < nF; ++k) {
+        const int f = f0 + k;
+        if (sh.ffit[f] == kFitNone) continue;
+        const int j0 = idx_get(sh.near[3 * f][0]), j3 = (int)sh.slot[sh.fs[f]];
+        const int j1a = idx_get(sh.near[3 * f + 1][0]), j1b = idx_get(sh.near[3 * f + 1][1]);
+        const int j2a = idx_get(sh.near[3 * f + 2][0]), j2b = idx_get(sh.near[3 * f + 2][1]);
+        const int m1 = j1b >= 0 ? 2 : 1, m2 = j2b >= 0 ? 2 : 1;
+        const int nh = 1 + (j0 >= 0) + (j1a >= 0) + (j2a >= 0);
+        for (int i = 0; i < m1 * m2; ++i) {
+            const int j1 = i / m2 ? j1b : j1a, j2 = i % m2 ? j2b : j2a;
+            const FitRes r = fit_combo(c, H, s2, j0, j1, j2, j3, (double)sh.z3[f], (double)H.gw[H.src[j3]]);
+            if (r.score == kNoScore) continue;
+            Candidate cand;
+            cand.score = r.score; cand.a = r.a; cand.b = r.b; cand.chi2 = r.chi2;
+            cand.nh = nh; cand.j0 = j0; cand.j1 = j1; cand.j2 = j2; cand.j3 = j3;
+            if (cand.score < best.score || (cand.score == best.score && tie_better(H, cand, best))) best = cand;
+        }
+    }
+    return best;
+}
+
+// A first window with more than max_first hits (seed of lane o), by the whole warp: lanes over the hits of the window, every
+// passing hit is ranked among all of them by (distance, id, index); the max_first closest go to the seed's slots in that order
+__device__ __forceinline__ void ev_select_warp(const DevConst &c, const EventCtx &E, EventWarp &sh, int o, unsigned mask3, float pt, float pw,
+                                            double off3, double xc3, double w0, double y3, int max_first)
+{
+    const unsigned FULL = 0xffffffffu;
+    const int lane = threadIdx.x & 31;
+    const HitsFused &H = E.H;
+    const int fl = xslice<kFine>(pt - pw, c.xb_off, c.xb_scale), fh = xslice<kFine>(pt + pw, c.xb_off, c.xb_scale);
+    double *cd = reinterpret_cast<double *>(&sh.near[0][0]);          // near[] is free in phase A: the distances,
+    uint16_t *cj = reinterpret_cast<uint16_t *>(cd + kSelCap);        //                            the hits
+    int n_list = 0;
+    for (unsigned m = mask3; m; m &= m - 1) {
+        int a, b;
+        ev_slices(c, E, 3, __ffs(m) - 1, fl, fh, a, b);
+        for (int jb = a; jb < b; jb += 32) {
+            const int j = jb + lane;
+            bool pass = false;
+            double d = 0.0;
+            if (j < b) {
+                d = fabs(((double)H.x0[j] + off3) - xc3);
+                pass = (d <= w0) && ev_y_ok(c, E, j, y3);
+            }
+            const unsigned pm = __ballot_sync(FULL, pass);
+            const int at = n_list + __popc(pm & lanemask_lt());
+            if (pass && at < kSelCap) { cj[at] = (uint16_t)j; cd[at] = d; }
+            n_list += __popc(pm);
+        }
+    }
+    __syncwarp();
+    if (n_list > kSelCap) {
+        if (lane == o) ev_select_serial(c, E, mask3, fl, fh, off3, xc3, w0, y3, max_first, sh.slot + o * kMaxFirst);
+    } else {
+        for (int i = lane; i < n_list; i += 32) {
+            const double di = cd[i];
+            const int ji = cj[i];
+            int rank = 0;
+            for (int q = 0; q < n_list; ++q) rank += (q != i && closer(H, cd[q], (int)cj[q], di, ji)) ? 1 : 0;
+            if (rank < max_first) sh.slot[o * kMaxFirst + rank] = (uint16_t)ji;
+        }
+    }
+    __syncwarp();
+}
+
+__device__ __forceinline__ void ev_general_track(const DevConst &c, const EventWarp &sh, const HitsFused &H, const ds_seeds &seeds,
+                                              const ds_tracks &out, int s, int f0, int nF, int o)
+{
+    const Candidate best = ev_choose_general(c, sh, H, f0, nF, o);
+    if (best.score == kNoScore) write_not_found(out, s);
+    else ev_write_track(c, H, seeds, out, s, best);
+}
+
 // Seeds [cb, ce) (at most 32) of the event, by one warp on its own, in rounds of the phases of track_chunk (ds_track.cuh):
 //   A  lane per seed: S2, first window in UTbX (S3); a window with more than max_first hits is ranked by the whole warp
 //   B  lane per first hit: the three refined windows (S4), the lane queues the fits
-//   F  lane per queued combination: fit (S5)      C  lane per seed: best candidate (S6), track record
-__device__ __forceinline__ void event_chunk(const DevConst &c, WarpShared<uint16_t, false> &sh, const EventCtx &E, const ds_seeds &seeds,
+//   F  lane per queued combination: fit (S5); the lane that holds a seed's one best fit writes the track record (S6)
+//   C  lane per seed: seeds without a track; seeds with exact score ties or more combinations than the queue holds
+__device__ __forceinline__ void event_chunk(const DevConst &c, EventWarp &sh, const EventCtx &E, const ds_seeds &seeds,
                                             int cb, int ce, const ds_tracks &out, const SeedPre &pre)
 {
     const unsigned FULL = 0xffffffffu;
@@ -180,18 +325,15 @@ __device__ __forceinline__ void event_chunk(const DevConst &c, WarpShared<uint16
         const int s = s_base + lane;
         const bool act = s < ce;
         int nF = 0;
-        float fy = 0.f, ftx = 0.f, fty = 0.f;   // kept for the track record (phase C)
         double a_xc3 = 0.0, a_off3 = 0.0, a_w0 = 0.0, a_y3 = 0.0;   // the window, kept for the warp's ranking
         unsigned a_mask3 = 0;
         float a_pt = 0.f, a_pw = 0.f;
         if (lane == 0) { sh.n_fit = 0; sh.fit_end = kFitCap; }
         sh.best_bits[lane] = (unsigned long long)__double_as_longlong(kNoScore);
-        sh.best_fit[lane] = INT32_MAX;
         sh.n_best[lane] = 0;
         if (act) {
             const SeedPre sp = pre.s == s ? pre : load_seed(seeds, s, true);
-            fy = sp.y; ftx = sp.tx; fty = sp.ty;
-            const S2 s2 = extrapolate_seed(c, sp.x, fy, ftx, fty, sp.qop);
+            const S2 s2 = extrapolate_seed(c, sp.x, sp.y, sp.tx, sp.ty, sp.qop);
             SeedRec &r = sh.rec[lane];
             r.xm = s2.xm; r.zm = s2.zm; r.w1 = s2.w1;
             r.y[0] = s2.y0; r.y[1] = s2.y1; r.y[2] = s2.y2; r.y[3] = s2.y3;
@@ -206,6 +348,7 @@ __device__ __forceinline__ void event_chunk(const DevConst &c, WarpShared<uint16
             for (unsigned m = a_mask3; m; m &= m - 1) {
                 int a, b;
                 ev_slices(c, E, 3, __ffs(m) - 1, fl, fh, a, b);
+#pragma unroll 1
                 for (int j = a; j < b; ++j) {
                     const float xj = H.x0[j];
                     if (!(fabsf(xj - pf.t) <= pf.w)) continue;
@@ -225,41 +368,7 @@ __device__ __forceinline__ void event_chunk(const DevConst &c, WarpShared<uint16
                          y3 = __shfl_sync(FULL, a_y3, o);
             const unsigned mask3 = __shfl_sync(FULL, a_mask3, o);
             const float pt = __shfl_sync(FULL, a_pt, o), pw = __shfl_sync(FULL, a_pw, o);
-            const int fl = xslice<kFine>(pt - pw, c.xb_off, c.xb_scale), fh = xslice<kFine>(pt + pw, c.xb_off, c.xb_scale);
-            uint16_t *cj = &sh.near[0][0];                       // free in phase A: the hits,
-            double *cd = reinterpret_cast<double *>(sh.res);     //                  their distances
-            static_assert(sizeof(sh.near) >= kSelCap * sizeof(uint16_t) && sizeof(sh.res) >= kSelCap * sizeof(double), "ranking lists");
-            int n_list = 0;
-            for (unsigned m = mask3; m; m &= m - 1) {
-                int a, b;
-                ev_slices(c, E, 3, __ffs(m) - 1, fl, fh, a, b);
-                for (int jb = a; jb < b; jb += 32) {
-                    const int j = jb + lane;
-                    bool pass = false;
-                    double d = 0.0;
-                    if (j < b) {
-                        d = fabs(((double)H.x0[j] + off3) - xc3);
-                        pass = (d <= w0) && ev_y_ok(c, E, j, y3);
-                    }
-                    const unsigned pm = __ballot_sync(FULL, pass);
-                    const int at = n_list + __popc(pm & lanemask_lt());
-                    if (pass && at < kSelCap) { cj[at] = (uint16_t)j; cd[at] = d; }
-                    n_list += __popc(pm);
-                }
-            }
-            __syncwarp();
-            if (n_list > kSelCap) {
-                if (lane == o) ev_select_serial(c, E, mask3, fl, fh, off3, xc3, w0, y3, max_first, my_slot);
-            } else {
-                for (int i = lane; i < n_list; i += 32) {
-                    const double di = cd[i];
-                    const int ji = cj[i];
-                    int rank = 0;
-                    for (int q = 0; q < n_list; ++q) rank += (q != i && closer(H, cd[q], (int)cj[q], di, ji)) ? 1 : 0;
-                    if (rank < max_first) sh.slot[o * kMaxFirst + rank] = (uint16_t)ji;
-                }
-            }
-            __syncwarp();
+            ev_select_warp(c, E, sh, o, mask3, pt, pw, off3, xc3, w0, y3, max_first);
         }
         hits_zw_ready(H);
         const int nFc = min(nF, max_first);
@@ -279,7 +388,7 @@ __device__ __forceinline__ void event_chunk(const DevConst &c, WarpShared<uint16
             sh.foff[lane] = (unsigned short)pos;
             for (int k = 0; k < nFc; ++k) {
                 sh.fs[pos + k] = (unsigned short)(lane * kMaxFirst + k);
-                sh.zw3[pos + k] = make_float2(hit_z(H, (int)my_slot[k]), 0.f);
+                sh.z3[pos + k] = hit_z(H, (int)my_slot[k]);
             }
         }
         __syncwarp();
@@ -292,7 +401,7 @@ __device__ __forceinline__ void event_chunk(const DevConst &c, WarpShared<uint16
                 const SeedRec &t2 = sh.rec[o];
                 // trajectory through (first hit, magnet point), refined windows
                 const double x3 = (double)H.x0[j3] + c.dxdy[3] * t2.y[3];
-                const double txc = (x3 - t2.xm) / ((double)sh.zw3[f].x - t2.zm);
+                const double txc = (x3 - t2.xm) / ((double)sh.z3[f] - t2.zm);
                 int nh = 1, m1 = 1, m2 = 1;
 #pragma unroll 1
                 for (int l = 0; l < 3; ++l) {
@@ -323,71 +432,43 @@ __device__ __forceinline__ void event_chunk(const DevConst &c, WarpShared<uint16
             }
         }
         __syncwarp();
-        // ---- fit phase ------------------------------------------------------------------------------------------------------------
+        // ---- fit phase: lane per queued combination; the lane with a seed's one best fit writes its track record ---------------------
         const int n_fit = min(sh.n_fit, sh.fit_end);
         {
             unsigned long long bits = (unsigned long long)__double_as_longlong(kNoScore);
             int o = 0;
+            Candidate cand;
+            cand.score = kNoScore;
             if (lane < n_fit) {
                 const int tk = sh.task[lane], f = tk & 511, i1 = (tk >> 9) & 1, i2 = (tk >> 10) & 1;
                 const int sl = sh.fs[f];
                 o = sl / kMaxFirst;
-                const float2 zw = sh.zw3[f];
-                const FitRes r = fit_combo(c, H, sh.rec[o], idx_get(sh.near[3 * f][0]), idx_get(sh.near[3 * f + 1][i1]),
-                                           idx_get(sh.near[3 * f + 2][i2]), (int)sh.slot[sl], (double)zw.x,
-                                           (double)first_w(H, zw, (int)sh.slot[sl]));
-                sh.res[lane] = r;
+                cand.j0 = idx_get(sh.near[3 * f][0]);
+                cand.j1 = idx_get(sh.near[3 * f + 1][i1]);
+                cand.j2 = idx_get(sh.near[3 * f + 2][i2]);
+                cand.j3 = (int)sh.slot[sl];
+                cand.nh = 1 + (cand.j0 >= 0) + (cand.j1 >= 0) + (cand.j2 >= 0);
+                const FitRes r = fit_combo(c, H, sh.rec[o], cand.j0, cand.j1, cand.j2, cand.j3, (double)sh.z3[f], (double)H.gw[H.src[cand.j3]]);
+                cand.score = r.score; cand.a = r.a; cand.b = r.b; cand.chi2 = r.chi2;
                 if (r.score != kNoScore) {
                     bits = (unsigned long long)__double_as_longlong(r.score);   // scores are >= +0: bit order = value order
                     atomicMin(&sh.best_bits[o], bits);
                 }
             }
             __syncwarp();
-            if (lane < n_fit && bits != (unsigned long long)__double_as_longlong(kNoScore) && bits == sh.best_bits[o]) {
-                atomicMin(&sh.best_fit[o], lane);
-                atomicAdd(&sh.n_best[o], 1);
-            }
+            const bool top = cand.score != kNoScore && bits == sh.best_bits[o];
+            if (top) atomicAdd(&sh.n_best[o], 1);
+            __syncwarp();
+            // one fit with the smallest score and every combination of the seed queued: that is the track
+            if (top && sh.n_best[o] == 1) ev_write_track(c, H, seeds, out, s_base + o, cand);
         }
-        __syncwarp();
-        // ---- phase C -----------------------------------------------------------------------------------------------------------
+        // ---- phase C: seeds without a track; exact score ties and fits that were not queued: the general comparison ---------
         if (take) {
-            const int f0 = sh.foff[lane];
-            // one fit with the smallest score: that is the track; exact ties and fits that were not queued go through the
-            // general comparison
             const int nb = sh.n_best[lane];
-            const int bt = nb == 1 ? sh.best_fit[lane] : -1;
-            Candidate best;
-            best.score = kNoScore;
-            if (nb >= 2) {
-                best = choose_general<uint16_t, false>(c, sh, H, f0, nFc, lane);
-            } else if (bt >= 0) {
-                const FitRes r = sh.res[bt];
-                const int tk = sh.task[bt], bf = tk & 511, i1 = (tk >> 9) & 1, i2 = (tk >> 10) & 1;
-                best.score = r.score; best.a = r.a; best.b = r.b; best.chi2 = r.chi2;
-                best.j0 = idx_get(sh.near[3 * bf][0]);
-                best.j1 = idx_get(sh.near[3 * bf + 1][i1]);
-                best.j2 = idx_get(sh.near[3 * bf + 2][i2]);
-                best.j3 = (int)sh.slot[sh.fs[bf]];
-                best.nh = 1 + (best.j0 >= 0) + (best.j1 >= 0) + (best.j2 >= 0);
-            }
-            if (best.score == kNoScore) {
+            if (nb == 0) {
                 write_not_found(out, s);
-            } else {
-                const double ys = (double)fy, txs = (double)ftx, tys = (double)fty;
-                out.x[s] = (float)best.a;
-                out.y[s] = (float)(ys + tys * (c.z_ref - c.z_seed));
-                out.tx[s] = (float)best.b;
-                out.ty[s] = (float)tys;
-                out.qop[s] = (float)((txs - best.b) / c.kick);
-                out.chi2[s] = (float)best.chi2;
-                out.nhits[s] = best.nh;
-                out.found[s] = 1;
-                int4 hv;
-                hv.x = best.j0 >= 0 ? hit_perm(H, best.j0) : -1;
-                hv.y = best.j1 >= 0 ? hit_perm(H, best.j1) : -1;
-                hv.z = best.j2 >= 0 ? hit_perm(H, best.j2) : -1;
-                hv.w = hit_perm(H, best.j3);
-                reinterpret_cast<int4 *>(out.hit)[s] = hv;
+            } else if (nb >= 2) {
+                ev_general_track(c, sh, H, seeds, out, s, sh.foff[lane], nFc, lane);
             }
         }
         s_base += n_take;
@@ -399,7 +480,8 @@ __device__ __forceinline__ void event_chunk(const DevConst &c, WarpShared<uint16
 template <int W, int kMinBlocks>
 __global__ void __launch_bounds__(32 * W, kMinBlocks)
 k_event(const __grid_constant__ DevConst c, const ds_hits hits, const ds_seeds seeds, const int32_t *__restrict__ hit_offsets,
-        const int32_t *__restrict__ seed_offsets, const ds_tracks out, int cap, int bulk, int32_t *__restrict__ redo)
+        const int32_t *__restrict__ seed_offsets, const ds_tracks out, const EventLayout L, int cap, int bulk,
+        int32_t *__restrict__ redo)
 {
     extern __shared__ __align__(16) unsigned char smem[];
     constexpr int T = 32 * W;
@@ -412,7 +494,6 @@ k_event(const __grid_constant__ DevConst c, const ds_hits hits, const ds_seeds s
     if (s_begin == s_end || !mine) return;
 
     const int nfine = c.n_bins * kSub, nw = nfine / 2;   // nw words hold the nfine counts; word nw takes the total
-    const EventLayout L = event_layout<W>(cap, nfine);
     EventHead &hd = *reinterpret_cast<EventHead *>(smem);
     uint32_t *hist = reinterpret_cast<uint32_t *>(smem + L.HI);
     float *b_s = reinterpret_cast<float *>(smem + L.S);
@@ -427,18 +508,19 @@ k_event(const __grid_constant__ DevConst c, const ds_hits hits, const ds_seeds s
 #pragma unroll
         for (int k = 0; k < 5; ++k) mbar_init(&hd.bars[k], 1);
         hd.nonuni = 0;
-        if (bulk && n > 0) {   // w is read much later, for fitted hits only: bring the event's slice into L2 now
+        if (bulk && n > 0) {   // w is read much later, for fitted hits only: bring the event's slice into L2 now;
             const int a0 = h0 & ~3, a1 = (h0 + n + 3) & ~3;   // the arrays are padded by 4 elements (ds.h)
             l2_prefetch(hits.w + a0, 4u * (uint32_t)(a1 - a0));
+            l2_prefetch(hits.z + a0, 4u * (uint32_t)(a1 - a0));   // z follows once the unsorted x0 has left its buffer
         }
     }
     for (int k = tid; k < (nw + 4) / 4; k += T) reinterpret_cast<uint4 *>(hist)[k] = make_uint4(0u, 0u, 0u, 0u);
     if (tid < kLayers * DS_MAX_SECTORS) hd.yb[tid] = make_float2(0.f, 0.f);
     __syncthreads();
-    stage_field(b_z, hits.x0, h0, n, &hd.bars[0], bulk != 0);
-    stage_field(b_p, hits.id, h0, n, &hd.bars[1], bulk != 0);
-    stage_field(b_s, hits.ymin, h0, n, &hd.bars[2], bulk != 0);
-    stage_field(b_y, hits.ymax, h0, n, &hd.bars[3], bulk != 0);
+    stage_words(b_z, hits.x0, h0, n, &hd.bars[0], bulk != 0);
+    stage_words(b_p, hits.id, h0, n, &hd.bars[1], bulk != 0);
+    stage_words(b_s, hits.ymin, h0, n, &hd.bars[2], bulk != 0);
+    stage_words(b_y, hits.ymax, h0, n, &hd.bars[3], bulk != 0);
     // the lane's first seed, fetched now so that the load is in flight with the hits
     SeedPre pre;
     {
@@ -467,7 +549,7 @@ k_event(const __grid_constant__ DevConst c, const ds_hits hits, const ds_seeds s
                 const uint32_t old = atomicAdd(&hist[b >> 1], 1u << sh16);
                 const uint32_t slot = (old >> sh16) & 0xffffu;
                 pk[u] = (int)(((uint32_t)b << 20) | slot);
-                if (slot == 0) hd.yb[b >> 6] = make_float2(lov[u], hiv[u]);
+                if (slot == 0) hd.yb[b >> kFineLog2] = make_float2(lov[u], hiv[u]);
             }
         }
         *reinterpret_cast<int4 *>(b_p + k0) = make_int4(pk[0], pk[1], pk[2], pk[3]);
@@ -478,6 +560,7 @@ k_event(const __grid_constant__ DevConst c, const ds_hits hits, const ds_seeds s
         const int per = ((nw + T - 1) / T) | 1;   // odd: the threads' runs start in different banks
         const int kb = min(tid * per, nw), ke = min(kb + per, nw);
         uint32_t sum = 0;
+#pragma unroll 1
         for (int k = kb; k < ke; ++k) {
             const uint32_t w = hist[k];
             sum += (w & 0xffffu) + (w >> 16);
@@ -493,6 +576,7 @@ k_event(const __grid_constant__ DevConst c, const ds_hits hits, const ds_seeds s
         __syncthreads();
         uint32_t run = inc - sum;
         for (int w = 0; w < wid; ++w) run += (uint32_t)ws[w];
+#pragma unroll 1
         for (int k = kb; k < ke; ++k) {
             const uint32_t w = hist[k], c0 = w & 0xffffu, c1 = w >> 16;
             hist[k] = run | ((run + c0) << 16);
@@ -512,7 +596,7 @@ k_event(const __grid_constant__ DevConst c, const ds_hits hits, const ds_seeds s
 #pragma unroll
             for (int u = 0; u < 4; ++u) {
                 const int k = k0 + u;
-                const float2 r = hd.yb[(uint32_t)pkv[u] >> 26];
+                const float2 r = hd.yb[(uint32_t)pkv[u] >> (20 + kFineLog2)];
                 differs |= (k >= d && k < kend) & ((lov[u] != r.x) | (hiv[u] != r.y));
             }
         }
@@ -537,9 +621,13 @@ k_event(const __grid_constant__ DevConst c, const ds_hits hits, const ds_seeds s
             }
         }
     }
+    if (tid < kLayers * DS_MAX_SECTORS) {
+        const float2 b = hd.yb[tid];
+        hd.ye[tid] = make_double2((double)b.x - c.y_tol, (double)b.y + c.y_tol);
+    }
     __syncthreads();
     // the unsorted x0 is dead: its buffer takes z (by index inside the event); the searches start while it is in flight
-    stage_field(b_z, hits.z, h0, n, &hd.bars[4], bulk != 0);
+    stage_words(b_z, hits.z, h0, n, &hd.bars[4], bulk != 0);
     __syncthreads();   // its last elements come by ordinary stores
 
     // ---- S2..S6 on the shared-memory copy ---------------------------------------------------------------------------------------------
@@ -549,12 +637,24 @@ k_event(const __grid_constant__ DevConst c, const ds_hits hits, const ds_seeds s
     E.H.zbar = &hd.bars[4];
     E.tab = tab;
     E.yb = hd.yb;
+    E.ye = hd.ye;
     E.uni = hd.nonuni == 0;
-    E.rsec = (int)floor(c.y_tol * c.inv_h + 1e-9) + 1;
-    WarpShared<uint16_t, false> *warps = reinterpret_cast<WarpShared<uint16_t, false> *>(smem + L.WS);
+    E.rsec = c.y_rsec;
+    EventWarp *warps = reinterpret_cast<EventWarp *>(smem + L.WS);
     const int chunk = seed_chunk<W>(s_begin, s_end);
     for (int cb = s_begin + wid * chunk; cb < s_end; cb += W * chunk)
         event_chunk(c, warps[wid], E, seeds, cb, min(cb + chunk, s_end), out, pre);
+}
+
+// Development aid: DS_EVENT_W=6|7 runs the 3-blocks-per-SM configuration with that many warps per block
+static int event_warps_override()
+{
+    static int v = -1;
+    if (v < 0) {
+        const char *e = getenv("DS_EVENT_W");
+        v = e ? atoi(e) : 0;
+    }
+    return v;
 }
 
 template <int W, int kMinBlocks>
@@ -566,7 +666,8 @@ static cudaError_t launch_event_one(const DevConst &c, const ds_hits &hits, cons
     const cudaError_t aerr = opt_in_max_smem(k_event<W, kMinBlocks>, &opted);
     if (aerr != cudaSuccess) return aerr;
     prof.begin(DS_K_EVENT, st);
-    k_event<W, kMinBlocks><<<n_events, 32 * W, smem, st>>>(c, hits, seeds, hit_offsets, seed_offsets, out, cap, bulk, redo);
+    k_event<W, kMinBlocks><<<n_events, 32 * W, smem, st>>>(c, hits, seeds, hit_offsets, seed_offsets, out, event_layout<W>(cap, c.n_bins * kSub),
+                                                           cap, bulk, redo);
     prof.end(st);
     return cudaGetLastError();
 }
@@ -584,7 +685,14 @@ cudaError_t launch_event(const DevConst &c, const ds_hits &hits, const ds_seeds 
                            reinterpret_cast<uintptr_t>(hits.ymin) | reinterpret_cast<uintptr_t>(hits.ymax) |
                            reinterpret_cast<uintptr_t>(hits.w) | reinterpret_cast<uintptr_t>(hits.id);
     const int bulk = (bits & 15) == 0;
-    size_t sm = event_layout<5>(cap, nfine).total;
+    const int want = event_warps_override();
+    size_t sm = event_layout<7>(cap, nfine).total;
+    if (want == 7 && 3 * (sm + kPerBlock) <= kSm + 1024)
+        return launch_event_one<7, 3>(c, hits, seeds, hit_offsets, seed_offsets, n_events, cap, sm, bulk, out, redo, st, prof);
+    sm = event_layout<6>(cap, nfine).total;
+    if (want == 6 && 3 * (sm + kPerBlock) <= kSm + 1024)
+        return launch_event_one<6, 3>(c, hits, seeds, hit_offsets, seed_offsets, n_events, cap, sm, bulk, out, redo, st, prof);
+    sm = event_layout<5>(cap, nfine).total;
     if (3 * (sm + kPerBlock) <= kSm + 1024)
         return launch_event_one<5, 3>(c, hits, seeds, hit_offsets, seed_offsets, n_events, cap, sm, bulk, out, redo, st, prof);
     sm = event_layout<8>(cap, nfine).total;

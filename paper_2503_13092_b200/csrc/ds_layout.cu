@@ -50,6 +50,11 @@ k_layout(const __grid_constant__ DevConst c, const LayoutPtrs p, const int32_t *
     int *hist = reinterpret_cast<int *>(s_src + cap);                  // [nfine + 1]
     unsigned long long *bar_x = &bars[0], *bar_i = &bars[1], *bar_b = &bars[2];
 
+    if (only) {   // normally nothing is left over: all marks of this block's events in one round of loads, then out
+        bool any = false;
+        for (int e = blockIdx.x + threadIdx.x * gridDim.x; e < n_events; e += blockDim.x * gridDim.x) any |= only[e] != 0;
+        if (!__syncthreads_or(any)) return;
+    }
     // one event per block; with `only` (the events k_event has left over) a small grid walks the event list and a block may
     // meet several marked events: the launcher then passes cap = 0, so that none of them takes the staged path (whose
     // mbarriers are armed once per block)

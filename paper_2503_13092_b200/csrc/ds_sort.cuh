@@ -7,7 +7,10 @@
 
 namespace ds {
 
-constexpr int kSub = 4;   // the sort cuts every x0 slice of the bin table into kSub sub-slices (a power of two)
+#ifndef DS_KSUB
+#define DS_KSUB 4
+#endif
+constexpr int kSub = DS_KSUB;   // the sort cuts every x0 slice of the bin table into kSub sub-slices (a power of two)
 
 // Sort bin of a hit: (layer, sector, x0 sub-slice).  t = (x0 + off) * scale is the same fp32 value xbin() floors, and
 // 4t is exact, so floor(floor(kSub * t) / kSub) = floor(t): sub-slice s lies in table slice s / kSub, clamps included.
@@ -62,6 +65,13 @@ __device__ inline void block_exclusive_scan(int *v, int n, int *warp_sums)
 // (a source pointer that is not 16-byte aligned) everything is loaded by ordinary loads and the barrier only armed.
 // Every thread of the block calls it; the buffer must be free (a __syncthreads after its last reader), and a
 // __syncthreads plus mbar_wait(bar) must precede the first read.
+template <typename T>
+__device__ __forceinline__ void stage_field(T *buf, const T *__restrict__ src, int h0, int n, unsigned long long *bar,
+                                            bool bulk);
+
+// the same out of line for 4-byte elements of either type (k_event calls it five times per event)
+__device__ void stage_words(void *buf, const void *src, int h0, int n, unsigned long long *bar, bool bulk);
+
 template <typename T>
 __device__ __forceinline__ void stage_field(T *buf, const T *__restrict__ src, int h0, int n, unsigned long long *bar,
                                             bool bulk)

@@ -81,6 +81,11 @@ k_track(const __grid_constant__ DevConst c, const LayoutPtrs L, const ds_seeds s
     float *st_x0 = reinterpret_cast<float *>(smem_raw + kHitsAt);   // [cap]
 
     const int tid = threadIdx.x;
+    if (only) {   // normally nothing is left over: all marks of this block's events in one round of loads, then out
+        bool any = false;
+        for (int e = blockIdx.x + threadIdx.x * gridDim.x; e < n_events; e += blockDim.x * gridDim.x) any |= only[e] != 0;
+        if (!__syncthreads_or(any)) return;
+    }
     // one event per block; with `only` (the events k_event has left over) a small grid walks the event list and a block may
     // meet several marked events: the launcher then passes cap = 0, so that none of them is staged (the mbarrier is armed
     // once per block)

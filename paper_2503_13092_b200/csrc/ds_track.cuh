@@ -208,6 +208,15 @@ __device__ __forceinline__ bool y_compatible(const DevConst &c, const HitsT &H, 
     return (lo <= y) & (y <= hi);
 }
 
+// Equal distances: smaller id, then (duplicates) the hit that comes first in the caller's arrays
+template <typename HitsT>
+__device__ __forceinline__ bool closer_tie(const HitsT &H, int j1, int j2)
+{
+    const int i1 = hit_id(H, j1), i2 = hit_id(H, j2);
+    if (i1 != i2) return i1 < i2;
+    return hit_perm(H, j1) < hit_perm(H, j2);
+}
+
 // (distance, id, index in the caller's arrays) order of the "closest hits" rules: a total order, so the result does
 // not depend on the order the hits are looked at; ids are only read on an exact distance tie
 template <typename HitsT>
@@ -215,9 +224,7 @@ __device__ __forceinline__ bool closer(const HitsT &H, double d1, int j1, double
 {
     if (d1 != d2) return d1 < d2;
     if (j2 < 0) return true;
-    const int i1 = hit_id(H, j1), i2 = hit_id(H, j2);
-    if (i1 != i2) return i1 < i2;
-    return hit_perm(H, j1) < hit_perm(H, j2);   // duplicates: the one that comes first in the caller's arrays
+    return closer_tie(H, j1, j2);
 }
 
 // fp32 superset test of "|x0 + off - x| <= w" (decided in fp64 afterwards): |x0 - t| <= w', with t = (float)(x - off)
