@@ -34,8 +34,23 @@ constexpr int kSelCap = 64;            // hits of an over-full first window that
 
 // State of one warp of k_event (cf. WarpShared of ds_track.cuh; no fit results are kept: the lane that fits the best
 // combination of a seed writes the track record itself)
+// What the later phases need of the warp's 32 seeds (SeedRec of ds_track.cuh), one array per field: lanes that read or
+// write their own seed, or first hits that read their seeds, then meet no shared-memory bank conflict by layout
+struct SeedRecs {
+    double xm[32], zm[32], w1[32], y[4][32];
+    unsigned short mask[4][32];
+    __device__ __forceinline__ SeedRec get(int o) const
+    {
+        SeedRec r;
+        r.xm = xm[o]; r.zm = zm[o]; r.w1 = w1[o];
+        r.y[0] = y[0][o]; r.y[1] = y[1][o]; r.y[2] = y[2][o]; r.y[3] = y[3][o];
+        r.mask[0] = mask[0][o]; r.mask[1] = mask[1][o]; r.mask[2] = mask[2][o]; r.mask[3] = mask[3][o];
+        return r;
+    }
+};
+
 struct EventWarp {
-    SeedRec rec[32];
+    SeedRecs rec;
     unsigned long long best_bits[32];     // per seed: smallest score among its fits (bits of the non-negative double)
     uint16_t near[3 * kFirstCap][2];      // phase B: closest / second closest hit of (first hit, layer); phase A: ranking lists
     float z3[kFirstCap];                  // z of the first hit
@@ -232,7 +247,7 @@ __device__ __forceinline__ Candidate ev_choose_general(const DevConst &c, const 
     Candidate best;
     best.score = kNoScore; best.a = 0.0; best.b = 0.0; best.chi2 = 0.0;
     best.nh = 0; best.j0 = -1; best.j1 = -1; best.j2 = -1; best.j3 = -1;
-    const SeedRec &s2 = sh.rec[o];
+    const SeedRec s2 = sh.rec.get(o);
     for (int k = 0; k < nF; ++k) {
         const int f = f0 + k;
         if (sh.ffit[f] == kFitNone) continue;
@@ -334,12 +349,12 @@ __device__ __forceinline__ void event_chunk(const DevConst &c, EventWarp &sh, co
         if (act) {
             const SeedPre sp = pre.s == s ? pre : load_seed(seeds, s, true);
             const S2 s2 = extrapolate_seed(c, sp.x, sp.y, sp.tx, sp.ty, sp.qop);
-            SeedRec &r = sh.rec[lane];
-            r.xm = s2.xm; r.zm = s2.zm; r.w1 = s2.w1;
-            r.y[0] = s2.y0; r.y[1] = s2.y1; r.y[2] = s2.y2; r.y[3] = s2.y3;
+            SeedRecs &r = sh.rec;
+            r.xm[lane] = s2.xm; r.zm[lane] = s2.zm; r.w1[lane] = s2.w1;
+            r.y[0][lane] = s2.y0; r.y[1][lane] = s2.y1; r.y[2][lane] = s2.y2; r.y[3][lane] = s2.y3;
 #pragma unroll 1
-            for (int l = 0; l < 4; ++l) r.mask[l] = (unsigned short)ev_sector_mask(c, E, l, r.y[l]);
-            a_mask3 = r.mask[3];
+            for (int l = 0; l < 4; ++l) r.mask[l][lane] = (unsigned short)ev_sector_mask(c, E, l, r.y[l][lane]);
+            a_mask3 = r.mask[3][lane];
             a_y3 = s2.y3; a_xc3 = s2.xc3; a_w0 = s2.w0;
             a_off3 = c.dxdy[3] * s2.y3;
             const Prefilter pf = make_prefilter(a_xc3 - a_off3, a_w0);
@@ -398,15 +413,16 @@ __device__ __forceinline__ void event_chunk(const DevConst &c, EventWarp &sh, co
             if (f < n_first) {
                 const int sl = sh.fs[f], o = sl / kMaxFirst;
                 const int j3 = (int)sh.slot[sl];
-                const SeedRec &t2 = sh.rec[o];
+                const SeedRecs &t2 = sh.rec;
+                const double xm = t2.xm[o], zm = t2.zm[o], w1 = t2.w1[o];
                 // trajectory through (first hit, magnet point), refined windows
-                const double x3 = (double)H.x0[j3] + c.dxdy[3] * t2.y[3];
-                const double txc = (x3 - t2.xm) / ((double)sh.z3[f] - t2.zm);
+                const double x3 = (double)H.x0[j3] + c.dxdy[3] * t2.y[3][o];
+                const double txc = (x3 - xm) / ((double)sh.z3[f] - zm);
                 int nh = 1, m1 = 1, m2 = 1;
 #pragma unroll 1
                 for (int l = 0; l < 3; ++l) {
-                    const double xp = t2.xm + txc * (c.z_layer[l] - t2.zm);
-                    int2 r = ev_search(c, E, l, xp, t2.y[l], t2.w1, (unsigned)t2.mask[l]);
+                    const double xp = xm + txc * (c.z_layer[l] - zm);
+                    int2 r = ev_search(c, E, l, xp, t2.y[l][o], w1, (unsigned)t2.mask[l][o]);
                     if (l == 0) r.y = -1;   // UTaX keeps the closest hit only
                     sh.near[3 * f + l][0] = (uint16_t)r.x;
                     sh.near[3 * f + l][1] = (uint16_t)r.y;
@@ -448,7 +464,7 @@ __device__ __forceinline__ void event_chunk(const DevConst &c, EventWarp &sh, co
                 cand.j2 = idx_get(sh.near[3 * f + 2][i2]);
                 cand.j3 = (int)sh.slot[sl];
                 cand.nh = 1 + (cand.j0 >= 0) + (cand.j1 >= 0) + (cand.j2 >= 0);
-                const FitRes r = fit_combo(c, H, sh.rec[o], cand.j0, cand.j1, cand.j2, cand.j3, (double)sh.z3[f], (double)H.gw[H.src[cand.j3]]);
+                const FitRes r = fit_combo(c, H, sh.rec.get(o), cand.j0, cand.j1, cand.j2, cand.j3, (double)sh.z3[f], (double)H.gw[H.src[cand.j3]]);
                 cand.score = r.score; cand.a = r.a; cand.b = r.b; cand.chi2 = r.chi2;
                 if (r.score != kNoScore) {
                     bits = (unsigned long long)__double_as_longlong(r.score);   // scores are >= +0: bit order = value order
@@ -473,6 +489,72 @@ __device__ __forceinline__ void event_chunk(const DevConst &c, EventWarp &sh, co
         }
         s_base += n_take;
         __syncwarp();   // the lists are rewritten by the next round
+    }
+}
+
+// ---- the sort passes over four neighbouring elements k0 .. k0+3 of the staged buffers (element i of the event sits at index
+//      d + i; kFull: all four belong to the event, which is every group but the first and the last) ---------------------------
+template <bool kFull>
+__device__ __forceinline__ void ev_hist4(const DevConst &c, uint32_t *hist, float2 *yb, int32_t *b_p, const float *b_z, const float *b_s,
+                                         const float *b_y, int k0, int d, int kend)
+{
+    const int4 id4 = *reinterpret_cast<const int4 *>(b_p + k0);
+    const float4 x4 = *reinterpret_cast<const float4 *>(b_z + k0), lo4 = *reinterpret_cast<const float4 *>(b_s + k0),
+                 hi4 = *reinterpret_cast<const float4 *>(b_y + k0);
+    const int idv[4] = {id4.x, id4.y, id4.z, id4.w};
+    const float xv[4] = {x4.x, x4.y, x4.z, x4.w}, lov[4] = {lo4.x, lo4.y, lo4.z, lo4.w}, hiv[4] = {hi4.x, hi4.y, hi4.z, hi4.w};
+    int pk[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+        const int k = k0 + u;
+        pk[u] = 0;
+        if (kFull || (k >= d && k < kend)) {
+            const int b = fine_bin(c, idv[u], xv[u]);
+            const int sh16 = (b & 1) * 16;
+            const uint32_t old = atomicAdd(&hist[b >> 1], 1u << sh16);
+            const uint32_t slot = (old >> sh16) & 0xffffu;
+            pk[u] = (int)(((uint32_t)b << 20) | slot);
+            if (slot == 0) yb[b >> kFineLog2] = make_float2(lov[u], hiv[u]);   // reference bounds of the (layer, sector)
+        }
+    }
+    *reinterpret_cast<int4 *>(b_p + k0) = make_int4(pk[0], pk[1], pk[2], pk[3]);
+}
+
+template <bool kFull>
+__device__ __forceinline__ bool ev_check4(const float2 *yb, const int32_t *b_p, const float *b_s, const float *b_y, int k0, int d, int kend)
+{
+    const int4 pk4 = *reinterpret_cast<const int4 *>(b_p + k0);
+    const float4 lo4 = *reinterpret_cast<const float4 *>(b_s + k0), hi4 = *reinterpret_cast<const float4 *>(b_y + k0);
+    const int pkv[4] = {pk4.x, pk4.y, pk4.z, pk4.w};
+    const float lov[4] = {lo4.x, lo4.y, lo4.z, lo4.w}, hiv[4] = {hi4.x, hi4.y, hi4.z, hi4.w};
+    bool differs = false;
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+        const int k = k0 + u;
+        const float2 r = yb[(uint32_t)pkv[u] >> (20 + kFineLog2)];
+        differs |= (kFull || (k >= d && k < kend)) & ((lov[u] != r.x) | (hiv[u] != r.y));
+    }
+    return differs;
+}
+
+template <bool kFull>
+__device__ __forceinline__ void ev_scatter4(const uint16_t *tab, const int32_t *b_p, const float *b_z, float *b_s, uint16_t *src, int k0,
+                                            int d, int kend)
+{
+    const int4 pk4 = *reinterpret_cast<const int4 *>(b_p + k0);
+    const float4 x4 = *reinterpret_cast<const float4 *>(b_z + k0);
+    const uint32_t pkv[4] = {(uint32_t)pk4.x, (uint32_t)pk4.y, (uint32_t)pk4.z, (uint32_t)pk4.w};
+    const float xv[4] = {x4.x, x4.y, x4.z, x4.w};
+    int pos[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) pos[u] = (int)tab[pkv[u] >> 20] + (int)(pkv[u] & 0xfffffu);
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+        const int k = k0 + u;
+        if (kFull || (k >= d && k < kend)) {
+            b_s[pos[u]] = xv[u];
+            src[pos[u]] = (uint16_t)(k - d);
+        }
     }
 }
 
@@ -531,28 +613,10 @@ k_event(const __grid_constant__ DevConst c, const ds_hits hits, const ds_seeds s
     __syncthreads();   // the elements after the last 16-byte boundary were stored by ordinary stores
 #pragma unroll
     for (int k = 0; k < 4; ++k) mbar_wait(&hd.bars[k], 0);
-    // ---- A: histogram; a thread takes four neighbouring elements of the staged buffers at a time ----------------------------
+    // ---- A: histogram; a thread takes four neighbouring elements of the staged buffers at a time (ev_hist4) -------------------
     for (int k0 = 4 * tid; k0 < kend; k0 += 4 * T) {
-        const int4 id4 = *reinterpret_cast<const int4 *>(b_p + k0);
-        const float4 x4 = *reinterpret_cast<const float4 *>(b_z + k0), lo4 = *reinterpret_cast<const float4 *>(b_s + k0),
-                     hi4 = *reinterpret_cast<const float4 *>(b_y + k0);
-        const int idv[4] = {id4.x, id4.y, id4.z, id4.w};
-        const float xv[4] = {x4.x, x4.y, x4.z, x4.w}, lov[4] = {lo4.x, lo4.y, lo4.z, lo4.w}, hiv[4] = {hi4.x, hi4.y, hi4.z, hi4.w};
-        int pk[4];
-#pragma unroll
-        for (int u = 0; u < 4; ++u) {
-            const int k = k0 + u;
-            pk[u] = 0;
-            if (k >= d && k < kend) {
-                const int b = fine_bin(c, idv[u], xv[u]);
-                const int sh16 = (b & 1) * 16;
-                const uint32_t old = atomicAdd(&hist[b >> 1], 1u << sh16);
-                const uint32_t slot = (old >> sh16) & 0xffffu;
-                pk[u] = (int)(((uint32_t)b << 20) | slot);
-                if (slot == 0) hd.yb[b >> kFineLog2] = make_float2(lov[u], hiv[u]);
-            }
-        }
-        *reinterpret_cast<int4 *>(b_p + k0) = make_int4(pk[0], pk[1], pk[2], pk[3]);
+        if (k0 >= d && k0 + 4 <= kend) ev_hist4<true>(c, hist, hd.yb, b_p, b_z, b_s, b_y, k0, d, kend);
+        else ev_hist4<false>(c, hist, hd.yb, b_p, b_z, b_s, b_y, k0, d, kend);
     }
     __syncthreads();
     // ---- B: exclusive scan of the counts, two 16-bit counts per word -> bin starts ---------------------------------------------
@@ -589,37 +653,16 @@ k_event(const __grid_constant__ DevConst c, const ds_hits hits, const ds_seeds s
     {
         bool differs = false;
         for (int k0 = 4 * tid; k0 < kend; k0 += 4 * T) {
-            const int4 pk4 = *reinterpret_cast<const int4 *>(b_p + k0);
-            const float4 lo4 = *reinterpret_cast<const float4 *>(b_s + k0), hi4 = *reinterpret_cast<const float4 *>(b_y + k0);
-            const int pkv[4] = {pk4.x, pk4.y, pk4.z, pk4.w};
-            const float lov[4] = {lo4.x, lo4.y, lo4.z, lo4.w}, hiv[4] = {hi4.x, hi4.y, hi4.z, hi4.w};
-#pragma unroll
-            for (int u = 0; u < 4; ++u) {
-                const int k = k0 + u;
-                const float2 r = hd.yb[(uint32_t)pkv[u] >> (20 + kFineLog2)];
-                differs |= (k >= d && k < kend) & ((lov[u] != r.x) | (hiv[u] != r.y));
-            }
+            if (k0 >= d && k0 + 4 <= kend) differs |= ev_check4<true>(hd.yb, b_p, b_s, b_y, k0, d, kend);
+            else differs |= ev_check4<false>(hd.yb, b_p, b_s, b_y, k0, d, kend);
         }
         if (differs) hd.nonuni = 1;
     }
     __syncthreads();   // ymin and ymax are dead from here: their buffers take the x0 in bin order and src
     // ---- C: scatter into bin order ------------------------------------------------------------------------------------------------
     for (int k0 = 4 * tid; k0 < kend; k0 += 4 * T) {
-        const int4 pk4 = *reinterpret_cast<const int4 *>(b_p + k0);
-        const float4 x4 = *reinterpret_cast<const float4 *>(b_z + k0);
-        const uint32_t pkv[4] = {(uint32_t)pk4.x, (uint32_t)pk4.y, (uint32_t)pk4.z, (uint32_t)pk4.w};
-        const float xv[4] = {x4.x, x4.y, x4.z, x4.w};
-        int pos[4];
-#pragma unroll
-        for (int u = 0; u < 4; ++u) pos[u] = (int)tab[pkv[u] >> 20] + (int)(pkv[u] & 0xfffffu);
-#pragma unroll
-        for (int u = 0; u < 4; ++u) {
-            const int k = k0 + u;
-            if (k >= d && k < kend) {
-                b_s[pos[u]] = xv[u];
-                src[pos[u]] = (uint16_t)(k - d);
-            }
-        }
+        if (k0 >= d && k0 + 4 <= kend) ev_scatter4<true>(tab, b_p, b_z, b_s, src, k0, d, kend);
+        else ev_scatter4<false>(tab, b_p, b_z, b_s, src, k0, d, kend);
     }
     if (tid < kLayers * DS_MAX_SECTORS) {
         const float2 b = hd.yb[tid];

@@ -648,13 +648,15 @@ def test_duplicate_hits_and_ties(ds, orc_mlp):
     check_both(ds, d2, orc_mlp, params=dict(P, dv1=1))
 
 
-def test_dense_window_more_than_ten_first_hits(ds, orc_mlp):
-    """A crowded UTbX: > 10 (and > 32) hits inside the first window -> the 10 closest by (distance, id)."""
+@pytest.mark.parametrize("extra_n,x_half", [(6000, 860.0), (8000, 200.0)])
+def test_dense_window_more_than_ten_first_hits(ds, orc_mlp, extra_n, x_half):
+    """A crowded UTbX: > 10 (and > 32) hits inside the first window -> the 10 closest by (distance, id).  The second
+    case packs the extra hits into |x| < 200 mm: first windows there hold more than 64 hits, which k_event ranks by the
+    seed's own lane instead of the whole warp."""
     d = gen.generate(1, n_events=6)
     rng = np.random.default_rng(2)
-    extra_n = 6000
     lay = np.full(extra_n, 3)
-    x = rng.uniform(-860, 860, extra_n)
+    x = rng.uniform(-x_half, x_half, extra_n)
     x[: extra_n // 2] = np.round(x[: extra_n // 2])                      # many exact ties in distance
     y = rng.uniform(-700, 700, extra_n)
     sec = np.clip(np.floor((y + 700) / 100).astype(np.int64), 0, 13)
@@ -668,6 +670,20 @@ def test_dense_window_more_than_ten_first_hits(ds, orc_mlp):
     ho[e + 1:] += extra_n
     st, sv, t, v = check_both(ds, dict(d, hits=hits, hit_offsets=ho), orc_mlp, params=dict(P, max_event_hits_hint=12288))
     assert st["found"] > 0
+
+
+def test_hint_between_event_sizes(ds, orc_mlp):
+    """A hint below the larger events of the batch: k_event takes the events that fit its staging, k_layout + k_track the
+    others, inside one ds_reconstruct call; the results are those of any other hint."""
+    d = gen.generate(1, n_events=60)
+    sizes = np.diff(d["hit_offsets"])
+    hint = int(np.median(sizes))
+    assert (sizes + 3 > ((hint + 7) & ~7) + 8).any() and (sizes + 3 <= ((hint + 7) & ~7) + 8).any()
+    st, sv, t, v = check_both(ds, d, orc_mlp, params=dict(P, max_event_hits_hint=hint))
+    t0, v0 = gpu_run(ds, d, params=dict(P, max_event_hits_hint=0))
+    for k in t:
+        assert np.array_equal(t[k], t0[k]), k
+    assert v["n"] == v0["n"]
 
 
 # ---- host-buffer path ---------------------------------------------------------------------------------------------------------
