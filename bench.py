@@ -373,28 +373,51 @@ def main():
     alg = algorithmic_bytes(events_rank, sum(n_hits), sum(n_seeds), n_found, n_keep, n_vtx)     # bytes per step
     traffic = ncu_traffic()
     kernels, launches = {}, sum(n for _, n in prof2.values())
-    for name, (ms, n) in prof.items():
+    leftover = ("k_layout", "k_track") if prof.get("k_event", (0, 0))[1] else ()   # with k_event: launches for the events it leaves
+    for name, (ms, n) in prof.items():                                                # over -- none in this workload
         if n == 0:
             continue
         per_launch_ms = ms / n
+        if name in leftover:
+            alg[name] = 0
         bytes_per_launch = alg[name] * args.steps / n
         gbs = bytes_per_launch / (per_launch_ms * 1e-3) / 1e9
         kernels[name] = {"ms_per_launch": per_launch_ms, "ms_per_step": ms / args.steps, "launches_per_step": n / args.steps,
                          "alg_bytes_per_launch": bytes_per_launch, "achieved_gbs": gbs, "frac": gbs / peak,
                          "traffic": traffic.get(name), "ms_per_launch_two_streams": prof2[name][0] / max(1, prof2[name][1])}
+        if name in leftover:
+            kernels[name].update(traffic=None, note="launch for the events above k_event's staging capacity: none here, its blocks leave at once")
     dom = max(kernels, key=lambda k: kernels[k]["ms_per_step"])
     ksum = sum(k["ms_per_step"] for k in kernels.values())
+    # k_event runs S1..S6 in one launch: its algorithmic bytes are the S1 and S2..S6 figures of SURVEY 8d together (what the
+    # steps move when each runs as its own HBM-bound kernel); `min_traffic` is what the fused launch has to move at least
+    # (every input array once, seeds in, tracks out) and `traffic` what ncu measured it to move
+    fused_min = (24 * sum(n_hits) + 28 * sum(n_seeds) + 52 * sum(n_seeds) + 16 * n_found) * args.steps
+    if "k_event" in kernels:
+        ke = kernels["k_event"]
+        ke["covers"] = "S1..S6 (layout, extrapolation, window searches, fits, best candidate)"
+        ke["min_traffic_bytes_per_launch"] = fused_min / (ke["launches_per_step"] * args.steps)
+        ke["min_traffic_gbs"] = ke["min_traffic_bytes_per_launch"] / (ke["ms_per_launch"] * 1e-3) / 1e9
+        ke["min_traffic_frac"] = ke["min_traffic_gbs"] / peak
     roofline = {"bound": "hbm", "kernel": dom, "achieved": kernels[dom]["achieved_gbs"], "peak": peak, "unit": "GB/s",
                 "frac": kernels[dom]["frac"], "traffic": kernels[dom]["traffic"], "peak_source": peak_src,
                 "share_of_step": kernels[dom]["ms_per_step"] / ksum,
+                "alg_bytes_per_launch": kernels[dom]["alg_bytes_per_launch"],
+                "alg_bytes_basis": "SURVEY 8d per-unit figures of the steps the launch covers x the units of one launch (DESIGN.md section 8)",
                 "timing": "CUDA events around every launch, one-stream pass of the same K steps right after the timed region"}
-    whole_gbs = sum(alg.values()) * args.steps / (ms_total * 1e-3) / 1e9
-    # the kernel BASELINE north_star sets the 40 % bar on: search + fit (S2..S6)
+    if dom == "k_event":
+        roofline.update(covers=kernels[dom]["covers"], min_traffic_frac=kernels[dom]["min_traffic_frac"])
+    # the launches of the leftover path are not part of the sum when they are empty
+    whole_gbs = sum(alg[k] for k in kernels if not ("k_event" in kernels and k in ("k_layout", "k_track"))) * args.steps / (ms_total * 1e-3) / 1e9
+    # the kernel BASELINE north_star sets the 40 % bar on: search + fit (S2..S6) -- k_event, which does them with S1 in one launch
     roofline_search_fit = None
-    if "k_track" in kernels:
-        kt = kernels["k_track"]
-        roofline_search_fit = {"bound": "hbm", "kernel": "k_track", "achieved": kt["achieved_gbs"], "peak": peak, "unit": "GB/s",
+    sf = "k_event" if "k_event" in kernels else ("k_track" if "k_track" in kernels else None)
+    if sf:
+        kt = kernels[sf]
+        roofline_search_fit = {"bound": "hbm", "kernel": sf, "achieved": kt["achieved_gbs"], "peak": peak, "unit": "GB/s",
                                "frac": kt["frac"], "traffic": kt["traffic"], "share_of_step": kt["ms_per_step"] / ksum}
+        if sf == "k_event":
+            roofline_search_fit.update(covers=kt["covers"], min_traffic_frac=kt["min_traffic_frac"])
 
     # ---- cfg3: the vertex kernels are bound by plain fp64 arithmetic, not by HBM -----------------------------------
     def vertex_alu_of(kern, trk_list, dev_list, n_pass):
@@ -458,6 +481,8 @@ def main():
             alg_l = algorithmic_bytes(n_ev, nh_l, ns_l, nf_l, nk_l, nv_l)
             kl = {}
             for name, (ms, n) in pl.items():
+                if n and pl.get("k_event", (0, 0))[1] and name in ("k_layout", "k_track"):
+                    alg_l[name] = 0   # launches for the events k_event leaves over: none
                 if n:
                     gbs = alg_l[name] * args.steps / n / (ms / n * 1e-3) / 1e9
                     kl[name] = {"ms_per_launch": ms / n, "ms_per_step": ms / args.steps, "alg_bytes_per_launch": alg_l[name] * args.steps / n,

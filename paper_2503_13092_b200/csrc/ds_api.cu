@@ -158,7 +158,7 @@ cudaError_t reconstruct_launches(ds_handle *h, const DevConst &c, const LayoutPt
 {
     const int32_t *only = nullptr;
     cudaError_t err = cudaSuccess;
-    if (!c.dv1 && !fused_off()) {
+    if (!c.dv1 && !fused_off() && event_kernel_wanted(c, hint)) {
         err = launch_event(c, hits, seeds, hit_offsets, seed_offsets, n_events, hint, out, L.redo, st, h->prof);
         only = L.redo;
     }

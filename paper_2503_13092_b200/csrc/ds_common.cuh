@@ -8,6 +8,15 @@
 
 #include "../../include/ds.h"
 
+// Checked build (DS_NVCC_EXTRA=-DDS_CHECKED): device-side asserts on the shared-memory indices and list sizes of the kernels;
+// a failing one traps and the call returns DS_E_CUDA.  Compiled out otherwise.
+#ifdef DS_CHECKED
+#include <cassert>
+#define DS_ASSERT(x) assert(x)
+#else
+#define DS_ASSERT(x) ((void)0)
+#endif
+
 namespace ds {
 
 constexpr int kLayers = 4;
@@ -71,9 +80,8 @@ __device__ __forceinline__ int id_sector(int id) { return (id >> kIdSectorShift)
 // the x0 order and a window [lo, hi] in x0 maps to the slice range [xbin(lo'), xbin(hi')] for any lo' <= lo, hi' >= hi.
 __device__ __forceinline__ int xbin(float x0, float off, float scale)
 {
-    float t = floorf((x0 + off) * scale);
-    t = fminf(fmaxf(t, 0.0f), (float)(kXBins - 1));
-    return (int)t;
+    const int t = __float2int_rd((x0 + off) * scale);   // floor, saturating, NaN -> 0
+    return min(max(t, 0), kXBins - 1);
 }
 
 // The same for a table with kSlices = kXBins * k slices per (layer, sector) (k a power of two): slice of x0 =
@@ -82,9 +90,9 @@ template <int kSlices>
 __device__ __forceinline__ int xslice(float x0, float off, float scale)
 {
     static_assert(kSlices % kXBins == 0, "slices refine the DS_XBINS slices of the public table");
-    float t = floorf((x0 + off) * scale * (float)(kSlices / kXBins));
-    t = fminf(fmaxf(t, 0.0f), (float)(kSlices - 1));
-    return (int)t;
+    // floor by the conversion itself (round down, saturating, NaN -> 0), then the clamp on the integer
+    const int t = __float2int_rd((x0 + off) * scale * (float)(kSlices / kXBins));
+    return min(max(t, 0), kSlices - 1);
 }
 
 // Order-preserving map float -> uint32 (-0.0 is first folded onto +0.0 so that it compares equal, like IEEE ==).
@@ -221,7 +229,9 @@ struct LayoutPtrs {
 cudaError_t launch_layout(const DevConst &c, const LayoutPtrs &p, const int32_t *hit_offsets, int n_events,
                           int max_event_hits_hint, const int32_t *only, cudaStream_t st, Prof &prof);
 
-// S1..S6 in one kernel (ds_event.cu), Dv0 only; redo[e] = 1 for the events it leaves to k_layout + k_track
+// S1..S6 in one kernel (ds_event.cu), Dv0 only; redo[e] = 1 for the events it leaves to k_layout + k_track.
+// event_kernel_wanted: false for hints so large that only one block of it would fit an SM (then k_layout + k_track run alone)
+bool event_kernel_wanted(const DevConst &c, int max_event_hits_hint);
 cudaError_t launch_event(const DevConst &c, const ds_hits &hits, const ds_seeds &seeds, const int32_t *hit_offsets,
                          const int32_t *seed_offsets, int n_events, int max_event_hits_hint, const ds_tracks &out, int32_t *redo,
                          cudaStream_t st, Prof &prof);

@@ -118,6 +118,7 @@ struct EventCtx {
     const float2 *yb;      // (ymin, ymax) of each (layer, sector)
     const double2 *ye;     // (ymin - y_tol, ymax + y_tol) of each (layer, sector)
     bool uni;              // every hit carries the bounds of its (layer, sector)
+    int n_hits;            // hits of the event (checked build)
     int rsec;              // sectors looked at on either side of the one a track's y falls into
 };
 
@@ -161,6 +162,7 @@ __device__ __forceinline__ void ev_slices(const DevConst &c, const EventCtx &E, 
     const int base = (layer * c.n_sectors + sector) * kFine;
     a = E.tab[base + fl];
     b = E.tab[base + fh + 1];
+    DS_ASSERT(fl >= 0 && fl <= fh && fh < kFine && a <= b && b <= E.n_hits);
 }
 
 // S4: closest and second closest y-compatible hit of layer l within w1 of the prediction xp; -1 = none
@@ -189,6 +191,7 @@ __device__ __forceinline__ int2 ev_search(const DevConst &c, const EventCtx &E, 
             }
         }
     }
+    DS_ASSERT(j0 < E.n_hits && j1 < E.n_hits && (j0 < 0 || j0 != j1));
     return make_int2(j0, j1);
 }
 
@@ -307,6 +310,7 @@ __device__ __forceinline__ void ev_select_warp(const DevConst &c, const EventCtx
             const int ji = cj[i];
             int rank = 0;
             for (int q = 0; q < n_list; ++q) rank += (q != i && closer(H, cd[q], (int)cj[q], di, ji)) ? 1 : 0;
+            DS_ASSERT(rank >= 0 && rank < n_list);
             if (rank < max_first) sh.slot[o * kMaxFirst + rank] = (uint16_t)ji;
         }
     }
@@ -402,6 +406,7 @@ __device__ __forceinline__ void event_chunk(const DevConst &c, EventWarp &sh, co
             const int pos = incl - nFc;
             sh.foff[lane] = (unsigned short)pos;
             for (int k = 0; k < nFc; ++k) {
+                DS_ASSERT(pos + k < kFirstCap && (int)my_slot[k] < E.n_hits);
                 sh.fs[pos + k] = (unsigned short)(lane * kMaxFirst + k);
                 sh.z3[pos + k] = hit_z(H, (int)my_slot[k]);
             }
@@ -424,8 +429,7 @@ __device__ __forceinline__ void event_chunk(const DevConst &c, EventWarp &sh, co
                     const double xp = xm + txc * (c.z_layer[l] - zm);
                     int2 r = ev_search(c, E, l, xp, t2.y[l][o], w1, (unsigned)t2.mask[l][o]);
                     if (l == 0) r.y = -1;   // UTaX keeps the closest hit only
-                    sh.near[3 * f + l][0] = (uint16_t)r.x;
-                    sh.near[3 * f + l][1] = (uint16_t)r.y;
+                    *reinterpret_cast<uint32_t *>(&sh.near[3 * f + l][0]) = ((uint32_t)r.x & 0xffffu) | ((uint32_t)r.y << 16);
                     if (r.x >= 0) { hit_prefetch(H, r.x); ++nh; }
                     if (r.y >= 0) { hit_prefetch(H, r.y); if (l == 1) m1 = 2; else m2 = 2; }
                 }
@@ -434,6 +438,7 @@ __device__ __forceinline__ void event_chunk(const DevConst &c, EventWarp &sh, co
                     hit_prefetch(H, j3);
                     const int base = atomicAdd(&sh.n_fit, m1 * m2);
                     if (base + m1 * m2 <= kFitCap) {
+                        DS_ASSERT(base >= 0 && f < 512);
                         ff = (unsigned short)(base | ((m1 * m2) << 12));
                         for (int i1 = 0; i1 < m1; ++i1)
                             for (int i2 = 0; i2 < m2; ++i2)
@@ -513,6 +518,7 @@ __device__ __forceinline__ void ev_hist4(const DevConst &c, uint32_t *hist, floa
             const int sh16 = (b & 1) * 16;
             const uint32_t old = atomicAdd(&hist[b >> 1], 1u << sh16);
             const uint32_t slot = (old >> sh16) & 0xffffu;
+            DS_ASSERT(b >= 0 && b < c.n_bins * kSub && slot < 0xffffu);
             pk[u] = (int)(((uint32_t)b << 20) | slot);
             if (slot == 0) yb[b >> kFineLog2] = make_float2(lov[u], hiv[u]);   // reference bounds of the (layer, sector)
         }
@@ -552,6 +558,7 @@ __device__ __forceinline__ void ev_scatter4(const uint16_t *tab, const int32_t *
     for (int u = 0; u < 4; ++u) {
         const int k = k0 + u;
         if (kFull || (k >= d && k < kend)) {
+            DS_ASSERT(pos[u] >= 0 && pos[u] < kend - d);
             b_s[pos[u]] = xv[u];
             src[pos[u]] = (uint16_t)(k - d);
         }
@@ -682,6 +689,8 @@ k_event(const __grid_constant__ DevConst c, const ds_hits hits, const ds_seeds s
     E.yb = hd.yb;
     E.ye = hd.ye;
     E.uni = hd.nonuni == 0;
+    E.n_hits = n;
+    DS_ASSERT((int)tab[nfine] == n && (int)tab[0] == 0);
     E.rsec = c.y_rsec;
     EventWarp *warps = reinterpret_cast<EventWarp *>(smem + L.WS);
     const int chunk = seed_chunk<W>(s_begin, s_end);
@@ -738,14 +747,21 @@ cudaError_t launch_event(const DevConst &c, const ds_hits &hits, const ds_seeds 
     sm = event_layout<5>(cap, nfine).total;
     if (3 * (sm + kPerBlock) <= kSm + 1024)
         return launch_event_one<5, 3>(c, hits, seeds, hit_offsets, seed_offsets, n_events, cap, sm, bulk, out, redo, st, prof);
+    // two blocks per SM: the largest capacity that still fits them (event_kernel_wanted has checked that the hint does)
+    while (2 * (event_layout<8>(cap, nfine).total + kPerBlock) > kSm + 1024) cap -= 8;
     sm = event_layout<8>(cap, nfine).total;
-    if (2 * (sm + kPerBlock) <= kSm + 1024)
-        return launch_event_one<8, 2>(c, hits, seeds, hit_offsets, seed_offsets, n_events, cap, sm, bulk, out, redo, st, prof);
-    // one block per SM: the largest capacity that fits (positions are uint16); larger events are left to the other kernels
-    if (cap > 65528) cap = 65528;
-    while (event_layout<12>(cap, nfine).total > kSm - kPerBlock) cap -= 8;
-    sm = event_layout<12>(cap, nfine).total;
-    return launch_event_one<12, 1>(c, hits, seeds, hit_offsets, seed_offsets, n_events, cap, sm, bulk, out, redo, st, prof);
+    return launch_event_one<8, 2>(c, hits, seeds, hit_offsets, seed_offsets, n_events, cap, sm, bulk, out, redo, st, prof);
+}
+
+// k_event pays when at least two blocks share an SM (one block's loads and sort overlap the other's searches).  Events so
+// large that only one would fit (cfg2-like, 8 000 hits: measured 0.36 ms per 1000 events against 0.33 ms) run k_layout +
+// k_track, whose sort has the SM's full thread count to itself.
+bool event_kernel_wanted(const DevConst &c, int max_event_hits_hint)
+{
+    const int hint = max_event_hits_hint > 0 ? max_event_hits_hint : 4096;
+    const int cap = ((hint + 7) & ~7) + 8;
+    const size_t kSm = 227 * 1024, kPerBlock = 1024;
+    return 2 * (event_layout<8>(cap, c.n_bins * kSub).total + kPerBlock) <= kSm + 1024;
 }
 
 }  // namespace ds

@@ -17,9 +17,7 @@ constexpr int kSub = DS_KSUB;   // the sort cuts every x0 slice of the bin table
 __device__ __forceinline__ int fine_bin(const DevConst &c, int id, float x0)
 {
     int sec = min(id_sector(id), c.n_sectors - 1);
-    float t = floorf((x0 + c.xb_off) * c.xb_scale * (float)kSub);
-    t = fminf(fmaxf(t, 0.0f), (float)(kXBins * kSub - 1));
-    return (id_layer(id) * c.n_sectors + sec) * (kXBins * kSub) + (int)t;
+    return (id_layer(id) * c.n_sectors + sec) * (kXBins * kSub) + xslice<kXBins * kSub>(x0, c.xb_off, c.xb_scale);
 }
 
 // exclusive scan of v[0..n) in place (n <= a few thousand), v[n] = total.  All threads of the block call it.
