@@ -30,6 +30,8 @@ namespace ds {
 constexpr int kFine = kXBins * kSub;   // x0 slices per (layer, sector) of the sort = of the table the searches use here
 constexpr int kFineLog2 = kFine == 64 ? 6 : (kFine == 32 ? 5 : (kFine == 128 ? 7 : -1));
 static_assert((1 << kFineLog2) == kFine, "coarse bin = fine bin >> kFineLog2");
+constexpr int kEvFirstCap = 64;   // first hits a warp handles per round (96 / 128 / 160 measured: no faster, a round rarely overflows)
+static_assert(kEvFirstCap >= DS_MAX_FIRST_HITS && kEvFirstCap <= 512, "a seed's first hits fit a round; f packs into 9 bits");
 constexpr int kSelCap = 64;            // hits of an over-full first window that the warp ranks together
 
 // State of one warp of k_event (cf. WarpShared of ds_track.cuh; no fit results are kept: the lane that fits the best
@@ -52,15 +54,15 @@ struct SeedRecs {
 struct EventWarp {
     SeedRecs rec;
     unsigned long long best_bits[32];     // per seed: smallest score among its fits (bits of the non-negative double)
-    uint16_t near[3 * kFirstCap][2];      // phase B: closest / second closest hit of (first hit, layer); phase A: ranking lists
-    float z3[kFirstCap];                  // z of the first hit
+    uint16_t near[3 * kEvFirstCap][2];      // phase B: closest / second closest hit of (first hit, layer); phase A: ranking lists
+    float z3[kEvFirstCap];                  // z of the first hit
     int n_best[32];                       // per seed: fits with that score (+ 2 for every first hit left to the seed's thread)
     int n_fit;                            // fit tasks appended this round (may exceed kFitCap)
     int fit_end;                          // tasks [0, fit_end) are queued; later appends did not fit the queue
     uint16_t slot[32 * kMaxFirst];        // phase A: the seed's first hits (positions in the event's bin-ordered x0)
     unsigned short foff[32];              // where the seed's first hits start in the round's list
-    unsigned short fs[kFirstCap];         // first-hit list: index into slot[]
-    unsigned short ffit[kFirstCap];       // first fit task of the first hit (| combinations << 12), kFitNone or kFitInline
+    unsigned short fs[kEvFirstCap];         // first-hit list: index into slot[]
+    unsigned short ffit[kEvFirstCap];       // first fit task of the first hit (| combinations << 12), kFitNone or kFitInline
     unsigned short task[kFitCap];         // fit task: first hit | i1 << 9 | i2 << 10
 };
 static_assert(sizeof(EventWarp) % 8 == 0 && sizeof(EventWarp::near) >= kSelCap * (sizeof(double) + sizeof(uint16_t)), "ranking lists fit near[]");
@@ -119,7 +121,7 @@ struct EventCtx {
     const double2 *ye;     // (ymin - y_tol, ymax + y_tol) of each (layer, sector)
     bool uni;              // every hit carries the bounds of its (layer, sector)
     int n_hits;            // hits of the event (checked build)
-    int rsec;              // sectors looked at on either side of the one a track's y falls into
+    int rsec;              // sectors looked at on either side of the one a track's y falls into; 0: only the nearer neighbour
 };
 
 // Events whose hits do not all carry their sector's bounds (rare: out of line): the sectors a track at height y can touch;
@@ -140,8 +142,16 @@ __device__ __forceinline__ bool ev_y_hit(const DevConst &c, const float *gymin, 
 __device__ __forceinline__ unsigned ev_sector_mask(const DevConst &c, const EventCtx &E, int layer, double y)
 {
     if (!E.uni) return ev_sector_mask_any(c, layer, y);
-    const int sc = __double2int_rd((y - c.y0) * c.inv_h);   // NaN -> 0: the tests below then fail
-    const int lo = max(sc - E.rsec, 0), hi = min(sc + E.rsec, c.n_sectors - 1);
+    const double u = (y - c.y0) * c.inv_h;
+    const int sc = __double2int_rd(u);   // NaN -> 0: the tests below then fail
+    int lo = sc - E.rsec, hi = sc + E.rsec;
+    if (E.rsec == 0) {   // y_tol below half a sector: besides its own sector only the neighbour y is nearer to can be compatible
+        const bool upper = u - (double)sc >= 0.5;
+        lo = upper ? sc : sc - 1;
+        hi = upper ? sc + 1 : sc;
+    }
+    lo = max(lo, 0);
+    hi = min(hi, c.n_sectors - 1);
     unsigned m = 0;
 #pragma unroll 1
     for (int s = lo; s <= hi; ++s) {
@@ -398,7 +408,7 @@ __device__ __forceinline__ void event_chunk(const DevConst &c, EventWarp &sh, co
             if (lane >= d) incl += t;
         }
         // the seeds taken this round are the longest prefix whose first hits fit the list
-        const bool take = act && incl <= kFirstCap;
+        const bool take = act && incl <= kEvFirstCap;
         const unsigned take_mask = __ballot_sync(FULL, take);
         const int n_take = __popc(take_mask);
         const int n_first = __shfl_sync(FULL, incl, n_take - 1);
@@ -406,7 +416,7 @@ __device__ __forceinline__ void event_chunk(const DevConst &c, EventWarp &sh, co
             const int pos = incl - nFc;
             sh.foff[lane] = (unsigned short)pos;
             for (int k = 0; k < nFc; ++k) {
-                DS_ASSERT(pos + k < kFirstCap && (int)my_slot[k] < E.n_hits);
+                DS_ASSERT(pos + k < kEvFirstCap && (int)my_slot[k] < E.n_hits);
                 sh.fs[pos + k] = (unsigned short)(lane * kMaxFirst + k);
                 sh.z3[pos + k] = hit_z(H, (int)my_slot[k]);
             }
@@ -691,7 +701,7 @@ k_event(const __grid_constant__ DevConst c, const ds_hits hits, const ds_seeds s
     E.uni = hd.nonuni == 0;
     E.n_hits = n;
     DS_ASSERT((int)tab[nfine] == n && (int)tab[0] == 0);
-    E.rsec = c.y_rsec;
+    E.rsec = (c.y_rsec == 1 && c.y_tol * c.inv_h < 0.5) ? 0 : c.y_rsec;
     EventWarp *warps = reinterpret_cast<EventWarp *>(smem + L.WS);
     const int chunk = seed_chunk<W>(s_begin, s_end);
     for (int cb = s_begin + wid * chunk; cb < s_end; cb += W * chunk)
