@@ -93,7 +93,7 @@ __device__ __forceinline__ float mlp_forward(const Net<H1, H2> &m, const float (
 #pragma unroll
         for (int i = 0; i < DS_MLP_IN / 4; ++i) {
             const float4 q = w[i];
-            t += q.x * f[4 * i] + q.y * f[4 * i + 1] + q.z * f[4 * i + 2] + q.w * f[4 * i + 3];
+            t = fmaf(q.x, f[4 * i], t); t = fmaf(q.y, f[4 * i + 1], t); t = fmaf(q.z, f[4 * i + 2], t); t = fmaf(q.w, f[4 * i + 3], t);
         }
         h1[j] = t > 0.f ? t : 0.f;
     }
@@ -108,7 +108,7 @@ __device__ __forceinline__ float mlp_forward(const Net<H1, H2> &m, const float (
 #pragma unroll
             for (int i = 0; i < H1 / 4; ++i) {
                 const float4 q = w[i];
-                u += q.x * h1[4 * i] + q.y * h1[4 * i + 1] + q.z * h1[4 * i + 2] + q.w * h1[4 * i + 3];
+                u = fmaf(q.x, h1[4 * i], u); u = fmaf(q.y, h1[4 * i + 1], u); u = fmaf(q.z, h1[4 * i + 2], u); u = fmaf(q.w, h1[4 * i + 3], u);
             }
             h2[j] = u > 0.f ? u : 0.f;
         }
@@ -166,9 +166,26 @@ k_mlp(const __grid_constant__ DevConst c, const void *__restrict__ gm, const ds_
     const int64_t begin = ((int64_t)blockIdx.x * (kMlpThreads / 32) + wid) * kMlpSpan;
     const int64_t end = begin + kMlpSpan < trk.n ? begin + kMlpSpan : trk.n;
     int nq = 0;
-    for (int64_t base = begin; base < end; base += 32) {
+    // the found flags of the lane's kMlpSpan / 32 slots in one round of loads (one after the other they are a chain of
+    // DRAM latencies: the ballots below keep the compiler from hoisting them)
+    static_assert(kMlpSpan / 32 <= 32, "one bit per slot of the lane");
+    unsigned bits = 0;
+    {
+        int fl[kMlpSpan / 32];
+#pragma unroll
+        for (int u = 0; u < kMlpSpan / 32; ++u) {
+            const int64_t s = begin + u * 32 + lane;
+            fl[u] = s < end ? trk.found[s] : 0;
+        }
+#pragma unroll
+        for (int u = 0; u < kMlpSpan / 32; ++u) bits |= fl[u] != 0 ? 1u << u : 0u;
+    }
+#pragma unroll 1
+    for (int u = 0; u < kMlpSpan / 32; ++u) {
+        const int64_t base = begin + u * 32;
+        if (base >= end) break;
         const int64_t s = base + lane;
-        const bool f = s < end && trk.found[s] != 0;
+        const bool f = s < end && ((bits >> u) & 1u) != 0;
         if (s < end && !f) { trk.score[s] = 0.f; trk.keep[s] = 0; }
         const unsigned mask = __ballot_sync(0xffffffffu, f);
         if (f) q[nq + __popc(mask & lanemask_lt())] = (int)(s - begin);
