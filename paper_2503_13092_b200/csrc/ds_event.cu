@@ -601,6 +601,7 @@ k_event(const __grid_constant__ DevConst c, const ds_hits hits, const ds_seeds s
     int32_t *b_p = reinterpret_cast<int32_t *>(smem + L.P);
     uint16_t *src = reinterpret_cast<uint16_t *>(b_y);
     const uint16_t *tab = reinterpret_cast<const uint16_t *>(hist);
+    const bool stagers = !bulk || tid < 64;   // a bulk copy is issued by thread 0, the few elements after it by threads 32..34
     const int d = h0 & 3, kend = d + n;   // element i of the event sits at index d + i of a staged buffer
 
     if (tid == 0) {
@@ -608,18 +609,20 @@ k_event(const __grid_constant__ DevConst c, const ds_hits hits, const ds_seeds s
         for (int k = 0; k < 5; ++k) mbar_init(&hd.bars[k], 1);
         hd.nonuni = 0;
         if (bulk && n > 0) {   // w is read much later, for fitted hits only: bring the event's slice into L2 now;
-            const int a0 = h0 & ~3, a1 = (h0 + n + 3) & ~3;   // the arrays are padded by 4 elements (ds.h)
-            l2_prefetch(hits.w + a0, 4u * (uint32_t)(a1 - a0));
-            l2_prefetch(hits.z + a0, 4u * (uint32_t)(a1 - a0));   // z follows once the unsorted x0 has left its buffer
+            const int a0 = h0 & ~3, a1 = (h0 + n) & ~3;       // whole 16-byte groups inside the arrays
+            if (a1 > a0) {
+                l2_prefetch(hits.w + a0, 4u * (uint32_t)(a1 - a0));
+                l2_prefetch(hits.z + a0, 4u * (uint32_t)(a1 - a0));
+            }   // z follows once the unsorted x0 has left its buffer
         }
     }
     for (int k = tid; k < (nw + 4) / 4; k += T) reinterpret_cast<uint4 *>(hist)[k] = make_uint4(0u, 0u, 0u, 0u);
     if (tid < kLayers * DS_MAX_SECTORS) hd.yb[tid] = make_float2(0.f, 0.f);
     __syncthreads();
-    stage_words(b_z, hits.x0, h0, n, &hd.bars[0], bulk != 0);
-    stage_words(b_p, hits.id, h0, n, &hd.bars[1], bulk != 0);
-    stage_words(b_s, hits.ymin, h0, n, &hd.bars[2], bulk != 0);
-    stage_words(b_y, hits.ymax, h0, n, &hd.bars[3], bulk != 0);
+    if (stagers) stage_words(b_z, hits.x0, h0, n, &hd.bars[0], bulk != 0);
+    if (stagers) stage_words(b_p, hits.id, h0, n, &hd.bars[1], bulk != 0);
+    if (stagers) stage_words(b_s, hits.ymin, h0, n, &hd.bars[2], bulk != 0);
+    if (stagers) stage_words(b_y, hits.ymax, h0, n, &hd.bars[3], bulk != 0);
     // the lane's first seed, fetched now so that the load is in flight with the hits
     SeedPre pre;
     {
@@ -638,13 +641,19 @@ k_event(const __grid_constant__ DevConst c, const ds_hits hits, const ds_seeds s
     __syncthreads();
     // ---- B: exclusive scan of the counts, two 16-bit counts per word -> bin starts ---------------------------------------------
     {
-        const int per = ((nw + T - 1) / T) | 1;   // odd: the threads' runs start in different banks
-        const int kb = min(tid * per, nw), ke = min(kb + per, nw);
+        // a thread takes per4 neighbouring groups of four words (128-bit accesses; 12 words apart for 160 threads and 14
+        // sectors: no bank conflict) and keeps them in registers between the two passes
+        constexpr int kQ = (4 * DS_MAX_SECTORS * kFine / 8 + T - 1) / T;
+        const int nq = nw / 4, per4 = (nq + T - 1) / T;
+        uint4 *h4 = reinterpret_cast<uint4 *>(hist);
+        uint4 q[kQ];
         uint32_t sum = 0;
-#pragma unroll 1
-        for (int k = kb; k < ke; ++k) {
-            const uint32_t w = hist[k];
-            sum += (w & 0xffffu) + (w >> 16);
+#pragma unroll
+        for (int u = 0; u < kQ; ++u) {
+            const int idx = tid * per4 + u;
+            q[u] = (u < per4 && idx < nq) ? h4[idx] : make_uint4(0u, 0u, 0u, 0u);
+            sum += (q[u].x & 0xffffu) + (q[u].x >> 16) + (q[u].y & 0xffffu) + (q[u].y >> 16) + (q[u].z & 0xffffu) + (q[u].z >> 16) +
+                   (q[u].w & 0xffffu) + (q[u].w >> 16);
         }
         uint32_t inc = sum;
 #pragma unroll
@@ -657,11 +666,17 @@ k_event(const __grid_constant__ DevConst c, const ds_hits hits, const ds_seeds s
         __syncthreads();
         uint32_t run = inc - sum;
         for (int w = 0; w < wid; ++w) run += (uint32_t)ws[w];
-#pragma unroll 1
-        for (int k = kb; k < ke; ++k) {
-            const uint32_t w = hist[k], c0 = w & 0xffffu, c1 = w >> 16;
-            hist[k] = run | ((run + c0) << 16);
+        auto scan_word = [&run](uint32_t w) {
+            const uint32_t c0 = w & 0xffffu, c1 = w >> 16, r = run | ((run + c0) << 16);
             run += c0 + c1;
+            return r;
+        };
+#pragma unroll
+        for (int u = 0; u < kQ; ++u) {
+            const int idx = tid * per4 + u;
+            uint4 r;
+            r.x = scan_word(q[u].x); r.y = scan_word(q[u].y); r.z = scan_word(q[u].z); r.w = scan_word(q[u].w);
+            if (u < per4 && idx < nq) h4[idx] = r;
         }
         if (tid == T - 1) hist[nw] = run;   // tab[nfine] = n
     }
@@ -687,7 +702,7 @@ k_event(const __grid_constant__ DevConst c, const ds_hits hits, const ds_seeds s
     }
     __syncthreads();
     // the unsorted x0 is dead: its buffer takes z (by index inside the event); the searches start while it is in flight
-    stage_words(b_z, hits.z, h0, n, &hd.bars[4], bulk != 0);
+    if (stagers) stage_words(b_z, hits.z, h0, n, &hd.bars[4], bulk != 0);
     __syncthreads();   // its last elements come by ordinary stores
 
     // ---- S2..S6 on the shared-memory copy ---------------------------------------------------------------------------------------------
