@@ -228,7 +228,7 @@ int ds_extrapolate(ds_handle *h, const ds_seeds *seeds, const ds_params *p, doub
 /* ---- S1..S7: ds_reconstruct ------------------------------------------------------------------------------------ */
 
 /* Bytes of DEVICE workspace ds_reconstruct needs for a call of this size (the sorted SoA, permutation and bin
- * tables of S1).  Alignment required: 256 B. */
+ * tables of S1 for the events that take the two-kernel path, one flag per event).  Alignment required: 256 B. */
 size_t ds_workspace_bytes(const ds_handle *h, int n_events, int64_t n_hits, int64_t n_seeds);
 
 /* Layout (S1) -> per seed: extrapolate (S2), first window in UTbX keeping the <= max_first_hits closest hits (S3,
@@ -236,7 +236,12 @@ size_t ds_workspace_bytes(const ds_handle *h, int n_events, int64_t n_hits, int6
  * weighted line fit + chi2 of every combination with the magnet point as pseudo-measurement (S5, A-8), best
  * candidate by score with id tie-breaks (S6) -> ghost-killer MLP score and keep flag (S7).
  * All deciding arithmetic is fp64 in registers; the MLP is fp32 (a decision within 1e-3 of the threshold is
- * re-evaluated in fp64).  seed_offsets: DEVICE int32 [n_events+1]. */
+ * re-evaluated in fp64).  seed_offsets: DEVICE int32 [n_events+1].
+ * Launches: with dv1 = 0, S1..S6 run as one kernel per event that sorts the event's hits in shared memory and searches
+ * the copy it holds; events above the staging capacity derived from max_event_hits_hint (and every event when the hint
+ * is so large that fewer than two such blocks fit an SM, or with dv1 = 1) take a layout kernel and a search kernel through
+ * the workspace.  The results do not depend on which path an event takes.  Then clone killing (clone_min_shared > 0) and
+ * the ghost killer. */
 int ds_reconstruct(ds_handle *h, const ds_hits *hits, const ds_seeds *seeds, const int32_t *hit_offsets,
                    const int32_t *seed_offsets, int n_events, const ds_params *p, ds_tracks *out, void *workspace,
                    size_t workspace_bytes, void *cuda_stream);
@@ -287,7 +292,8 @@ int ds_process_host(ds_handle *h, const ds_hits *hits, const ds_seeds *seeds, co
 
 /* ---- per-kernel device timing (measurement aid; no effect on results) ------------------------------------------ */
 
-/* Kernels of the path, in launch order. */
+/* Kernels of the path.  DS_K_EVENT = S1..S6 in one kernel (ds_reconstruct, dv1 = 0); DS_K_LAYOUT / DS_K_TRACK = the same
+ * steps as two kernels (ds_layout; dv1 = 1; events DS_K_EVENT leaves over -- launched after it, empty if there are none). */
 enum { DS_K_LAYOUT = 0, DS_K_TRACK, DS_K_MLP, DS_K_VTX_COUNT, DS_K_VTX_SCAN, DS_K_VTX_WRITE, DS_K_CLONE, DS_K_LINES, DS_K_EVENT, DS_K_COUNT };
 
 typedef struct {
