@@ -389,7 +389,7 @@ k_vertex_write(const __grid_constant__ DevConst c, const ds_tracks trk, const in
 //                   and the sum of the counts of every group of kGroup events (atomicAdd)
 // k_vertex_write_w  warp per event: offset = counts of the earlier groups + counts of the earlier events of the group;
 //                   only the pairs whose mask bit is set are computed again and written, in pair order
-constexpr int kWThreads = 128;
+constexpr int kWThreads = 32;    // 32 / 64 / 128 / 256 measured on cfg4: 0.041 / 0.042 / 0.043 / 0.047 ms per 10 000 events
 constexpr int kWWarps = kWThreads / 32;
 constexpr int kWCap = 96;       // kept tracks of an event staged per warp
 constexpr int kGroup = 256;     // events per group sum
@@ -505,7 +505,7 @@ k_vertex_count_w(const __grid_constant__ DevConst c, const ds_tracks trk, const 
     }
 }
 
-constexpr int kW2Threads = 256;
+constexpr int kW2Threads = 32;   // 32 / 64 / 128 / 256 / 512 measured: 0.027 / 0.030 / 0.027 / 0.031 / 0.035 ms
 constexpr int kW2Warps = kW2Threads / 32;
 static_assert(kGroup % kW2Warps == 0, "a block of k_vertex_write_w stays inside one group");
 
