@@ -34,6 +34,7 @@ enum {
     DS_E_NOGEOM = -2,    /* ds_upload_geometry has not been called on this handle                       */
     DS_E_WORKSPACE = -3, /* workspace pointer NULL or workspace_bytes smaller than ds_*_workspace_bytes */
     DS_E_CUDA = -4,      /* a CUDA runtime call failed (no device, launch error, out of memory)         */
+    DS_E_LIMIT = -5,     /* ds_vertex_static: the call is larger than its fixed scratch (DS_STATIC_MAX_*) */
 };
 
 /* Ghost-killer architecture (BASELINE cfg0: 8 -> 32 -> 16 -> 1; the paper's own is 8 -> 14 -> 1).
@@ -266,6 +267,28 @@ size_t ds_vertex_workspace_bytes(const ds_handle *h, int n_events, int64_t n_see
  * are read.  Deciding arithmetic in fp64. */
 int ds_vertex(ds_handle *h, const ds_tracks *trk, const int32_t *seed_offsets, int n_events, const ds_params *p,
               ds_vertices *out, void *workspace, size_t workspace_bytes, void *cuda_stream);
+
+/* ---- ds_vertex without any allocation: the scratch is a fixed device array inside the library ------------------- */
+
+/* For callers that cannot allocate: code under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc.
+ * ds_vertex_static is ds_vertex (same kernels, same output, bit for bit) with its workspace in a file-scope
+ * `static __device__` array of DS_STATIC_SCRATCH_BYTES (4.03 MiB) that every GPU that loads the library holds until the
+ * process exits.  The caller passes inputs and outputs only.  It calls no cudaMalloc / cudaFree / allocating routine (the
+ * ds_profile_* event pairs are not recorded for it).
+ * Limits: n_events <= DS_STATIC_MAX_EVENTS and trk->n <= DS_STATIC_MAX_SEEDS, else DS_E_LIMIT (nothing is launched).
+ * Sharing: there is ONE array per device.  Every call uses it and finds the previous call's contents (what has to start
+ * at zero is cleared by the call itself, on its stream).  Calls that overlap on the GPU -- two streams, two handles or
+ * two threads on the same device -- race on it and corrupt each other's vertex lists: keep them on one stream, or order
+ * them with events.
+ * ds_vertex_static_setup resolves the array's device address for the handle's device (once per device; cheap when
+ * repeated).  ds_vertex_static does the same on its first call for a device; call the set-up beforehand if that first
+ * call must not touch the runtime (e.g. under stream capture). */
+#define DS_STATIC_MAX_EVENTS 2048
+#define DS_STATIC_MAX_SEEDS 524288
+#define DS_STATIC_SCRATCH_BYTES 4227072
+int ds_vertex_static_setup(ds_handle *h);
+int ds_vertex_static(ds_handle *h, const ds_tracks *trk, const int32_t *seed_offsets, int n_events, const ds_params *p,
+                     ds_vertices *out, void *cuda_stream);
 
 /* ---- HLT1 line NNs on the vertices (P:277-P:285, A-33) ------------------------------------------- */
 

@@ -1,6 +1,7 @@
 // C ABI of libds (include/ds.h): handle, argument checks, workspace carving, launch order, host-buffer path.
 // No arithmetic of the method lives here.
 #include <cstdlib>
+#include <mutex>
 #include <new>
 
 #include "ds_common.cuh"
@@ -22,7 +23,30 @@ struct ds_handle {
     Prof prof;
 };
 
+// Scratch of ds_vertex_static (include/ds.h): a fixed device array instead of a caller's workspace.  In host code this
+// name is only a stand-in for the symbol, never a device address: the address comes from cudaGetSymbolAddress (below).
+static __device__ __align__(256) unsigned char ds_static_scratch[DS_STATIC_SCRATCH_BYTES];
+
 namespace {
+
+// Device address of ds_static_scratch on device `dev`, which must be current: resolved once per device, then cached.
+std::mutex g_static_mu;
+void *g_static_ptr[64] = {};
+
+cudaError_t static_scratch_address(int dev, void **ptr)
+{
+    if (dev < 0 || dev >= 64) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(g_static_mu);
+    if (!g_static_ptr[dev]) {
+        void *p = nullptr;
+        const cudaError_t err = cudaGetSymbolAddress(&p, ds_static_scratch);
+        if (err != cudaSuccess) return err;
+        if (!p || (reinterpret_cast<uintptr_t>(p) & 255) != 0) return cudaErrorInvalidSymbol;
+        g_static_ptr[dev] = p;
+    }
+    *ptr = g_static_ptr[dev];
+    return cudaSuccess;
+}
 
 struct DeviceGuard {
     int prev = -1;
@@ -181,6 +205,7 @@ const char *ds_error_string(int code)
         case DS_E_NOGEOM: return "geometry not uploaded";
         case DS_E_WORKSPACE: return "workspace missing or too small";
         case DS_E_CUDA: return "CUDA error";
+        case DS_E_LIMIT: return "call larger than the fixed scratch of ds_vertex_static (DS_STATIC_MAX_EVENTS / DS_STATIC_MAX_SEEDS)";
         default: return "unknown error";
     }
 }
@@ -438,6 +463,47 @@ int ds_vertex(ds_handle *h, const ds_tracks *trk, const int32_t *seed_offsets, i
     DeviceGuard guard(h->device);
     if (!guard.ok) return DS_E_CUDA;
     if (launch_vertex(c, *trk, seed_offsets, n_events, *out, workspace, (cudaStream_t)cuda_stream, h->prof) != cudaSuccess) {
+        cudaGetLastError();
+        return DS_E_CUDA;
+    }
+    return DS_OK;
+}
+
+int ds_vertex_static_setup(ds_handle *h)
+{
+    if (!h) return DS_E_ARG;
+    DeviceGuard guard(h->device);
+    if (!guard.ok) return DS_E_CUDA;
+    void *scratch = nullptr;
+    if (static_scratch_address(h->device, &scratch) != cudaSuccess) {
+        cudaGetLastError();
+        return DS_E_CUDA;
+    }
+    return DS_OK;
+}
+
+int ds_vertex_static(ds_handle *h, const ds_tracks *trk, const int32_t *seed_offsets, int n_events, const ds_params *p,
+                     ds_vertices *out, void *cuda_stream)
+{
+    if (!h || !trk || trk->n < 0 || !seed_offsets || n_events < 0 || !vertices_ok(out)) return DS_E_ARG;
+    if (trk->n > 0 && !(trk->x && trk->y && trk->tx && trk->ty && trk->qop && trk->keep)) return DS_E_ARG;
+    if (!h->has_geom) return DS_E_NOGEOM;
+    DevConst c;
+    if (!make_const(h->geom, p, c)) return DS_E_ARG;
+    if (n_events > DS_STATIC_MAX_EVENTS || trk->n > DS_STATIC_MAX_SEEDS ||
+        vertex_workspace_bytes(n_events, trk->n) > (size_t)DS_STATIC_SCRATCH_BYTES)
+        return DS_E_LIMIT;
+    DeviceGuard guard(h->device);
+    if (!guard.ok) return DS_E_CUDA;
+    void *scratch = nullptr;
+    if (static_scratch_address(h->device, &scratch) != cudaSuccess) {
+        cudaGetLastError();
+        return DS_E_CUDA;
+    }
+    Prof none;   // never on: no event is created or recorded for these launches
+    // launch_vertex clears what has to start at zero (the group sums) on the stream, ahead of its kernels; everything
+    // else it reads of the scratch it has written in the same call
+    if (launch_vertex(c, *trk, seed_offsets, n_events, *out, scratch, (cudaStream_t)cuda_stream, none) != cudaSuccess) {
         cudaGetLastError();
         return DS_E_CUDA;
     }

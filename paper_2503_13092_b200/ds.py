@@ -16,7 +16,8 @@ import numpy as np
 
 from . import build as _build
 
-DS_OK, DS_E_ARG, DS_E_NOGEOM, DS_E_WORKSPACE, DS_E_CUDA = 0, -1, -2, -3, -4
+DS_OK, DS_E_ARG, DS_E_NOGEOM, DS_E_WORKSPACE, DS_E_CUDA, DS_E_LIMIT = 0, -1, -2, -3, -4, -5
+DS_STATIC_MAX_EVENTS, DS_STATIC_MAX_SEEDS, DS_STATIC_SCRATCH_BYTES = 2048, 524288, 4227072
 DS_MLP_IN, DS_MLP_H1, DS_MLP_H2 = 8, 32, 16
 DS_XBINS, DS_MAX_SECTORS, DS_MAX_FIRST_HITS = 16, 16, 10
 
@@ -152,6 +153,8 @@ def lib() -> ct.CDLL:
         L.ds_vertex_workspace_bytes.restype = ct.c_size_t
         L.ds_vertex.argtypes = [vp, ct.POINTER(DsTracks), vp, ct.c_int, ct.POINTER(DsParams), ct.POINTER(DsVertices),
                                 vp, ct.c_size_t, vp]
+        L.ds_vertex_static_setup.argtypes = [vp]
+        L.ds_vertex_static.argtypes = [vp, ct.POINTER(DsTracks), vp, ct.c_int, ct.POINTER(DsParams), ct.POINTER(DsVertices), vp]
         L.ds_process_host.argtypes = [vp, ct.POINTER(DsHits), ct.POINTER(DsSeeds), vp, vp, ct.c_int,
                                       ct.POINTER(DsParams), ct.POINTER(DsTracks), ct.POINTER(DsVertices),
                                       ct.POINTER(ct.c_int64), vp]
@@ -371,6 +374,17 @@ def ds_vertex(h, tracks, seed_offsets, n_events, params: DsParams, out, capacity
                            _stream_ptr(stream)), "ds_vertex")
 
 
+def ds_vertex_static_setup(h) -> None:
+    _check(lib().ds_vertex_static_setup(h), "ds_vertex_static_setup")
+
+
+def ds_vertex_static(h, tracks, seed_offsets, n_events, params: DsParams, out, capacity, stream=None) -> None:
+    """ds_vertex with the scratch in the library's fixed device array: no workspace argument, no allocation."""
+    ts, vs = _tracks(tracks), _vertices(out, capacity)
+    _check(lib().ds_vertex_static(h, ct.byref(ts), _ptr(seed_offsets), n_events, ct.byref(params), ct.byref(vs),
+                                  _stream_ptr(stream)), "ds_vertex_static")
+
+
 def _hp(a):
     """Host pointer of a numpy array or a (pinned) torch CPU tensor."""
     if a is None:
@@ -552,6 +566,11 @@ class Downstream:
         if workspace is None:
             workspace = self._on_stream(self.vertex_workspace(ne, tracks["x"].numel()), stream)
         ds_vertex(self.h, tracks, seed_offsets, ne, self.params, out, out["capacity"], workspace, stream)
+        return out
+
+    def vertex_static(self, tracks: dict, seed_offsets, out: dict, stream=None):
+        """ds_vertex_static: the caller's `out` (empty_vertices), the library's fixed scratch; allocates nothing."""
+        ds_vertex_static(self.h, tracks, seed_offsets, seed_offsets.numel() - 1, self.params, out, out["capacity"], stream)
         return out
 
     def process_host(self, hits: dict, seeds: dict, hit_offsets, seed_offsets, out_tracks: dict, out_vertices: dict,
