@@ -275,7 +275,7 @@ def test_cfg4_subbatch_sampled(ds, orc_mlp):
 # ---- variants of the parameters ---------------------------------------------------------------------------------------
 @pytest.mark.parametrize("override", [
     dict(max_first_hits=3), dict(min_hits=4), dict(mlp_keep_above=0, mlp_thr=0.5), dict(w0_b=400.0, w0_max=600.0),
-    dict(chi2ndf_max=1.0, miss_penalty=0.5), dict(y_tol=60.0), dict(doca_max=0.5, dm_ks=10.0, zv_min=1000.0),
+    dict(chi2ndf_max=1.0, miss_penalty=0.5), dict(y_tol=60.0), dict(y_tol=130.0), dict(doca_max=0.5, dm_ks=10.0, zv_min=1000.0),
 ])
 def test_parameter_variants(ds, orc_mlp, override):
     d = gen.generate(1, n_events=100)
